@@ -1,0 +1,167 @@
+/* swept.h — C ABI of the B200 swept time-space decomposition library (libswept_b200.so).
+ *
+ * The hot path of "Accelerating solutions of one-dimensional unsteady PDEs with GPU-based swept
+ * time-space decomposition" (arXiv 1705.03162; citations below are PAPER.md line numbers):
+ * explicit finite-difference / finite-volume time stepping of 1-D periodic PDEs, advanced either
+ *   - per step   ("Classic", Fig. 6): one kernel launch per sub-timestep,
+ *                working array in global memory; or
+ *   - swept      (§4.2, §4.3): UpTriangle, then alternating
+ *                SplitDiamond / WholeDiamond, then DownTriangle; each thread block advances one tile of
+ *                `tile_width` points through its whole domain of dependence on chip; only the two-row
+ *                edge state goes through HBM between launches; the tiling
+ *                shifts by half a tile each phase.
+ * Both variants evaluate the same IEEE expression trees, so their results are bit-identical
+ * ("the swept rule performs the same operations in a different order and location").
+ *
+ * Conventions
+ *   - Every function is extern "C"; no exception crosses the boundary; no torch type appears.
+ *   - "host" pointers are ordinary host memory (pageable or pinned), caller-owned.
+ *     "device" pointers are CUDA device memory.
+ *   - Field layout: component-major C arrays of N REALs.  heat/KS: u[N].  Euler: rho[N], rho*u[N], E[N]
+ *     (E = total energy per volume; Eq. D.2 PAPER.md:366 with reading X4 of DESIGN.md).
+ *     REAL is double (SWEPT_F64) or float (SWEPT_F32).
+ *   - All work is enqueued on the state's stream (swept_set_stream); swept_run never synchronises.
+ *   - Return codes: 0 ok; SWEPT_EINVAL bad argument; SWEPT_EUNSUPPORTED unsupported combination;
+ *     SWEPT_ECUDA CUDA error (text in swept_last_error); SWEPT_ENOMEM allocation failed.
+ *   - A swept_state is not thread-safe; distinct states are independent (multi-GPU = one state per
+ *     device, "replicas only": the paper's method is single-GPU).
+ *   - There is no CPU fallback: without a CUDA device every compute call fails with SWEPT_ECUDA.
+ */
+#ifndef SWEPT_H_
+#define SWEPT_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct swept_state swept_state; /* opaque; owns its device buffers */
+
+enum { SWEPT_HEAT = 0, SWEPT_KS = 1, SWEPT_EULER = 2 };     /* problem (App. B-D)  */
+enum { SWEPT_PER_STEP = 0, SWEPT_SWEPT = 1 };               /* variant                           */
+enum { SWEPT_F64 = 0, SWEPT_F32 = 1 };                      /* dtype                             */
+enum { SWEPT_RK2_MIDPOINT = 0, SWEPT_RK2_HEUN = 1 };        /* KS/Euler integrator (
+                                                               Heun is BASELINE.json config 4)   */
+enum { SWEPT_OK = 0, SWEPT_EINVAL = -1, SWEPT_EUNSUPPORTED = -2, SWEPT_ECUDA = -3, SWEPT_ENOMEM = -4 };
+
+/* swept kernel flavours (how a tile is evaluated on chip; results are identical) */
+enum {
+  SWEPT_FLAVOR_AUTO = 0,  /* library picks (autotuned value if swept_autotune was run)                 */
+  SWEPT_FLAVOR_TIER = 1,  /* one CTA per tile, two-row working array in shared memory, one block barrier
+                             per tier (the paper's "Shared" arrangement, re-sized)        */
+  SWEPT_FLAVOR_CHAR = 2   /* register-resident sweep along characteristics: a lane group per tile,
+                             halo exchange by warp shuffles only, no block barrier       */
+};
+
+/* Optional device allocator hooks (so that PyTorch's caching allocator owns the memory).
+ * alloc returns a device pointer or NULL; both are called on the thread that calls swept_create/destroy. */
+typedef void* (*swept_alloc_fn)(void* ctx, uint64_t nbytes);
+typedef void (*swept_free_fn)(void* ctx, void* device_ptr);
+
+typedef struct {
+  uint32_t struct_size; /* = sizeof(swept_params); ABI versioning                                    */
+  int32_t dtype;        /* SWEPT_F64 (default) or SWEPT_F32                                          */
+  int32_t rk2;          /* SWEPT_RK2_*; ignored for heat                                             */
+  int32_t device;       /* CUDA ordinal, -1 = current device                                         */
+  double alpha;         /* heat diffusivity (Eq. B.1)                                  */
+  double gamma;         /* Euler heat-capacity ratio, 1.4                             */
+  void* stream;         /* cudaStream_t used by all calls on this state (NULL = legacy default stream) */
+  swept_alloc_fn alloc; /* NULL = cudaMalloc                                                         */
+  swept_free_fn free;   /* NULL = cudaFree                                                           */
+  void* alloc_ctx;      /* passed back to alloc/free                                                 */
+} swept_params;
+
+/* swept_create — set up one problem: N periodic points, spacing dx, fixed timestep dt.
+ * Scheme constants are computed once, in double, on the host (Fo = alpha dt/dx^2; etc.) and
+ * rounded once to REAL.  p may be NULL (FP64, midpoint, alpha = 1, gamma = 1.4, current device).
+ * Requires N >= 32 (and N >= 8 for per-step only use), dx > 0, dt > 0.  Returns NULL on error. */
+swept_state* swept_create(int problem, int64_t N, double dx, double dt, const swept_params* p);
+
+/* swept_write — copy initial data from HOST memory (C*N REALs, layout above) to the device, asynchronously
+ * on the state's stream (the host buffer must stay valid until the stream reaches the copy; pageable
+ * memory makes the call synchronous).  Resets the step counter. */
+int swept_write(swept_state* s, const void* host_buf);
+
+/* swept_write_device — same, from DEVICE memory (device-to-device copy on the stream). */
+int swept_write_device(swept_state* s, const void* device_buf);
+
+/* swept_run — advance by nsteps full timesteps (PAPER.md:236 counts timesteps; KS/Euler timesteps have two
+ * sub-timesteps).
+ *   variant SWEPT_PER_STEP: tile_width = threads per block of the per-step kernel (32..1024, power of two;
+ *                           0 = library default).
+ *   variant SWEPT_SWEPT   : tile_width = n = spatial points per tile ("node"), a power of two,
+ *                           32 <= n <= 4096 (the paper sweeps 32..1024), n >= 16 h for the
+ *                           5-point problems, N % n == 0; 0 = autotuned / default value.
+ *                           The run is Up, D diamonds, Down, covering the largest T = (D+1) n/(2h)
+ *                           sub-timesteps that fit, and the remainder is finished with per-step stages
+ *                           (readout granularity; reading G5).  If N has no admissible tile
+ *                           the call fails with SWEPT_EUNSUPPORTED.
+ * Asynchronous on the state's stream; launch errors surface at the next synchronising call. */
+int swept_run(swept_state* s, int64_t nsteps, int32_t tile_width, int variant);
+
+/* swept_run_flavor — swept_run with an explicit swept kernel flavour (SWEPT_FLAVOR_*). */
+int swept_run_flavor(swept_state* s, int64_t nsteps, int32_t tile_width, int variant, int flavor);
+
+/* swept_read — synchronise the stream and copy the current field to HOST memory (same layout as
+ * swept_write). */
+int swept_read(swept_state* s, void* host_buf);
+
+/* swept_device_ptr — DEVICE pointer to the current full time level (C*N REALs), valid until the next
+ * swept_run/swept_write on this state; stream-ordered (no synchronisation). */
+const void* swept_device_ptr(swept_state* s);
+
+/* swept_autotune — time short runs over admissible tile widths (and flavours) for `variant`
+ * (the paper also keeps the best block size per N), restore the field, remember and return
+ * the best tile width.  Synchronises. */
+int swept_autotune(swept_state* s, int variant, int32_t* best_tile_width);
+
+/* swept_tuned — what swept_autotune remembered for `variant`: tile width, swept flavour and its group
+ * parameter (TIER: points per thread; CHAR: lanes per tile); zeros if autotune has not run. */
+int swept_tuned(const swept_state* s, int variant, int32_t* tile_width, int32_t* flavor, int32_t* group);
+
+/* swept_set_stream — change the stream used by subsequent calls (cudaStream_t). */
+int swept_set_stream(swept_state* s, void* stream);
+
+/* swept_steps_done — timesteps advanced since the last swept_write. */
+int64_t swept_steps_done(const swept_state* s);
+
+/* swept_last_launches — number of kernel launches (graph nodes included) issued by the last swept_run. */
+int64_t swept_last_launches(const swept_state* s);
+
+void swept_destroy(swept_state* s);
+
+/* swept_last_error — thread-local message of the last failing call on this thread. */
+const char* swept_last_error(void);
+
+/* ---- host-only helpers (no GPU needed) ------------------------------------------------------------ */
+
+/* One phase of the swept schedule: kind 0 Up, 1 SplitDiamond, 2 WholeDiamond, 3 Down,
+ * 4 per-step remainder.  `shift` = offset of the tiling in points (0 or n/2), `tier0` = global sub-timestep
+ * index at which the phase's relative tier 0 sits, `ntiers` = tiers it computes at its tallest column. */
+typedef struct {
+  int32_t kind;
+  int32_t shift;
+  int64_t tier0;
+  int64_t ntiers;
+} swept_phase;
+
+/* swept_plan — the phase list swept_run would execute for nsub = sigma*nsteps sub-timesteps with tile width
+ * n and stencil half-width h.  Writes at most max_phases entries, returns the number of phases needed
+ * (or a negative error code). */
+int64_t swept_plan(int64_t nsub, int32_t n, int32_t h, swept_phase* out, int64_t max_phases);
+
+/* ---- measurement helpers --------------------------------------------------------------------------- */
+
+/* swept_probe_fp64 — run a register-only DFMA chain on every SM of `device` and return FP64 pipe
+ * instructions per second (warp-instructions * 32 lanes), i.e. the measured ALU roofline denominator. */
+int swept_probe_fp64(int device, void* stream, double* fp64_lane_ops_per_s);
+
+/* swept_probe_launch — average cost in microseconds of launching an empty kernel `count` times
+ * back to back on `stream` (PAPER.md:253 measures the same on the K40c: about 4 us). */
+int swept_probe_launch(int device, void* stream, int count, double* us_per_launch);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SWEPT_H_ */

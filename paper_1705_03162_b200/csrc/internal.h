@@ -1,0 +1,49 @@
+// internal.h — host-side launcher interface between swept_api.cu and the per-problem kernel files.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace swept {
+
+struct PerStepLaunch {
+  const void* in;
+  const void* base;
+  void* out;
+  int64_t N;
+  int odd;
+  int threads;  // threads per block
+  int P;        // points per thread (N % P == 0)
+  const double* consts;  // 5 doubles, rounded once to REAL by the launcher
+  cudaStream_t stream;
+};
+
+struct TileLaunch {
+  int kind;  // KIND_*
+  const void* in0;
+  const void* in1;
+  void* out0;
+  void* out1;
+  int64_t N;
+  int n, shift, ntiers;
+  int P;       // TIER: points per thread.  CHAR: lanes per tile (L)
+  int flavor;  // SWEPT_FLAVOR_TIER / SWEPT_FLAVOR_CHAR
+  const double* consts;
+  cudaStream_t stream;
+};
+
+// dtype: 0 f64, 1 f32.  rk2: 0 midpoint, 1 Heun.  Return cudaError_t as int, or -1000 if the
+// combination has no kernel.
+int launch_per_step_heat(int dtype, const PerStepLaunch& a);
+int launch_per_step_ks(int dtype, int rk2, const PerStepLaunch& a);
+int launch_per_step_euler(int dtype, int rk2, const PerStepLaunch& a);
+int launch_tile_heat(int dtype, const TileLaunch& a);
+int launch_tile_ks(int dtype, int rk2, const TileLaunch& a);
+int launch_tile_euler(int dtype, int rk2, const TileLaunch& a);
+// does a kernel exist for (flavor, n, P)?  (host-only query used by the autotuner and argument checks)
+bool tile_config_ok_heat(int dtype, int flavor, int n, int P);
+bool tile_config_ok_ks(int dtype, int flavor, int n, int P);
+bool tile_config_ok_euler(int dtype, int flavor, int n, int P);
+
+constexpr int NO_KERNEL = -1000;
+
+}  // namespace swept

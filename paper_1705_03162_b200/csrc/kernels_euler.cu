@@ -1,0 +1,19 @@
+// kernels_euler.cu — Euler equations / Sod tube (App. D) kernel instantiations, FP64.
+#include "kernels_impl.cuh"
+namespace swept {
+int launch_per_step_euler(int dtype, int rk2, const PerStepLaunch& a) {
+  if (dtype != 0) return NO_KERNEL;
+  return rk2 == 0 ? per_step_T<Euler<double, 0>, 2>(a) : per_step_T<Euler<double, 1>, 2>(a);
+}
+bool tile_config_ok_euler(int dtype, int flavor, int n, int P) {
+  if (dtype != 0) return false;
+  if (flavor == SWEPT_FLAVOR_TIER) return tier_ok<Euler<double, 0>>(n, P, 2);
+  return false;
+}
+int launch_tile_euler(int dtype, int rk2, const TileLaunch& a) {
+  if (dtype != 0) return NO_KERNEL;
+  if (a.flavor == SWEPT_FLAVOR_TIER)
+    return rk2 == 0 ? tier_T<Euler<double, 0>, 2>(a) : tier_T<Euler<double, 1>, 2>(a);
+  return NO_KERNEL;
+}
+}  // namespace swept

@@ -1,0 +1,15 @@
+// kernels_heat.cu — heat equation (App. B) kernel instantiations, FP64 and FP32.
+#include "kernels_impl.cuh"
+namespace swept {
+int launch_per_step_heat(int dtype, const PerStepLaunch& a) {
+  return dtype == 0 ? per_step_T<Heat<double>, 4>(a) : per_step_T<Heat<float>, 4>(a);
+}
+bool tile_config_ok_heat(int dtype, int flavor, int n, int P) {
+  if (flavor == SWEPT_FLAVOR_TIER) return dtype == 0 ? tier_ok<Heat<double>>(n, P, 4) : tier_ok<Heat<float>>(n, P, 4);
+  return false;
+}
+int launch_tile_heat(int dtype, const TileLaunch& a) {
+  if (a.flavor == SWEPT_FLAVOR_TIER) return dtype == 0 ? tier_T<Heat<double>, 4>(a) : tier_T<Heat<float>, 4>(a);
+  return NO_KERNEL;
+}
+}  // namespace swept

@@ -1,0 +1,84 @@
+// per_step.cuh — the per-step ("Classic") kernel: one launch per sub-timestep, working array in global
+// memory (Fig. 6).  SURVEY.md §8(a) row a0.
+//
+// B200 layout: each thread advances P contiguous points; the P-point body of the window is one (or two)
+// 16-byte vector loads, the 2h halo values are scalar loads that hit L1 (they are the neighbours' bodies);
+// the periodic wrap (PAPER.md:196-201 uses `& lastidx`, which needs N = 2^k) is a compare-and-add so any
+// N divisible by P works.  Algorithmic traffic per point and sub-timestep: C*sizeof(R) read + the same
+// written (+ the same again for the final stage's base read).
+#pragma once
+#include "functors.cuh"
+
+namespace swept {
+
+template <class R, int P>
+__device__ __forceinline__ void load_vec(const R* __restrict__ p, R (&v)[P]) {
+  if constexpr (sizeof(R) * P >= 16 && (sizeof(R) * P) % 16 == 0) {
+    constexpr int NV = (int)(sizeof(R) * P / 16);
+    const int4* q = reinterpret_cast<const int4*>(p);
+    int4 t[NV];
+#pragma unroll
+    for (int i = 0; i < NV; ++i) t[i] = __ldg(q + i);
+#pragma unroll
+    for (int i = 0; i < NV; ++i) reinterpret_cast<int4*>(v)[i] = t[i];
+  } else {
+#pragma unroll
+    for (int i = 0; i < P; ++i) v[i] = __ldg(p + i);
+  }
+}
+template <class R, int P>
+__device__ __forceinline__ void store_vec(R* __restrict__ p, const R (&v)[P]) {
+  if constexpr (sizeof(R) * P >= 16 && (sizeof(R) * P) % 16 == 0) {
+    constexpr int NV = (int)(sizeof(R) * P / 16);
+#pragma unroll
+    for (int i = 0; i < NV; ++i) reinterpret_cast<int4*>(p)[i] = reinterpret_cast<const int4*>(v)[i];
+  } else {
+#pragma unroll
+    for (int i = 0; i < P; ++i) p[i] = v[i];
+  }
+}
+
+// in: stage input (tier t-1), base: tier t-2 field (only read when SIGMA == 2 and !odd), out: tier t.
+template <class Prob, int P>
+__global__ void __launch_bounds__(1024)
+per_step_kernel(const typename Prob::R* __restrict__ in, const typename Prob::R* __restrict__ base,
+                typename Prob::R* __restrict__ out, int64_t N, int odd, Consts<typename Prob::R> k) {
+  using R = typename Prob::R;
+  constexpr int H = Prob::H, C = Prob::C;
+  const int64_t i0 = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) * P;
+  if (i0 >= N) return;
+  alignas(16) R win[C][P + 2 * H];
+  alignas(16) R bs[C][P];
+  alignas(16) R o[C][P];
+#pragma unroll
+  for (int c = 0; c < C; ++c) {
+    const R* src = in + (int64_t)c * N;
+    alignas(16) R body[P];
+    load_vec<R, P>(src + i0, body);
+#pragma unroll
+    for (int j = 0; j < P; ++j) win[c][H + j] = body[j];
+#pragma unroll
+    for (int j = 0; j < H; ++j) {
+      int64_t il = i0 - H + j;
+      if (il < 0) il += N;
+      int64_t ir = i0 + P + j;
+      if (ir >= N) ir -= N;
+      win[c][j] = __ldg(src + il);
+      win[c][H + P + j] = __ldg(src + ir);
+    }
+  }
+  if (Prob::SIGMA == 2 && !odd) {
+#pragma unroll
+    for (int c = 0; c < C; ++c) load_vec<R, P>(base + (int64_t)c * N + i0, bs[c]);
+  } else {
+#pragma unroll
+    for (int c = 0; c < C; ++c)
+#pragma unroll
+      for (int j = 0; j < P; ++j) bs[c][j] = win[c][H + j];
+  }
+  Prob::template stage<P>(win, bs, o, odd, k);
+#pragma unroll
+  for (int c = 0; c < C; ++c) store_vec<R, P>(out + (int64_t)c * N + i0, o[c]);
+}
+
+}  // namespace swept

@@ -1,0 +1,540 @@
+// swept_api.cu — the C ABI declared in include/swept.h: state, phase driver,
+// per-step driver with CUDA-graph replay, autotuner (row a8) and measurement probes.
+//
+// Nothing here touches the field values on the host except the explicit copies of swept_write/read;
+// there is no CPU fallback: every compute path is a kernel launch.
+#include <cuda_runtime.h>
+
+#include <algorithm>
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <map>
+#include <string>
+#include <tuple>
+#include <vector>
+
+#include "../../include/swept.h"
+#include "internal.h"
+
+namespace {
+
+thread_local std::string g_err;
+
+int fail(int code, const char* fmt, ...) {
+  char buf[512];
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(buf, sizeof buf, fmt, ap);
+  va_end(ap);
+  g_err = buf;
+  return code;
+}
+#define CUDA_TRY(expr)                                                                      \
+  do {                                                                                      \
+    cudaError_t e_ = (expr);                                                                \
+    if (e_ != cudaSuccess)                                                                  \
+      return fail(e_ == cudaErrorMemoryAllocation ? SWEPT_ENOMEM : SWEPT_ECUDA, "%s: %s", #expr, \
+                  cudaGetErrorString(e_));                                                  \
+  } while (0)
+
+constexpr int KIND_UP = 0, KIND_SPLIT = 1, KIND_WHOLE = 2, KIND_DOWN = 3, KIND_REMAINDER = 4;
+
+struct ProblemShape {
+  int h, sigma, C;
+};
+const ProblemShape kShape[3] = {{1, 1, 1}, {2, 2, 1}, {2, 2, 3}};
+
+struct GraphKey {
+  int threads, P, cur, steps;
+  bool operator<(const GraphKey& o) const {
+    return std::tie(threads, P, cur, steps) < std::tie(o.threads, o.P, o.cur, o.steps);
+  }
+};
+
+}  // namespace
+
+struct swept_state {
+  int problem = 0, dtype = 0, rk2 = 0, device = 0;
+  int64_t N = 0;
+  double dx = 0, dt = 0, alpha = 1, gamma = 1.4;
+  double consts[5] = {0, 0, 0, 0, 0};
+  cudaStream_t stream = nullptr;
+  cudaStream_t capture_stream = nullptr;  // graphs are recorded here (the legacy default stream cannot capture)
+  swept_alloc_fn alloc = nullptr;
+  swept_free_fn free_ = nullptr;
+  void* alloc_ctx = nullptr;
+  size_t slab_bytes = 0;
+  void* slab[4] = {nullptr, nullptr, nullptr, nullptr};
+  int cur = 0;  // slab holding the current full time level
+  int64_t steps_done = 0, last_launches = 0;
+  // autotune results: [variant] -> tile width, flavour, P
+  int tuned_width[2] = {0, 0};
+  int tuned_flavor = 0, tuned_P = 0;
+  std::map<GraphKey, cudaGraphExec_t> graphs;
+  size_t elem() const { return dtype == SWEPT_F64 ? 8 : 4; }
+};
+
+namespace {
+
+using swept::NO_KERNEL;
+
+int set_device(const swept_state* s) {
+  CUDA_TRY(cudaSetDevice(s->device));
+  return 0;
+}
+
+int launch_per_step(swept_state* s, const void* in, const void* base, void* out, int odd, int threads, int P) {
+  swept::PerStepLaunch a{in, base, out, s->N, odd, threads, P, s->consts, s->stream};
+  int rc;
+  switch (s->problem) {
+    case SWEPT_HEAT: rc = swept::launch_per_step_heat(s->dtype, a); break;
+    case SWEPT_KS: rc = swept::launch_per_step_ks(s->dtype, s->rk2, a); break;
+    default: rc = swept::launch_per_step_euler(s->dtype, s->rk2, a); break;
+  }
+  if (rc == NO_KERNEL) return fail(SWEPT_EUNSUPPORTED, "no per-step kernel for this problem/dtype/P=%d", P);
+  if (rc != 0) return fail(SWEPT_ECUDA, "per-step launch: %s", cudaGetErrorString((cudaError_t)rc));
+  return 0;
+}
+
+int launch_tile(swept_state* s, swept::TileLaunch& a) {
+  a.N = s->N;
+  a.consts = s->consts;
+  a.stream = s->stream;
+  int rc;
+  switch (s->problem) {
+    case SWEPT_HEAT: rc = swept::launch_tile_heat(s->dtype, a); break;
+    case SWEPT_KS: rc = swept::launch_tile_ks(s->dtype, s->rk2, a); break;
+    default: rc = swept::launch_tile_euler(s->dtype, s->rk2, a); break;
+  }
+  if (rc == NO_KERNEL)
+    return fail(SWEPT_EUNSUPPORTED, "no swept kernel for flavor=%d n=%d P=%d", a.flavor, a.n, a.P);
+  if (rc != 0) return fail(SWEPT_ECUDA, "swept launch: %s", cudaGetErrorString((cudaError_t)rc));
+  return 0;
+}
+
+bool tile_ok(const swept_state* s, int flavor, int n, int P) {
+  if (n <= 0 || s->N % n != 0) return false;
+  switch (s->problem) {
+    case SWEPT_HEAT: return swept::tile_config_ok_heat(s->dtype, flavor, n, P);
+    case SWEPT_KS: return swept::tile_config_ok_ks(s->dtype, flavor, n, P);
+    default: return swept::tile_config_ok_euler(s->dtype, flavor, n, P);
+  }
+}
+
+int per_step_P(const swept_state* s) {
+  const int pmax = s->problem == SWEPT_EULER ? 2 : 4;
+  for (int P = pmax; P > 1; P /= 2)
+    if (s->N % P == 0 && (s->N / P) >= 32) return P;
+  return 1;
+}
+
+// ---- per-step driver --------------------------------------------------------------------------------
+// One timestep = sigma launches.  Buffers: cur -> (pred) -> nxt, then cur and nxt swap, so an even number
+// of steps returns to the same buffer assignment and a captured chunk can be replayed.
+int enqueue_steps(swept_state* s, int64_t steps, int threads, int P, int* cur_io) {
+  const int sigma = kShape[s->problem].sigma;
+  int cur = *cur_io;
+  int nxt = (cur + 1) & 3, pred = (cur + 2) & 3;
+  for (int64_t i = 0; i < steps; ++i) {
+    if (sigma == 1) {
+      if (int rc = launch_per_step(s, s->slab[cur], s->slab[cur], s->slab[nxt], 0, threads, P)) return rc;
+    } else {
+      if (int rc = launch_per_step(s, s->slab[cur], s->slab[cur], s->slab[pred], 1, threads, P)) return rc;
+      if (int rc = launch_per_step(s, s->slab[pred], s->slab[cur], s->slab[nxt], 0, threads, P)) return rc;
+    }
+    std::swap(cur, nxt);
+  }
+  *cur_io = cur;
+  return 0;
+}
+
+int run_per_step(swept_state* s, int64_t steps, int threads) {
+  if (steps <= 0) return 0;
+  const int sigma = kShape[s->problem].sigma;
+  const int P = per_step_P(s);
+  if (threads == 0) threads = 256;
+  if (threads < 32 || threads > 1024 || (threads & (threads - 1)))
+    return fail(SWEPT_EINVAL, "per-step tile_width (threads per block) must be a power of two in 32..1024");
+  // replay chunks of CH steps from a captured graph (CH even so the buffer assignment is periodic)
+  const int64_t CH = 256;
+  int64_t left = steps;
+  while (left >= CH) {
+    GraphKey key{threads, P, s->cur, (int)CH};
+    auto it = s->graphs.find(key);
+    if (it == s->graphs.end()) {
+      cudaGraph_t g = nullptr;
+      if (!s->capture_stream) CUDA_TRY(cudaStreamCreateWithFlags(&s->capture_stream, cudaStreamNonBlocking));
+      CUDA_TRY(cudaStreamBeginCapture(s->capture_stream, cudaStreamCaptureModeThreadLocal));
+      int cur = s->cur;
+      cudaStream_t user_stream = s->stream;
+      s->stream = s->capture_stream;
+      int rc = enqueue_steps(s, CH, threads, P, &cur);
+      s->stream = user_stream;
+      cudaError_t e = cudaStreamEndCapture(s->capture_stream, &g);
+      if (rc) {
+        if (g) cudaGraphDestroy(g);
+        return rc;
+      }
+      if (e != cudaSuccess) return fail(SWEPT_ECUDA, "graph capture: %s", cudaGetErrorString(e));
+      cudaGraphExec_t ge = nullptr;
+      e = cudaGraphInstantiate(&ge, g, 0);
+      cudaGraphDestroy(g);
+      if (e != cudaSuccess) return fail(SWEPT_ECUDA, "graph instantiate: %s", cudaGetErrorString(e));
+      it = s->graphs.emplace(key, ge).first;
+    }
+    CUDA_TRY(cudaGraphLaunch(it->second, s->stream));
+    left -= CH;  // CH even: s->cur unchanged
+    s->last_launches += CH * sigma;
+  }
+  if (left > 0) {
+    int cur = s->cur;
+    if (int rc = enqueue_steps(s, left, threads, P, &cur)) return rc;
+    s->cur = cur;
+    s->last_launches += left * sigma;
+  }
+  return 0;
+}
+
+// ---- swept phase plan -------------------------------------------------------------------------------
+int64_t make_plan(int64_t nsub, int n, int h, std::vector<swept_phase>* out) {
+  if (n < 4 * h || (n & (n - 1)) || nsub < 0) return SWEPT_EINVAL;
+  const int64_t m = n / (2 * h);
+  int64_t done = 0;
+  if (nsub >= m) {
+    const int64_t D = nsub / m - 1;
+    out->push_back({KIND_UP, 0, 0, m - 1});
+    for (int64_t k = 1; k <= D; ++k) {
+      const bool split = (k & 1) != 0;
+      out->push_back({split ? KIND_SPLIT : KIND_WHOLE, split ? n / 2 : 0, (k - 1) * m, 2 * m - 1});
+    }
+    out->push_back({KIND_DOWN, (D & 1) ? 0 : n / 2, D * m, m});
+    done = (D + 1) * m;
+  }
+  if (nsub > done) out->push_back({KIND_REMAINDER, 0, done, nsub - done});
+  return (int64_t)out->size();
+}
+
+void default_tile(const swept_state* s, int* n_io, int* flavor_io, int* P_io) {
+  int n = *n_io, flavor = *flavor_io, P = *P_io;
+  if (n == 0 && s->tuned_width[SWEPT_SWEPT]) {
+    n = s->tuned_width[SWEPT_SWEPT];
+    if (flavor == SWEPT_FLAVOR_AUTO) {
+      flavor = s->tuned_flavor;
+      P = s->tuned_P;
+    }
+  }
+  if (n == 0) {
+    for (int cand : {256, 512, 128, 1024, 64, 32, 2048, 4096})
+      if (s->N % cand == 0) {
+        n = cand;
+        break;
+      }
+  }
+  if (flavor == SWEPT_FLAVOR_AUTO) {
+    flavor = SWEPT_FLAVOR_TIER;
+    P = 0;
+  }
+  if (P == 0) {
+    if (flavor == SWEPT_FLAVOR_TIER) {
+      const int pmax = s->problem == SWEPT_EULER ? 2 : 4;
+      P = std::min(pmax, std::max(1, n / 256));
+      while (P < pmax && n / P > 1024) P *= 2;
+      if (P == 3) P = 2;
+    }
+  }
+  *n_io = n;
+  *flavor_io = flavor;
+  *P_io = P;
+}
+
+int run_swept(swept_state* s, int64_t nsteps, int n, int flavor, int P) {
+  const ProblemShape sh = kShape[s->problem];
+  default_tile(s, &n, &flavor, &P);
+  if (n <= 0) return fail(SWEPT_EUNSUPPORTED, "N=%lld has no admissible tile width", (long long)s->N);
+  if (!tile_ok(s, flavor, n, P))
+    return fail(s->N % n ? SWEPT_EINVAL : SWEPT_EUNSUPPORTED,
+                "tile_width=%d (flavor %d, P=%d) not admissible for N=%lld", n, flavor, P, (long long)s->N);
+  std::vector<swept_phase> plan;
+  const int64_t np = make_plan(nsteps * sh.sigma, n, sh.h, &plan);
+  if (np < 0) return fail(SWEPT_EINVAL, "cannot plan tile_width=%d", n);
+  int r0 = -1, r1 = -1;  // slabs holding the current two-row state
+  for (const swept_phase& ph : plan) {
+    if (ph.kind == KIND_REMAINDER) {
+      if (int rc = run_per_step(s, ph.ntiers / sh.sigma, 0)) return rc;
+      continue;
+    }
+    swept::TileLaunch a{};
+    a.kind = ph.kind;
+    a.n = n;
+    a.shift = ph.shift;
+    a.ntiers = (int)ph.ntiers;
+    a.P = P;
+    a.flavor = flavor;
+    int o0, o1;
+    if (ph.kind == KIND_UP) {
+      o0 = (s->cur + 1) & 3;
+      o1 = (s->cur + 2) & 3;
+      a.in0 = s->slab[s->cur];
+      a.in1 = nullptr;
+    } else {
+      // the two slabs that are not the input rows
+      int f[2], k = 0;
+      for (int i = 0; i < 4; ++i)
+        if (i != r0 && i != r1) f[k++] = i;
+      o0 = f[0];
+      o1 = f[1];
+      a.in0 = s->slab[r0];
+      a.in1 = s->slab[r1];
+    }
+    a.out0 = s->slab[o0];
+    a.out1 = s->slab[o1];
+    if (int rc = launch_tile(s, a)) return rc;
+    s->last_launches += 1;
+    r0 = o0;
+    r1 = o1;
+    if (ph.kind == KIND_DOWN) s->cur = o0;  // row0 holds the full time level (T is even)
+  }
+  return 0;
+}
+
+}  // namespace
+
+// =======================================================================================================
+extern "C" {
+
+const char* swept_last_error(void) { return g_err.c_str(); }
+
+swept_state* swept_create(int problem, int64_t N, double dx, double dt, const swept_params* p) {
+  if (problem < 0 || problem > 2) { fail(SWEPT_EINVAL, "unknown problem %d", problem); return nullptr; }
+  if (N < 8 || N > (int64_t)1 << 31) { fail(SWEPT_EINVAL, "N out of range"); return nullptr; }
+  if (!(dx > 0) || !(dt > 0)) { fail(SWEPT_EINVAL, "dx and dt must be positive"); return nullptr; }
+  swept_params q;
+  std::memset(&q, 0, sizeof q);
+  q.struct_size = sizeof q;
+  q.dtype = SWEPT_F64;
+  q.device = -1;
+  q.alpha = 1.0;
+  q.gamma = 1.4;
+  if (p) {
+    if (p->struct_size < 4 || p->struct_size > sizeof q) { fail(SWEPT_EINVAL, "bad params.struct_size"); return nullptr; }
+    std::memcpy(&q, p, p->struct_size);
+  }
+  if (q.dtype != SWEPT_F64 && q.dtype != SWEPT_F32) { fail(SWEPT_EINVAL, "bad dtype"); return nullptr; }
+  if (q.rk2 != SWEPT_RK2_MIDPOINT && q.rk2 != SWEPT_RK2_HEUN) { fail(SWEPT_EINVAL, "bad rk2"); return nullptr; }
+  if (q.dtype == SWEPT_F32 && problem != SWEPT_HEAT) {
+    fail(SWEPT_EUNSUPPORTED, "FP32 is provided for the heat problem only (BASELINE.json config 2)");
+    return nullptr;
+  }
+  if ((q.alloc == nullptr) != (q.free == nullptr)) { fail(SWEPT_EINVAL, "alloc and free must be given together"); return nullptr; }
+  int dev = q.device;
+  if (dev < 0) {
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) { fail(SWEPT_ECUDA, "cudaGetDevice: %s (no CPU fallback exists)", cudaGetErrorString(e)); return nullptr; }
+  }
+  {
+    cudaError_t e = cudaSetDevice(dev);
+    if (e != cudaSuccess) { fail(SWEPT_ECUDA, "cudaSetDevice(%d): %s (no CPU fallback exists)", dev, cudaGetErrorString(e)); return nullptr; }
+  }
+  swept_state* s = new swept_state();
+  s->problem = problem; s->dtype = q.dtype; s->rk2 = q.rk2; s->device = dev;
+  s->N = N; s->dx = dx; s->dt = dt; s->alpha = q.alpha; s->gamma = q.gamma;
+  s->stream = (cudaStream_t)q.stream;
+  s->alloc = q.alloc; s->free_ = q.free; s->alloc_ctx = q.alloc_ctx;
+  // scheme constants: double on the host, rounded once to REAL at launch
+  if (problem == SWEPT_HEAT) {
+    const double Fo = q.alpha * dt / (dx * dx);
+    s->consts[0] = Fo;
+    s->consts[1] = 1.0 - 2.0 * Fo;
+  } else if (problem == SWEPT_KS) {
+    s->consts[0] = 1.0 / (4.0 * dx);
+    s->consts[1] = 1.0 / (dx * dx);
+    s->consts[2] = 1.0 / ((dx * dx) * (dx * dx));
+    s->consts[3] = dt;
+    s->consts[4] = 0.5 * dt;
+  } else {
+    const double lam = dt / dx;
+    s->consts[0] = q.gamma - 1.0;
+    s->consts[1] = q.gamma * (q.gamma - 1.0);
+    s->consts[2] = lam;
+    s->consts[3] = 0.5 * lam;
+  }
+  s->slab_bytes = (size_t)kShape[problem].C * (size_t)N * s->elem();
+  for (int i = 0; i < 4; ++i) {
+    void* ptr = nullptr;
+    if (s->alloc) {
+      ptr = s->alloc(s->alloc_ctx, s->slab_bytes);
+    } else if (cudaMalloc(&ptr, s->slab_bytes) != cudaSuccess) {
+      ptr = nullptr;
+      cudaGetLastError();
+    }
+    if (!ptr) {
+      fail(SWEPT_ENOMEM, "device allocation of %zu bytes failed", s->slab_bytes);
+      swept_destroy(s);
+      return nullptr;
+    }
+    if (((uintptr_t)ptr & 15) != 0) {
+      s->slab[i] = ptr;
+      fail(SWEPT_EINVAL, "allocator returned a pointer that is not 16-byte aligned");
+      swept_destroy(s);
+      return nullptr;
+    }
+    s->slab[i] = ptr;
+  }
+  return s;
+}
+
+void swept_destroy(swept_state* s) {
+  if (!s) return;
+  cudaSetDevice(s->device);
+  cudaStreamSynchronize(s->stream);
+  for (auto& kv : s->graphs) cudaGraphExecDestroy(kv.second);
+  if (s->capture_stream) cudaStreamDestroy(s->capture_stream);
+  for (int i = 0; i < 4; ++i) {
+    if (!s->slab[i]) continue;
+    if (s->free_) s->free_(s->alloc_ctx, s->slab[i]);
+    else cudaFree(s->slab[i]);
+  }
+  delete s;
+}
+
+int swept_set_stream(swept_state* s, void* stream) {
+  if (!s) return fail(SWEPT_EINVAL, "null state");
+  s->stream = (cudaStream_t)stream;
+  return 0;
+}
+
+int swept_write(swept_state* s, const void* host_buf) {
+  if (!s || !host_buf) return fail(SWEPT_EINVAL, "null argument");
+  if (int rc = set_device(s)) return rc;
+  CUDA_TRY(cudaMemcpyAsync(s->slab[s->cur], host_buf, s->slab_bytes, cudaMemcpyHostToDevice, s->stream));
+  s->steps_done = 0;
+  return 0;
+}
+
+int swept_write_device(swept_state* s, const void* device_buf) {
+  if (!s || !device_buf) return fail(SWEPT_EINVAL, "null argument");
+  if (int rc = set_device(s)) return rc;
+  CUDA_TRY(cudaMemcpyAsync(s->slab[s->cur], device_buf, s->slab_bytes, cudaMemcpyDeviceToDevice, s->stream));
+  s->steps_done = 0;
+  return 0;
+}
+
+int swept_read(swept_state* s, void* host_buf) {
+  if (!s || !host_buf) return fail(SWEPT_EINVAL, "null argument");
+  if (int rc = set_device(s)) return rc;
+  CUDA_TRY(cudaMemcpyAsync(host_buf, s->slab[s->cur], s->slab_bytes, cudaMemcpyDeviceToHost, s->stream));
+  CUDA_TRY(cudaStreamSynchronize(s->stream));
+  return 0;
+}
+
+const void* swept_device_ptr(swept_state* s) { return s ? s->slab[s->cur] : nullptr; }
+int64_t swept_steps_done(const swept_state* s) { return s ? s->steps_done : -1; }
+int64_t swept_last_launches(const swept_state* s) { return s ? s->last_launches : -1; }
+
+int swept_run_flavor(swept_state* s, int64_t nsteps, int32_t tile_width, int variant, int flavor) {
+  if (!s) return fail(SWEPT_EINVAL, "null state");
+  if (nsteps < 0) return fail(SWEPT_EINVAL, "nsteps must be >= 0");
+  if (tile_width < 0) return fail(SWEPT_EINVAL, "tile_width must be >= 0");
+  if (int rc = set_device(s)) return rc;
+  s->last_launches = 0;
+  int rc;
+  if (variant == SWEPT_PER_STEP) {
+    int tw = tile_width ? tile_width : s->tuned_width[SWEPT_PER_STEP];
+    rc = run_per_step(s, nsteps, tw);
+  } else if (variant == SWEPT_SWEPT) {
+    int fl = flavor & 0xff, P = (flavor >> 8) & 0xff;  // bits 8..15: explicit P / lane-group size (0 = default)
+    if (fl != SWEPT_FLAVOR_AUTO && fl != SWEPT_FLAVOR_TIER && fl != SWEPT_FLAVOR_CHAR)
+      return fail(SWEPT_EINVAL, "unknown flavor %d", fl);
+    rc = run_swept(s, nsteps, tile_width, fl, P);
+  } else {
+    return fail(SWEPT_EINVAL, "unknown variant %d", variant);
+  }
+  if (rc == 0) s->steps_done += nsteps;
+  return rc;
+}
+
+int swept_run(swept_state* s, int64_t nsteps, int32_t tile_width, int variant) {
+  return swept_run_flavor(s, nsteps, tile_width, variant, SWEPT_FLAVOR_AUTO);
+}
+
+int64_t swept_plan(int64_t nsub, int32_t n, int32_t h, swept_phase* out, int64_t max_phases) {
+  if (h != 1 && h != 2) return fail(SWEPT_EINVAL, "h must be 1 or 2");
+  std::vector<swept_phase> plan;
+  const int64_t np = make_plan(nsub, n, h, &plan);
+  if (np < 0) return fail(SWEPT_EINVAL, "tile width %d not plannable for h=%d", n, h);
+  if (out)
+    for (int64_t i = 0; i < np && i < max_phases; ++i) out[i] = plan[(size_t)i];
+  return np;
+}
+
+int swept_tuned(const swept_state* s, int variant, int32_t* tile_width, int32_t* flavor, int32_t* group) {
+  if (!s || (variant != SWEPT_PER_STEP && variant != SWEPT_SWEPT)) return fail(SWEPT_EINVAL, "bad argument");
+  if (tile_width) *tile_width = s->tuned_width[variant];
+  if (flavor) *flavor = variant == SWEPT_SWEPT ? s->tuned_flavor : 0;
+  if (group) *group = variant == SWEPT_SWEPT ? s->tuned_P : 0;
+  return 0;
+}
+
+int swept_autotune(swept_state* s, int variant, int32_t* best_tile_width) {
+  if (!s) return fail(SWEPT_EINVAL, "null state");
+  if (variant != SWEPT_PER_STEP && variant != SWEPT_SWEPT) return fail(SWEPT_EINVAL, "unknown variant");
+  if (int rc = set_device(s)) return rc;
+  const ProblemShape sh = kShape[s->problem];
+  // keep the field: the trial runs scribble over all four slabs
+  void* backup = nullptr;
+  CUDA_TRY(cudaMalloc(&backup, s->slab_bytes));
+  cudaMemcpyAsync(backup, s->slab[s->cur], s->slab_bytes, cudaMemcpyDeviceToDevice, s->stream);
+  const int64_t saved_steps = s->steps_done;
+  cudaEvent_t e0, e1;
+  cudaEventCreate(&e0);
+  cudaEventCreate(&e1);
+  double best = 1e300;
+  int best_n = 0, best_fl = 0, best_P = 0;
+  struct Cand { int n, fl, P; };
+  std::vector<Cand> cands;
+  if (variant == SWEPT_PER_STEP) {
+    for (int t = 32; t <= 1024; t *= 2) cands.push_back({t, 0, 0});
+  } else {
+    for (int n = 32; n <= 4096; n *= 2)
+      for (int fl : {SWEPT_FLAVOR_TIER, SWEPT_FLAVOR_CHAR})
+        for (int P : {1, 2, 4, 8, 16, 32})
+          if (tile_ok(s, fl, n, P)) cands.push_back({n, fl, P});
+  }
+  int rc_final = 0;
+  for (const Cand& c : cands) {
+    // enough steps for Up + >= 4 diamonds + Down at this width (and a few graph chunks for per-step)
+    int64_t steps;
+    if (variant == SWEPT_PER_STEP) steps = 512;
+    else steps = std::max<int64_t>(6 * (c.n / (2 * sh.h)) / sh.sigma, 64);
+    double t_best = 1e300;
+    for (int rep = 0; rep < 3; ++rep) {  // rep 0 warms up (graph capture, attribute setting)
+      cudaMemcpyAsync(s->slab[s->cur], backup, s->slab_bytes, cudaMemcpyDeviceToDevice, s->stream);
+      cudaEventRecord(e0, s->stream);
+      int rc = variant == SWEPT_PER_STEP ? run_per_step(s, steps, c.n) : run_swept(s, steps, c.n, c.fl, c.P);
+      cudaEventRecord(e1, s->stream);
+      if (rc) { rc_final = rc; break; }
+      if (cudaEventSynchronize(e1) != cudaSuccess) { rc_final = fail(SWEPT_ECUDA, "autotune trial failed: %s", cudaGetErrorString(cudaGetLastError())); break; }
+      float ms = 0;
+      cudaEventElapsedTime(&ms, e0, e1);
+      if (rep > 0) t_best = std::min(t_best, (double)ms / (double)steps);
+    }
+    if (rc_final) break;
+    if (t_best < best) { best = t_best; best_n = c.n; best_fl = c.fl; best_P = c.P; }
+  }
+  cudaMemcpyAsync(s->slab[s->cur], backup, s->slab_bytes, cudaMemcpyDeviceToDevice, s->stream);
+  cudaStreamSynchronize(s->stream);
+  cudaFree(backup);
+  cudaEventDestroy(e0);
+  cudaEventDestroy(e1);
+  s->steps_done = saved_steps;
+  if (rc_final) return rc_final;
+  if (best_n == 0) return fail(SWEPT_EUNSUPPORTED, "no admissible tile width for N=%lld", (long long)s->N);
+  s->tuned_width[variant] = best_n;
+  if (variant == SWEPT_SWEPT) { s->tuned_flavor = best_fl; s->tuned_P = best_P; }
+  if (best_tile_width) *best_tile_width = best_n;
+  return 0;
+}
+
+}  // extern "C"

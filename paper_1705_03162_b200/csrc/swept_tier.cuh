@@ -1,0 +1,163 @@
+// swept_tier.cuh — swept kernels, flavour TIER: one CTA per tile ("node"), the two-row
+// working array of PAPER.md:97-99 staged in shared memory, one block barrier per tier.
+//
+// SURVEY.md §8(a) rows a1 (UpTriangle), a3 (SplitDiamond), a4 (WholeDiamond), a5 (DownTriangle); the
+// inter-launch state is row a2: two global rows, row0[x] / row1[x] = latest even- / odd-tier value at x
+// (the paper's L/R edge arrays, re-expressed with the same bytes).
+//
+// A tile starting at S = shift + blockIdx.x * n (periodic; the last shifted tile wraps across the
+// boundary = the paper's boundary-split node) does:
+//   1. TMA 1-D bulk copies (cp.async.bulk, mbarrier completion) of row0/row1[S, S+n) into shared memory,
+//      plus 2h halo values per row with plain loads (the widest tier reads [S-h, S+n+h));
+//   2. tiers t = 1..ntiers: each thread owns P contiguous points, reads its (P+2h)-wide window of the other
+//      row, applies the stencil functor, overwrites its own row where the tier is active (interior values
+//      are overwritten once used, edges survive: PAPER.md:97); __syncthreads() per tier;
+//        Up:       tier t covers [S + h t, S + n - h t),           t = 1 .. m-1
+//        Diamond:  tier t covers [c - h t, c + h t) for t <= m and
+//                  [c - h(2m-t), c + h(2m-t)) for t > m,            t = 1 .. 2m-1
+//        Down:     tier t covers [c - h t, c + h t),                t = 1 .. m
+//      with c = S + n/2 and m = n/(2h);
+//   3. TMA bulk stores of both rows (Down: row0 only = the full time level) to the OTHER global buffer
+//      (phases ping-pong between two 2 x N buffers, SURVEY.md §8(d) note).
+#pragma once
+#include "common.cuh"
+#include "functors.cuh"
+
+namespace swept {
+
+enum { KIND_UP = 0, KIND_SPLIT = 1, KIND_WHOLE = 2, KIND_DOWN = 3 };
+
+template <class R>
+struct TierArgs {
+  const R* in0;  // row0 of the input buffer (C components, stride N)
+  const R* in1;  // row1 of the input buffer (unused by Up)
+  R* out0;
+  R* out1;  // unused by Down
+  int64_t N;
+  int n;       // tile width in points
+  int shift;   // 0 or n/2
+  int ntiers;  // tiers to compute
+  Consts<R> k;
+};
+
+template <int KIND>
+__device__ __forceinline__ void tier_range(int t, int n, int h, int m, int& lo, int& hi) {
+  if (KIND == KIND_UP) {
+    lo = h * t;
+    hi = n - h * t;
+  } else {
+    const int w = (KIND == KIND_DOWN || t <= m) ? h * t : h * (2 * m - t);
+    lo = n / 2 - w;
+    hi = n / 2 + w;
+  }
+}
+
+template <class Prob, int P, int KIND>
+__global__ void __launch_bounds__(1024) swept_tier_kernel(const TierArgs<typename Prob::R> a) {
+  using R = typename Prob::R;
+  constexpr int H = Prob::H, C = Prob::C, PAD = Pad16<R>::value;
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  const int n = a.n;
+  const int RS = n + 2 * PAD;  // padded row stride: body starts 16 bytes in
+  R* rows = reinterpret_cast<R*>(smem_raw);
+  uint64_t* mbar = reinterpret_cast<uint64_t*>(smem_raw + (size_t)2 * C * RS * sizeof(R));
+  const int64_t N = a.N;
+  const int tid = threadIdx.x;
+  int64_t S = (int64_t)a.shift + (int64_t)blockIdx.x * n;
+  if (S >= N) S -= N;
+  const int len1 = (int)((N - S) < (int64_t)n ? (N - S) : (int64_t)n);  // part before the periodic wrap
+  const int len2 = n - len1;
+  constexpr int NROWS_IN = (KIND == KIND_UP) ? 1 : 2;
+
+  if (tid == 0) {
+    mbar_init(mbar, 1);
+    fence_mbar_init();
+  }
+  __syncthreads();
+  if (tid == 0) {
+    mbar_arrive_expect_tx(mbar, (uint32_t)(NROWS_IN * C * n * sizeof(R)));
+#pragma unroll
+    for (int r = 0; r < NROWS_IN; ++r) {
+      const R* src = r == 0 ? a.in0 : a.in1;
+#pragma unroll
+      for (int c = 0; c < C; ++c) {
+        R* dst = rows + (r * C + c) * RS + PAD;
+        bulk_g2s(dst, src + (int64_t)c * N + S, (uint32_t)(len1 * sizeof(R)), mbar);
+        if (len2 > 0) bulk_g2s(dst + len1, src + (int64_t)c * N, (uint32_t)(len2 * sizeof(R)), mbar);
+      }
+    }
+  }
+  if (KIND == KIND_UP) {
+    // tier -1 does not exist: give row1 a defined value (its edge slots are stored but never used)
+    for (int i = tid; i < C * RS; i += blockDim.x) rows[C * RS + i] = (R)0;
+  } else {
+    // halo: H points either side of the tile, both rows, plain loads (periodic)
+    for (int i = tid; i < 2 * C * 2 * H; i += blockDim.x) {
+      const int r = i / (C * 2 * H), c = (i / (2 * H)) % C, j = i % (2 * H);
+      const R* src = (r == 0 ? a.in0 : a.in1) + (int64_t)c * N;
+      int64_t g = (j < H) ? (S - H + j) : (S + n + (j - H));
+      if (g < 0) g += N;
+      if (g >= N) g -= N;
+      const int s = (j < H) ? (PAD - H + j) : (PAD + n + (j - H));
+      rows[(r * C + c) * RS + s] = src[g];
+    }
+  }
+  mbar_wait(mbar, 0);
+  __syncthreads();
+
+  const int m = n / (2 * H);
+  const int j0 = tid * P;
+  for (int t = 1; t <= a.ntiers; ++t) {
+    const int par = t & 1;  // phases start on even global tiers (m is even): odd = predictor
+    const R* src = rows + (1 - par) * C * RS + PAD;
+    R* dst = rows + par * C * RS + PAD;
+    int lo, hi;
+    tier_range<KIND>(t, n, H, m, lo, hi);
+    if (j0 < hi && j0 + P > lo) {
+      R win[C][P + 2 * H], bs[C][P], o[C][P];
+#pragma unroll
+      for (int c = 0; c < C; ++c)
+#pragma unroll
+        for (int q = 0; q < P + 2 * H; ++q) win[c][q] = src[c * RS + j0 - H + q];
+#pragma unroll
+      for (int c = 0; c < C; ++c)
+#pragma unroll
+        for (int j = 0; j < P; ++j)
+          bs[c][j] = (Prob::SIGMA == 2 && !par) ? dst[c * RS + j0 + j] : win[c][H + j];
+      Prob::template stage<P>(win, bs, o, par, a.k);
+#pragma unroll
+      for (int j = 0; j < P; ++j)
+        if (j0 + j >= lo && j0 + j < hi) {
+#pragma unroll
+          for (int c = 0; c < C; ++c) dst[c * RS + j0 + j] = o[c][j];
+        }
+    }
+    __syncthreads();
+  }
+
+  fence_proxy_async_smem();
+  __syncthreads();
+  if (tid == 0) {
+    constexpr int NROWS_OUT = (KIND == KIND_DOWN) ? 1 : 2;
+#pragma unroll
+    for (int r = 0; r < NROWS_OUT; ++r) {
+      R* dstg = r == 0 ? a.out0 : a.out1;
+#pragma unroll
+      for (int c = 0; c < C; ++c) {
+        const R* s = rows + (r * C + c) * RS + PAD;
+        bulk_s2g(dstg + (int64_t)c * N + S, s, (uint32_t)(len1 * sizeof(R)));
+        if (len2 > 0) bulk_s2g(dstg + (int64_t)c * N, s + len1, (uint32_t)(len2 * sizeof(R)));
+      }
+    }
+    bulk_commit();
+    bulk_wait_all();
+  }
+}
+
+template <class Prob>
+inline size_t tier_smem_bytes(int n) {
+  using R = typename Prob::R;
+  return (size_t)2 * Prob::C * (n + 2 * Pad16<R>::value) * sizeof(R) + 16;
+}
+
+}  // namespace swept

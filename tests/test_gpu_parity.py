@@ -1,0 +1,214 @@
+"""GPU parity (run with -m gpu on the B200): the CUDA path, called through the C ABI, against the CPU oracle
+on the same seeded inputs, and swept against per-step bit for bit.
+
+Tolerances (north_star): max relative error <= 1e-12 in FP64 and <= 1e-5 in FP32 after the full run, where
+"relative" is ||gpu - oracle||_inf / ||oracle||_inf per component (reading X14) and the FP32 path is gated
+against the FP32 instantiation of the oracle (reading X15).  Because both sides evaluate the same IEEE
+expression trees the expected difference is exactly zero; the tests record that too.
+"""
+import numpy as np
+import pytest
+
+import oracle
+import paper_1705_03162_b200 as sw
+import swept_inputs as si
+
+pytestmark = pytest.mark.gpu
+
+TOL = {np.dtype(np.float64): 1e-12, np.dtype(np.float32): 1e-5}
+
+
+def relerr(got, ref, C):
+    got = got.reshape(C, -1).astype(np.float64)
+    ref = ref.reshape(C, -1).astype(np.float64)
+    return max(np.max(np.abs(g - r)) / max(np.max(np.abs(r)), 1e-300) for g, r in zip(got, ref))
+
+
+def gpu_run(w, nsteps, variant, tile_width=0, flavor=sw.FLAVOR_AUTO, group=0, dtype=np.float64):
+    s = sw.Swept.from_workload(w, dtype=dtype)
+    try:
+        s.run(nsteps, tile_width, variant, flavor, group)
+        out = s.read()
+        launches = s.last_launches
+    finally:
+        s.close()
+    return out, launches
+
+
+def check(w, nsteps, tile_widths, dtype=np.float64, flavors=((sw.FLAVOR_TIER, 0),), exact=True):
+    C = w.components
+    ref = oracle.run_workload(w, nsteps=nsteps, dtype=dtype)
+    ps, _ = gpu_run(w, nsteps, sw.PER_STEP, dtype=dtype)
+    tol = TOL[np.dtype(dtype)]
+    assert np.all(np.isfinite(ps))
+    assert relerr(ps, ref, C) <= tol, f"per_step vs oracle: {relerr(ps, ref, C)}"
+    if exact:
+        assert np.array_equal(ps, ref), "same expression trees: expected 0 ulp"
+    for n in tile_widths:
+        for fl, grp in flavors:
+            sx, _ = gpu_run(w, nsteps, sw.SWEPT, n, fl, grp, dtype=dtype)
+            assert np.array_equal(sx, ps), f"swept(n={n}, flavor={fl}, group={grp}) != per_step bitwise"
+            assert relerr(sx, ref, C) <= tol
+
+
+# ---------------------------------------------------------------- small cases spanning several tiles
+@pytest.mark.parametrize("N,nsteps", [(256, 0), (256, 7), (256, 64), (512, 333), (96, 50)])
+def test_heat_small(N, nsteps):
+    w = si.heat_sines(N, 8, 11, nsteps)
+    widths = [n for n in (32, 64, 128, 256) if N % n == 0]
+    check(w, nsteps, widths, flavors=((sw.FLAVOR_TIER, 1), (sw.FLAVOR_TIER, 2)))
+
+
+@pytest.mark.parametrize("rk2", [si.RK2_MIDPOINT, si.RK2_HEUN])
+@pytest.mark.parametrize("N,nsteps", [(256, 5), (512, 100), (1024, 77)])
+def test_ks_small(N, nsteps, rk2):
+    w = si.ks_cos(N, 5, nsteps)
+    w.rk2 = rk2
+    check(w, nsteps, [32, 64, 256], flavors=((sw.FLAVOR_TIER, 1), (sw.FLAVOR_TIER, 2), (sw.FLAVOR_TIER, 4)))
+
+
+@pytest.mark.parametrize("rk2", [si.RK2_MIDPOINT, si.RK2_HEUN])
+@pytest.mark.parametrize("N,nsteps", [(256, 3), (512, 150)])
+def test_euler_small(N, nsteps, rk2):
+    w = si.euler_double_sod(N, nsteps, rk2=rk2)
+    check(w, nsteps, [32, 128, 256], flavors=((sw.FLAVOR_TIER, 1), (sw.FLAVOR_TIER, 2)))
+
+
+def test_euler_random_data():
+    N = 384
+    w = si.euler_double_sod(N, 40)
+    w.u0 = si.random_smooth(si.EULER, N, 123)
+    w.dt = 0.1 * w.dx
+    check(w, 40, [32, 64, 128])
+
+
+def test_single_tile_wraps_onto_itself():
+    # N == n: the one shifted tile is split across the periodic boundary
+    for w in (si.heat_sines(64, 4, 3, 200), si.ks_cos(64, 3, 60)):
+        check(w, w.nsteps, [64])
+
+
+def test_heat_fp32():
+    w = si.heat_sines(1024, 16, 21, 500)
+    check(w, 500, [32, 128, 1024], dtype=np.float32, flavors=((sw.FLAVOR_TIER, 1), (sw.FLAVOR_TIER, 4)))
+
+
+def test_wide_tiles():
+    w = si.heat_sines(8192, 16, 5, 3000)
+    check(w, 3000, [2048, 4096], flavors=((sw.FLAVOR_TIER, 4),))
+    w = si.ks_cos(8192, 5, 700)
+    check(w, 700, [2048, 4096], flavors=((sw.FLAVOR_TIER, 4),))
+
+
+def test_per_step_non_power_of_two_N():
+    # the paper's `& lastidx` wrap needs N = 2^k; ours does not
+    for N in (1000, 1001, 1002):
+        w = si.heat_sines(N, 4, 9, 120)
+        ref = oracle.run_workload(w)
+        got, _ = gpu_run(w, 120, sw.PER_STEP)
+        assert np.array_equal(got, ref)
+    w = si.ks_cos(1001, 9, 30)
+    assert np.array_equal(gpu_run(w, 30, sw.PER_STEP)[0], oracle.run_workload(w))
+
+
+def test_repeated_runs_accumulate_and_launch_counts():
+    w = si.heat_sines(4096, 8, 2, 0)
+    s = sw.Swept.from_workload(w)
+    s.run(1000, 64, sw.SWEPT)
+    # m = 32: D = 1000/32 - 1 = 30 diamonds + Up + Down, remainder 8 per-step launches
+    assert s.last_launches == 32 + 8
+    s.run(300, 0, sw.PER_STEP)
+    assert s.last_launches == 300
+    s.run(500, 512, sw.SWEPT)
+    got = s.read()
+    s.close()
+    assert np.array_equal(got, oracle.run_workload(w, nsteps=1800))
+
+
+def test_error_codes():
+    w = si.heat_sines(4096, 8, 2, 0)
+    s = sw.Swept.from_workload(w)
+    with pytest.raises(sw.SweptError):
+        s.run(10, 48, sw.SWEPT)          # not a power of two
+    with pytest.raises(sw.SweptError):
+        s.run(10, 8192, sw.SWEPT)        # does not divide N
+    with pytest.raises(sw.SweptError):
+        s.run(-1, 64, sw.SWEPT)
+    with pytest.raises(sw.SweptError):
+        s.run(10, 100, sw.PER_STEP)      # threads per block not a power of two
+    with pytest.raises(sw.SweptError):
+        sw.swept_create(sw.KS, 4096, 0.5, 0.005, dtype=sw.F32)  # FP32 is heat only
+    s.run(10, 64, sw.SWEPT)              # still usable after errors
+    assert np.array_equal(s.read(), oracle.run_workload(w, nsteps=10))
+    s.close()
+
+
+# ---------------------------------------------------------------- the five configs
+def test_config1_full():
+    w = si.config(1)  # heat FP64 N=2048, 20000 steps
+    check(w, w.nsteps, [32, 64, 128, 256, 512, 1024], flavors=((sw.FLAVOR_TIER, 1), (sw.FLAVOR_TIER, 2)))
+
+
+@pytest.mark.parametrize("dtype", [np.float64, np.float32])
+def test_config2_full_length(dtype):
+    for N in (1 << 11, 1 << 16):  # full 10000 steps against the oracle
+        w = si.config(2, N=N)
+        check(w, w.nsteps, [32, 256, 1024], dtype=dtype, flavors=((sw.FLAVOR_TIER, 2),))
+
+
+@pytest.mark.parametrize("dtype", [np.float64, np.float32])
+def test_config2_large_N(dtype):
+    # oracle over a reduced step count covering > 2 swept cycles + remainder; full run swept == per_step
+    for N in (1 << 20, 1 << 22):
+        w = si.config(2, N=N)
+        check(w, 1100, [256, 1024], dtype=dtype, flavors=((sw.FLAVOR_TIER, 2),))
+    w = si.config(2, N=1 << 20)
+    ps, _ = gpu_run(w, w.nsteps, sw.PER_STEP, dtype=dtype)
+    sx, _ = gpu_run(w, w.nsteps, sw.SWEPT, 256, dtype=dtype)
+    assert np.array_equal(ps, sx)
+
+
+def test_config3_ks():
+    w = si.config(3, N=1 << 14)  # full 20000 steps
+    check(w, w.nsteps, [64, 256, 1024], flavors=((sw.FLAVOR_TIER, 2),))
+    w = si.config(3, N=1 << 20)
+    check(w, 300, [256], flavors=((sw.FLAVOR_TIER, 2),))
+    ps, _ = gpu_run(w, 4000, sw.PER_STEP)
+    sx, _ = gpu_run(w, 4000, sw.SWEPT, 512)
+    assert np.array_equal(ps, sx) and np.all(np.isfinite(ps)) and np.max(np.abs(ps)) < 10
+
+
+@pytest.mark.parametrize("rk2", [si.RK2_HEUN, si.RK2_MIDPOINT])
+def test_config4_euler(rk2):
+    for N in (1 << 11, 1 << 14):  # full 5000 steps
+        w = si.config(4, N=N, rk2=rk2)
+        check(w, w.nsteps, [64, 256], flavors=((sw.FLAVOR_TIER, 2),))
+    w = si.config(4, N=1 << 20, rk2=rk2)
+    check(w, 70, [256], flavors=((sw.FLAVOR_TIER, 2),))
+
+
+def test_config5_sampled_grid():
+    # swept == per_step bit for bit over the (problem, N, n) grid; oracle on the smallest N of each
+    for problem, steps in ((si.HEAT, 2000), (si.KS, 600), (si.EULER, 150)):
+        for N in (1 << 11, 1 << 17, 1 << 22):
+            w = si.config(5, N=N, problem=problem, nsteps=steps)
+            ps, _ = gpu_run(w, steps, sw.PER_STEP)
+            if N == 1 << 11:
+                assert np.array_equal(ps, oracle.run_workload(w, nsteps=steps))
+            for n in (32, 128, 512, 1024):
+                sx, _ = gpu_run(w, steps, sw.SWEPT, n)
+                assert np.array_equal(ps, sx), (problem, N, n)
+
+
+def test_autotune_picks_admissible_width_and_keeps_state():
+    w = si.heat_sines(1 << 16, 8, 2, 0)
+    s = sw.Swept.from_workload(w)
+    s.run(100, 64, sw.SWEPT)
+    best = s.autotune(sw.SWEPT)
+    assert best in (32, 64, 128, 256, 512, 1024, 2048, 4096) and (1 << 16) % best == 0
+    bt = s.autotune(sw.PER_STEP)
+    assert 32 <= bt <= 1024
+    s.run(100, 0, sw.SWEPT)  # uses the tuned width; the field was restored after tuning
+    got = s.read()
+    s.close()
+    assert np.array_equal(got, oracle.run_workload(w, nsteps=200))

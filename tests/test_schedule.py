@@ -1,0 +1,127 @@
+"""P10 — exact-integer simulation of the swept schedule, driven by the phase list the
+LIBRARY's host-side planner (`swept_plan`, C ABI, no GPU needed) produces.
+
+State: two ping-pong buffers of two global rows; row p holds, per point, the tier index of the latest value
+of parity p (or None).  Each phase does what a tile kernel does: load rows over [S-h, S+n+h) from the input
+buffer, compute its tiers, write rows over [S, S+n) to the output buffer.  Every stencil read is asserted to
+carry exactly the tier the scheme needs (t-1 for the 2h+1 window, t-2 for the own-point base of a final
+stage), so a wrong range, shift, tier count or parity anywhere fails.  Counts are pinned to the paper's
+printed numbers (65 792 values for n = 512; KS n = 32 -> 4 timesteps per cycle).
+"""
+import pytest
+
+import paper_1705_03162_b200 as sw
+
+UP, SPLIT, WHOLE, DOWN, REM = 0, 1, 2, 3, 4
+
+
+def active_range(kind, t, n, h):
+    m = n // (2 * h)
+    if kind == UP:
+        return h * t, n - h * t
+    w = h * t if (kind == DOWN or t <= m) else h * (2 * m - t)
+    return n // 2 - w, n // 2 + w
+
+
+def simulate(N, n, h, sigma, nsub):
+    plan = sw.swept_plan(nsub, n, h)
+    bufs = [[[None] * N, [None] * N], [[None] * N, [None] * N]]
+    bufs[0][0] = [0] * N  # tier 0 everywhere in row 0
+    cur, updates, launches = 0, 0, 0
+    field_tier = 0
+    for kind, shift, tier0, ntiers in plan:
+        if kind == REM:
+            assert tier0 == field_tier and ntiers % sigma == 0
+            field_tier += ntiers
+            updates += N * ntiers
+            launches += ntiers
+            continue
+        launches += 1
+        src, dst = bufs[cur], bufs[1 - cur]
+        new_dst = [list(dst[0]), list(dst[1])]
+        assert N % n == 0 and shift in (0, n // 2)
+        for tile in range(N // n):
+            S = (shift + tile * n) % N
+            # local copy of [S-h, S+n+h)
+            loc = [[src[r][(S - h + j) % N] for j in range(n + 2 * h)] for r in range(2)]
+            if kind == UP:
+                loc[1] = [None] * (n + 2 * h)
+            for t in range(1, ntiers + 1):
+                g = tier0 + t  # global tier
+                par = g % 2
+                assert par == t % 2, "phases must start on even tiers"
+                lo, hi = active_range(kind, t, n, h)
+                assert 0 <= lo < hi <= n
+                new_vals = {}
+                for j in range(lo, hi):
+                    for d in range(-h, h + 1):
+                        assert loc[1 - par][h + j + d] == g - 1, (kind, t, j, d, loc[1 - par][h + j + d], g - 1)
+                    if sigma == 2 and par == 0:
+                        assert loc[par][h + j] == g - 2
+                    new_vals[j] = g
+                for j, v in new_vals.items():
+                    loc[par][h + j] = v
+                updates += hi - lo
+            rows_out = (0,) if kind == DOWN else (0, 1)
+            for r in rows_out:
+                for j in range(n):
+                    new_dst[r][(S + j) % N] = loc[r][h + j]
+        bufs[1 - cur] = new_dst
+        cur = 1 - cur
+        if kind == DOWN:
+            field_tier = tier0 + ntiers
+            assert field_tier % 2 == 0
+            assert all(v == field_tier for v in bufs[cur][0]), "Down must leave a full time level in row 0"
+    assert field_tier == nsub
+    assert updates == N * nsub, "the swept schedule performs exactly the per-step work (PAPER.md:37)"
+    return plan, launches
+
+
+@pytest.mark.parametrize("N,n,h,sigma,D", [
+    (64, 16, 1, 1, 0), (64, 16, 1, 1, 1), (64, 16, 1, 1, 2), (64, 16, 1, 1, 3), (128, 32, 2, 2, 1),
+    (128, 32, 2, 2, 2), (128, 32, 2, 2, 3), (64, 32, 2, 2, 3), (32, 32, 2, 2, 3), (256, 64, 2, 2, 5),
+    (64, 32, 1, 1, 4), (32, 32, 1, 1, 2)])
+def test_schedule_exact(N, n, h, sigma, D):
+    m = n // (2 * h)
+    plan, _ = simulate(N, n, h, sigma, (D + 1) * m)
+    kinds = [p[0] for p in plan]
+    assert kinds[0] == UP and kinds[-1] == DOWN and len(plan) == D + 2
+    assert kinds[1:-1] == [SPLIT if k % 2 == 1 else WHOLE for k in range(1, D + 1)]
+
+
+@pytest.mark.parametrize("nsub", [0, 2, 14, 16, 18, 46, 100])
+def test_remainder_policy_g5(nsub):
+    # nsub not a multiple of m: largest T = (D+1) m <= nsub by swept phases, the rest per-step (reading G5)
+    N, n, h, sigma = 64, 32, 1, 1
+    plan, _ = simulate(N, n, h, sigma, nsub)
+    m = n // (2 * h)
+    swept_part = sum(1 for p in plan if p[0] != REM)
+    if nsub < m:
+        assert swept_part == 0
+    else:
+        assert swept_part == nsub // m + 1
+    rem = [p for p in plan if p[0] == REM]
+    assert (len(rem) == 1 and rem[0][3] == nsub % m) if nsub % m else not rem
+
+
+def test_paper_counts():
+    # the triangle of a 512-point node holds 65 792 values (incl. the initial row), h = 1
+    n, h = 512, 1
+    m = n // (2 * h)
+    total = n + sum(active_range(UP, t, n, h)[1] - active_range(UP, t, n, h)[0] for t in range(1, m))
+    assert total == 65792
+    # KS with n = 32: four timesteps per cycle (m = n/(2h) = 8 sub-timesteps)
+    plan = sw.swept_plan(2 * 4 * 3, 32, 2)
+    assert plan[1][3] == 15 and plan[2][2] - plan[1][2] == 8
+    # n sub-timesteps per pair of global accesses: a diamond advances n/h - 1 tiers at its centre
+    assert sw.swept_plan(64 * 10, 64, 1)[1][3] == 63
+    # launch counts: heat N=2^20 n=256, 50 000 steps: D + 2 launches (~392)
+    plan = sw.swept_plan(50000, 256, 1)
+    assert sum(1 for p in plan if p[0] != REM) == 50000 // 128 + 1 == 391
+
+
+def test_plan_rejects_bad_arguments():
+    with pytest.raises(sw.SweptError):
+        sw.swept_plan(10, 48, 1)  # not a power of two
+    with pytest.raises(sw.SweptError):
+        sw.swept_plan(10, 64, 3)
