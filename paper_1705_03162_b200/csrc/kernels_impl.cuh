@@ -68,7 +68,7 @@ inline bool tier_ok(int n, int P, int pmax) {
   if (P != 1 && P != 2 && P != 4) return false;
   if (P > pmax) return false;
   const int threads = n / P;
-  if (threads < 32 || threads > 1024) return false;
+  if (threads < 8 || threads > 1024) return false;
   return tier_smem_bytes<Prob>(n) <= 227 * 1024;
 }
 
