@@ -42,6 +42,7 @@ template <class R_>
 struct Heat {
   using R = R_;
   static constexpr int H = 1, C = 1, SIGMA = 1;
+  static constexpr int MAX_THREADS = 1024;  // per CTA, for __launch_bounds__ (register budget)
   __device__ __forceinline__ static R point(R um, R u0, R up, const Consts<R>& k) {
     const R s = um + up;
     const R t = k.a1 * u0;
@@ -62,6 +63,7 @@ template <class R_, int HEUN>
 struct KS {
   using R = R_;
   static constexpr int H = 2, C = 1, SIGMA = 2;
+  static constexpr int MAX_THREADS = 1024;
   __device__ __forceinline__ static R rhs(R vm2, R vm1, R v0, R vp1, R vp2, const Consts<R>& k) {
     const R s1 = vp1 + vm1;
     const R s2 = vp2 + vm2;
@@ -100,6 +102,7 @@ template <class R_, int HEUN>
 struct Euler {
   using R = R_;
   static constexpr int H = 2, C = 3, SIGMA = 2;
+  static constexpr int MAX_THREADS = 256;  // ~250 live registers per thread (P:270 'greater low-level memory usage')
 
   __device__ __forceinline__ static R pressure(R rho, R M, R E, const Consts<R>& k) {  // (D.4), X4
     const R u = M / rho;

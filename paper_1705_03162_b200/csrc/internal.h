@@ -40,9 +40,9 @@ int launch_tile_heat(int dtype, const TileLaunch& a);
 int launch_tile_ks(int dtype, int rk2, const TileLaunch& a);
 int launch_tile_euler(int dtype, int rk2, const TileLaunch& a);
 // does a kernel exist for (flavor, n, P)?  (host-only query used by the autotuner and argument checks)
-bool tile_config_ok_heat(int dtype, int flavor, int n, int P);
-bool tile_config_ok_ks(int dtype, int flavor, int n, int P);
-bool tile_config_ok_euler(int dtype, int flavor, int n, int P);
+bool tile_config_ok_heat(int dtype, int flavor, int64_t N, int n, int P);
+bool tile_config_ok_ks(int dtype, int flavor, int64_t N, int n, int P);
+bool tile_config_ok_euler(int dtype, int flavor, int64_t N, int n, int P);
 
 constexpr int NO_KERNEL = -1000;
 

@@ -5,15 +5,18 @@ int launch_per_step_euler(int dtype, int rk2, const PerStepLaunch& a) {
   if (dtype != 0) return NO_KERNEL;
   return rk2 == 0 ? per_step_T<Euler<double, 0>, 2>(a) : per_step_T<Euler<double, 1>, 2>(a);
 }
-bool tile_config_ok_euler(int dtype, int flavor, int n, int P) {
+bool tile_config_ok_euler(int dtype, int flavor, int64_t N, int n, int P) {
   if (dtype != 0) return false;
-  if (flavor == SWEPT_FLAVOR_TIER) return tier_ok<Euler<double, 0>>(n, P, 2);
+  if (flavor == SWEPT_FLAVOR_TIER) return tier_ok<Euler<double, 0>>(n, P, 4);
+  if (flavor == SWEPT_FLAVOR_CHAR) return char_ok<Euler<double, 0>, 16>(N, n, P);
   return false;
 }
 int launch_tile_euler(int dtype, int rk2, const TileLaunch& a) {
   if (dtype != 0) return NO_KERNEL;
   if (a.flavor == SWEPT_FLAVOR_TIER)
-    return rk2 == 0 ? tier_T<Euler<double, 0>, 2>(a) : tier_T<Euler<double, 1>, 2>(a);
+    return rk2 == 0 ? tier_T<Euler<double, 0>, 4>(a) : tier_T<Euler<double, 1>, 4>(a);
+  if (a.flavor == SWEPT_FLAVOR_CHAR)
+    return rk2 == 0 ? char_T<Euler<double, 0>, 16>(a) : char_T<Euler<double, 1>, 16>(a);
   return NO_KERNEL;
 }
 }  // namespace swept

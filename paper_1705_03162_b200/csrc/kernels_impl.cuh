@@ -3,6 +3,7 @@
 #include "internal.h"
 #include "per_step.cuh"
 #include "swept_tier.cuh"
+#include "swept_char.cuh"
 #include "../../include/swept.h"
 
 namespace swept {
@@ -18,8 +19,9 @@ template <class Prob, int P>
 inline int per_step_go(const PerStepLaunch& a) {
   using R = typename Prob::R;
   const int64_t nthreads = a.N / P;
-  const unsigned grid = (unsigned)((nthreads + a.threads - 1) / a.threads);
-  per_step_kernel<Prob, P><<<grid, a.threads, 0, a.stream>>>((const R*)a.in, (const R*)a.base, (R*)a.out,
+  const int threads = a.threads < Prob::MAX_THREADS ? a.threads : Prob::MAX_THREADS;
+  const unsigned grid = (unsigned)((nthreads + threads - 1) / threads);
+  per_step_kernel<Prob, P><<<grid, threads, 0, a.stream>>>((const R*)a.in, (const R*)a.base, (R*)a.out,
                                                              a.N, a.odd, round_consts<R>(a.consts));
   return (int)cudaGetLastError();
 }
@@ -68,7 +70,7 @@ inline bool tier_ok(int n, int P, int pmax) {
   if (P != 1 && P != 2 && P != 4) return false;
   if (P > pmax) return false;
   const int threads = n / P;
-  if (threads < 8 || threads > 1024) return false;
+  if (threads < 8 || threads > Prob::MAX_THREADS) return false;
   return tier_smem_bytes<Prob>(n) <= 227 * 1024;
 }
 
@@ -79,6 +81,75 @@ inline int tier_T(const TileLaunch& a) {
     case 1: return tier_kind<Prob, 1>(a);
     case 2: return tier_kind<Prob, 2>(a);
     case 4: if (PMAX >= 4) return tier_kind<Prob, (PMAX >= 4 ? 4 : 1)>(a); break;
+  }
+  return NO_KERNEL;
+}
+
+
+// ---- CHAR flavour: a.P = L (lanes per tile), B = n / L lines per lane ---------------------------------
+inline int char_threads(int64_t N, int B) {
+  for (int T : {64, 32})
+    if (N % ((int64_t)T * B) == 0) return T;
+  return 0;
+}
+
+template <class Prob, int B, int L, int KIND>
+inline int char_go(const TileLaunch& a) {
+  using R = typename Prob::R;
+  const int T = char_threads(a.N, B);
+  if (T == 0 || T < L) return NO_KERNEL;
+  TierArgs<R> t;
+  t.in0 = (const R*)a.in0; t.in1 = (const R*)a.in1; t.out0 = (R*)a.out0; t.out1 = (R*)a.out1;
+  t.N = a.N; t.n = a.n; t.shift = a.shift; t.ntiers = a.ntiers; t.k = round_consts<R>(a.consts);
+  const size_t smem = char_smem_bytes<Prob>(T, B);
+  auto kern = swept_char_kernel<Prob, B, L, KIND>;
+  if (smem > 48 * 1024) {
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return (int)e;
+  }
+  kern<<<(unsigned)(a.N / ((int64_t)T * B)), T, smem, a.stream>>>(t);
+  return (int)cudaGetLastError();
+}
+
+template <class Prob, int B, int L>
+inline int char_kind(const TileLaunch& a) {
+  switch (a.kind) {
+    case KIND_UP: return char_go<Prob, B, L, KIND_UP>(a);
+    case KIND_SPLIT: return char_go<Prob, B, L, KIND_SPLIT>(a);
+    case KIND_WHOLE: return char_go<Prob, B, L, KIND_WHOLE>(a);
+    case KIND_DOWN: return char_go<Prob, B, L, KIND_DOWN>(a);
+  }
+  return NO_KERNEL;
+}
+
+template <class Prob, int BMAX>
+inline bool char_ok(int64_t N, int n, int L) {
+  if (L != 8 && L != 16 && L != 32) return false;
+  if (n % L) return false;
+  const int B = n / L;
+  if (B != 8 && B != 16 && B != 32) return false;
+  if (B > BMAX || B % (2 * Prob::H)) return false;
+  const int T = char_threads(N, B);
+  return T >= L && N % n == 0;
+}
+
+template <class Prob, int B>
+inline int char_L(const TileLaunch& a) {
+  switch (a.P) {
+    case 8: return char_kind<Prob, B, 8>(a);
+    case 16: return char_kind<Prob, B, 16>(a);
+    case 32: return char_kind<Prob, B, 32>(a);
+  }
+  return NO_KERNEL;
+}
+
+template <class Prob, int BMAX>
+inline int char_T(const TileLaunch& a) {
+  if (!char_ok<Prob, BMAX>(a.N, a.n, a.P)) return NO_KERNEL;
+  switch (a.n / a.P) {
+    case 8: return char_L<Prob, 8>(a);
+    case 16: if (BMAX >= 16) return char_L<Prob, (BMAX >= 16 ? 16 : 8)>(a); break;
+    case 32: if (BMAX >= 32) return char_L<Prob, (BMAX >= 32 ? 32 : 8)>(a); break;
   }
   return NO_KERNEL;
 }

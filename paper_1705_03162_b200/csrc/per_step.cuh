@@ -40,7 +40,7 @@ __device__ __forceinline__ void store_vec(R* __restrict__ p, const R (&v)[P]) {
 
 // in: stage input (tier t-1), base: tier t-2 field (only read when SIGMA == 2 and !odd), out: tier t.
 template <class Prob, int P>
-__global__ void __launch_bounds__(1024)
+__global__ void __launch_bounds__(Prob::MAX_THREADS)
 per_step_kernel(const typename Prob::R* __restrict__ in, const typename Prob::R* __restrict__ base,
                 typename Prob::R* __restrict__ out, int64_t N, int odd, Consts<typename Prob::R> k) {
   using R = typename Prob::R;

@@ -117,9 +117,9 @@ int launch_tile(swept_state* s, swept::TileLaunch& a) {
 bool tile_ok(const swept_state* s, int flavor, int n, int P) {
   if (n <= 0 || s->N % n != 0) return false;
   switch (s->problem) {
-    case SWEPT_HEAT: return swept::tile_config_ok_heat(s->dtype, flavor, n, P);
-    case SWEPT_KS: return swept::tile_config_ok_ks(s->dtype, flavor, n, P);
-    default: return swept::tile_config_ok_euler(s->dtype, flavor, n, P);
+    case SWEPT_HEAT: return swept::tile_config_ok_heat(s->dtype, flavor, s->N, n, P);
+    case SWEPT_KS: return swept::tile_config_ok_ks(s->dtype, flavor, s->N, n, P);
+    default: return swept::tile_config_ok_euler(s->dtype, flavor, s->N, n, P);
   }
 }
 
@@ -238,9 +238,9 @@ void default_tile(const swept_state* s, int* n_io, int* flavor_io, int* P_io) {
   }
   if (P == 0) {
     if (flavor == SWEPT_FLAVOR_TIER) {
-      const int pmax = s->problem == SWEPT_EULER ? 2 : 4;
+      const int pmax = 4, tmax = s->problem == SWEPT_EULER ? 256 : 1024;
       P = std::min(pmax, std::max(1, n / 256));
-      while (P < pmax && n / P > 1024) P *= 2;
+      while (P < pmax && n / P > tmax) P *= 2;
       if (P == 3) P = 2;
     }
   }

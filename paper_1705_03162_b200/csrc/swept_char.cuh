@@ -1,0 +1,224 @@
+// swept_char.cuh — swept kernels, flavour CHAR: register-resident sweep of a tile along its characteristics.
+//
+// Same space-time regions as swept_tier.cuh (UpTriangle / Split-, WholeDiamond / DownTriangle of PAPER.md
+// §4.2-4.3, edges through the two global rows, half-tile shift) — only the ORDER in which the points of one
+// tile are evaluated on chip differs, which the swept rule leaves free.
+//
+// Geometry.  In a diamond of width n centred at c, relative tier t, x' = x - c, use the characteristic
+// coordinates  p = x' + h t,  q = h t - x' - 1.  The diamond is exactly the square 0 <= p, q < n (lattice
+// points: p + q + 1 = 2 h t).  Point (p, q) depends on (p-2h+k, q-k), k = 0..2h (its 2h+1 stencil inputs at
+// tier t-1) and, for a final stage, on (p-2h, q-2h) (its own value at tier t-2).  So any order with p
+// ascending and, inside a column, q ascending is valid, and a "line" q = const needs only ONE live value:
+// its latest point.  A tile is owned by a group of L lanes; lane gl keeps the B = n/L lines
+// q in [gl B, gl B + B) in registers (v[.]), sweeps p upwards 2h columns ("super-column") per step, and lags
+// its lower neighbour by one step, so the only communication is: per step, the 2h top lines of lane gl-1
+// by __shfl_up.  Lane 0 takes them from the staged input rows instead (the diamond's lower-right edge),
+// lane L-1 streams its top lines out (the upper-left edge), and the last values of all lines form the
+// upper-right edge.  Every lane is busy m = n/(2h) of the m + L - 1 steps: lane utilisation m/(m+L-1)
+// instead of the ~50 % of a tier-by-tier diamond (PAPER.md:211 names idle threads as the first drawback).
+// No block barrier and no shared-memory traffic inside the sweep.
+//
+// Up / Down are the upper / lower half of the same square (tiers t > m, resp. t <= m, with m the tier of the
+// anti-diagonal p + q + 1 = n); the other half is masked.
+//
+// Shared memory holds the CTA's chunk of both rows (T*B contiguous points, all tiles of the CTA), loaded and
+// stored with TMA 1-D bulk copies, and is updated in place: stream / final writes only touch slots whose
+// input value has already been consumed (see DESIGN.md §5.3 for the hazard argument).
+#pragma once
+#include "common.cuh"
+#include "functors.cuh"
+#include "swept_tier.cuh"
+
+namespace swept {
+
+template <class R>
+__device__ __forceinline__ R shfl_up_(R v, int width);
+template <>
+__device__ __forceinline__ double shfl_up_<double>(double v, int width) {
+  return __shfl_up_sync(0xffffffffu, v, 1, width);
+}
+template <>
+__device__ __forceinline__ float shfl_up_<float>(float v, int width) {
+  return __shfl_up_sync(0xffffffffu, v, 1, width);
+}
+
+template <class Prob, int B, int L, int KIND>
+__global__ void __launch_bounds__(128) swept_char_kernel(const TierArgs<typename Prob::R> a) {
+  using R = typename Prob::R;
+  constexpr int H = Prob::H, C = Prob::C, PAD = Pad16<R>::value;
+  constexpr int n = B * L;          // tile width
+  constexpr int m = n / (2 * H);    // super-columns per tile = tiers per half diamond
+  constexpr int BP = B / (2 * H);   // points per lane per sub-column (chain length)
+  static_assert(B % (2 * H) == 0, "lines per lane must be a multiple of 2h");
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  const int T = blockDim.x;
+  const int chunk = T * B;  // points staged by this CTA (T/L adjacent tiles)
+  const int RS = chunk + 2 * PAD;
+  R* rows = reinterpret_cast<R*>(smem_raw);
+  uint64_t* mbar = reinterpret_cast<uint64_t*>(smem_raw + (size_t)2 * C * RS * sizeof(R));
+  const int64_t N = a.N;
+  const int tid = threadIdx.x;
+  int64_t S = ((int64_t)a.shift + (int64_t)blockIdx.x * chunk) % N;
+  const int len1 = (int)((N - S) < (int64_t)chunk ? (N - S) : (int64_t)chunk);
+  const int len2 = chunk - len1;
+  constexpr int NROWS_IN = (KIND == KIND_UP) ? 1 : 2;
+
+  if (tid == 0) {
+    mbar_init(mbar, 1);
+    fence_mbar_init();
+  }
+  __syncthreads();
+  if (tid == 0) {
+    mbar_arrive_expect_tx(mbar, (uint32_t)(NROWS_IN * C * chunk * sizeof(R)));
+#pragma unroll
+    for (int r = 0; r < NROWS_IN; ++r) {
+      const R* src = r == 0 ? a.in0 : a.in1;
+#pragma unroll
+      for (int c = 0; c < C; ++c) {
+        R* dst = rows + (r * C + c) * RS + PAD;
+        bulk_g2s(dst, src + (int64_t)c * N + S, (uint32_t)(len1 * sizeof(R)), mbar);
+        if (len2 > 0) bulk_g2s(dst + len1, src + (int64_t)c * N, (uint32_t)(len2 * sizeof(R)), mbar);
+      }
+    }
+  }
+  if (KIND == KIND_UP) {
+    for (int i = tid; i < C * RS; i += T) rows[C * RS + i] = (R)0;  // tier -1 does not exist
+  } else {
+    for (int i = tid; i < 2 * C * 2 * H; i += T) {  // halo of the chunk, both rows (periodic)
+      const int r = i / (C * 2 * H), c = (i / (2 * H)) % C, j = i % (2 * H);
+      const R* src = (r == 0 ? a.in0 : a.in1) + (int64_t)c * N;
+      int64_t g = (j < H) ? (S - H + j) : (S + chunk + (j - H));
+      if (g < 0) g += N;
+      if (g >= N) g -= N;
+      const int s = (j < H) ? (PAD - H + j) : (PAD + chunk + (j - H));
+      rows[(r * C + c) * RS + s] = src[g];
+    }
+  }
+  mbar_wait(mbar, 0);
+  __syncthreads();
+
+  const int gl = tid % L;                       // lane within the tile's group
+  const int ctr = PAD + (tid / L) * n + n / 2;  // smem slot of x' = 0 of this thread's tile
+  auto slot = [&](int row, int c, int xp) -> R& { return rows[(row * C + c) * RS + ctr + xp]; };
+
+  R v[C][B], hal[C][2 * H], halp[C][2 * H];
+  // initial line values: the point of line q just below the square (super-column -1), which is the latest
+  // (or second latest) tier stored at x' = -(h tq + r + 1); Up: the anti-diagonal = tier-0 data
+#pragma unroll
+  for (int i = 0; i < B; ++i) {
+    const int q = gl * B + i;
+    int xp, row;
+    if (KIND == KIND_UP) {
+      xp = n / 2 - 1 - q;
+      row = 0;
+    } else {
+      const int tq = q / (2 * H), r = i % (2 * H);
+      xp = -(H * tq + r + 1);
+      row = tq & 1;
+    }
+#pragma unroll
+    for (int c = 0; c < C; ++c) v[c][i] = slot(row, c, xp);
+  }
+#pragma unroll
+  for (int c = 0; c < C; ++c)
+#pragma unroll
+    for (int e = 0; e < 2 * H; ++e) hal[c][e] = halp[c][e] = (R)0;
+  __syncwarp();
+
+  for (int s = 0; s < m + L - 1; ++s) {
+    const int sc = s - gl;  // this lane's super-column
+    // halo: top 2h lines of the lower neighbour lane (it finished super-column sc one step ago);
+    // group lane 0 reads the staged lower-right edge: line -1-e at super-column sc is (x' = h sc + e, tier sc)
+    {
+      const int scc = sc < 0 ? 0 : (sc >= m ? m - 1 : sc);
+#pragma unroll
+      for (int c = 0; c < C; ++c)
+#pragma unroll
+        for (int e = 0; e < 2 * H; ++e) {
+          halp[c][e] = hal[c][e];
+          const R up = shfl_up_<R>(v[c][B - 1 - e], L);
+          hal[c][e] = up;
+          if (gl == 0) hal[c][e] = slot(scc & 1, c, H * scc + e);
+        }
+    }
+    if (sc >= 0 && sc < m) {
+#pragma unroll
+      for (int rho = 0; rho < 2 * H; ++rho) {
+        R carry[C];  // previous value of line i-2h (tier t-2 of the point being computed)
+#pragma unroll
+        for (int c = 0; c < C; ++c) carry[c] = halp[c][rho];
+#pragma unroll
+        for (int aa = 0; aa < BP; ++aa) {
+          const int i = 2 * H - 1 - rho + 2 * H * aa;  // line updated in this sub-column
+          const int t = sc + gl * BP + aa + 1;         // its relative tier
+          const int odd = t & 1;
+          const bool act = KIND == KIND_UP ? (t > m) : (KIND == KIND_DOWN ? (t <= m) : true);
+          R win[C][2 * H + 1], bs[C][1], o[C][1];
+#pragma unroll
+          for (int c = 0; c < C; ++c) {
+#pragma unroll
+            for (int k = 0; k <= 2 * H; ++k) win[c][k] = (i - k >= 0) ? v[c][(i - k >= 0) ? i - k : 0]
+                                                                      : hal[c][(i - k >= 0) ? 0 : k - i - 1];
+            bs[c][0] = (Prob::SIGMA == 2 && !odd) ? carry[c] : win[c][H];
+          }
+          Prob::template stage<1>(win, bs, o, odd, a.k);
+#pragma unroll
+          for (int c = 0; c < C; ++c) {
+            carry[c] = v[c][i];
+            if (act) v[c][i] = o[c][0];
+          }
+        }
+      }
+      // upper-left edge: the top 2h lines of the last lane leave the tile (x' = -n/2 + h sc + e, tier m+sc)
+      if (KIND != KIND_DOWN && gl == L - 1) {
+#pragma unroll
+        for (int c = 0; c < C; ++c)
+#pragma unroll
+          for (int e = 0; e < 2 * H; ++e) slot(sc & 1, c, -n / 2 + H * sc + e) = v[c][B - 1 - e];
+      }
+    }
+  }
+  __syncwarp();
+  // upper-right edge (Down: the full time level): last value of every line
+#pragma unroll
+  for (int i = 0; i < B; ++i) {
+    const int q = gl * B + i;
+    int xp, row;
+    if (KIND == KIND_DOWN) {
+      xp = n / 2 - 1 - q;
+      row = 0;
+    } else {
+      const int tq = q / (2 * H), r = i % (2 * H);
+      xp = n / 2 - 1 - H * tq - r;
+      row = tq & 1;
+    }
+#pragma unroll
+    for (int c = 0; c < C; ++c) slot(row, c, xp) = v[c][i];
+  }
+
+  fence_proxy_async_smem();
+  __syncthreads();
+  if (tid == 0) {
+    constexpr int NROWS_OUT = (KIND == KIND_DOWN) ? 1 : 2;
+#pragma unroll
+    for (int r = 0; r < NROWS_OUT; ++r) {
+      R* dstg = r == 0 ? a.out0 : a.out1;
+#pragma unroll
+      for (int c = 0; c < C; ++c) {
+        const R* sm = rows + (r * C + c) * RS + PAD;
+        bulk_s2g(dstg + (int64_t)c * N + S, sm, (uint32_t)(len1 * sizeof(R)));
+        if (len2 > 0) bulk_s2g(dstg + (int64_t)c * N, sm + len1, (uint32_t)(len2 * sizeof(R)));
+      }
+    }
+    bulk_commit();
+    bulk_wait_all();
+  }
+}
+
+template <class Prob>
+inline size_t char_smem_bytes(int threads, int B) {
+  using R = typename Prob::R;
+  return (size_t)2 * Prob::C * ((size_t)threads * B + 2 * Pad16<R>::value) * sizeof(R) + 16;
+}
+
+}  // namespace swept

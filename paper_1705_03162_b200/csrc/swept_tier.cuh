@@ -53,7 +53,7 @@ __device__ __forceinline__ void tier_range(int t, int n, int h, int m, int& lo, 
 }
 
 template <class Prob, int P, int KIND>
-__global__ void __launch_bounds__(1024) swept_tier_kernel(const TierArgs<typename Prob::R> a) {
+__global__ void __launch_bounds__(Prob::MAX_THREADS) swept_tier_kernel(const TierArgs<typename Prob::R> a) {
   using R = typename Prob::R;
   constexpr int H = Prob::H, C = Prob::C, PAD = Pad16<R>::value;
   extern __shared__ __align__(128) unsigned char smem_raw[];

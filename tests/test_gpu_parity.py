@@ -35,7 +35,11 @@ def gpu_run(w, nsteps, variant, tile_width=0, flavor=sw.FLAVOR_AUTO, group=0, dt
     return out, launches
 
 
-def check(w, nsteps, tile_widths, dtype=np.float64, flavors=((sw.FLAVOR_TIER, 0),), exact=True):
+CHAR = tuple((sw.FLAVOR_CHAR, L) for L in (8, 16, 32))
+TIER12 = ((sw.FLAVOR_TIER, 1), (sw.FLAVOR_TIER, 2))
+
+
+def check(w, nsteps, tile_widths, dtype=np.float64, flavors=((sw.FLAVOR_TIER, 0),) + CHAR, exact=True):
     C = w.components
     ref = oracle.run_workload(w, nsteps=nsteps, dtype=dtype)
     ps, _ = gpu_run(w, nsteps, sw.PER_STEP, dtype=dtype)
@@ -44,11 +48,20 @@ def check(w, nsteps, tile_widths, dtype=np.float64, flavors=((sw.FLAVOR_TIER, 0)
     assert relerr(ps, ref, C) <= tol, f"per_step vs oracle: {relerr(ps, ref, C)}"
     if exact:
         assert np.array_equal(ps, ref), "same expression trees: expected 0 ulp"
+    ran = 0
     for n in tile_widths:
         for fl, grp in flavors:
-            sx, _ = gpu_run(w, nsteps, sw.SWEPT, n, fl, grp, dtype=dtype)
+            try:
+                sx, _ = gpu_run(w, nsteps, sw.SWEPT, n, fl, grp, dtype=dtype)
+            except sw.SweptError as e:
+                if "not admissible" in str(e):  # e.g. CHAR needs n/L in {8,16,32} and 32*B | N
+                    continue
+                raise
+            ran += 1
             assert np.array_equal(sx, ps), f"swept(n={n}, flavor={fl}, group={grp}) != per_step bitwise"
             assert relerr(sx, ref, C) <= tol
+    assert ran >= min(1, len(tile_widths)), "no swept configuration was admissible"
+    return ran
 
 
 # ---------------------------------------------------------------- small cases spanning several tiles
@@ -56,7 +69,7 @@ def check(w, nsteps, tile_widths, dtype=np.float64, flavors=((sw.FLAVOR_TIER, 0)
 def test_heat_small(N, nsteps):
     w = si.heat_sines(N, 8, 11, nsteps)
     widths = [n for n in (32, 64, 128, 256) if N % n == 0]
-    check(w, nsteps, widths, flavors=((sw.FLAVOR_TIER, 1), (sw.FLAVOR_TIER, 2)))
+    check(w, nsteps, widths, flavors=TIER12 + CHAR)
 
 
 @pytest.mark.parametrize("rk2", [si.RK2_MIDPOINT, si.RK2_HEUN])
@@ -64,14 +77,14 @@ def test_heat_small(N, nsteps):
 def test_ks_small(N, nsteps, rk2):
     w = si.ks_cos(N, 5, nsteps)
     w.rk2 = rk2
-    check(w, nsteps, [32, 64, 256], flavors=((sw.FLAVOR_TIER, 1), (sw.FLAVOR_TIER, 2), (sw.FLAVOR_TIER, 4)))
+    check(w, nsteps, [32, 64, 128, 256], flavors=TIER12 + ((sw.FLAVOR_TIER, 4),) + CHAR)
 
 
 @pytest.mark.parametrize("rk2", [si.RK2_MIDPOINT, si.RK2_HEUN])
 @pytest.mark.parametrize("N,nsteps", [(256, 3), (512, 150)])
 def test_euler_small(N, nsteps, rk2):
     w = si.euler_double_sod(N, nsteps, rk2=rk2)
-    check(w, nsteps, [32, 128, 256], flavors=((sw.FLAVOR_TIER, 1), (sw.FLAVOR_TIER, 2)))
+    check(w, nsteps, [32, 64, 128, 256], flavors=TIER12 + CHAR)
 
 
 def test_euler_random_data():
@@ -90,7 +103,7 @@ def test_single_tile_wraps_onto_itself():
 
 def test_heat_fp32():
     w = si.heat_sines(1024, 16, 21, 500)
-    check(w, 500, [32, 128, 1024], dtype=np.float32, flavors=((sw.FLAVOR_TIER, 1), (sw.FLAVOR_TIER, 4)))
+    check(w, 500, [32, 128, 256, 1024], dtype=np.float32, flavors=((sw.FLAVOR_TIER, 1), (sw.FLAVOR_TIER, 4)) + CHAR)
 
 
 def test_wide_tiles():
@@ -146,14 +159,14 @@ def test_error_codes():
 # ---------------------------------------------------------------- the five configs
 def test_config1_full():
     w = si.config(1)  # heat FP64 N=2048, 20000 steps
-    check(w, w.nsteps, [32, 64, 128, 256, 512, 1024], flavors=((sw.FLAVOR_TIER, 1), (sw.FLAVOR_TIER, 2)))
+    check(w, w.nsteps, [32, 64, 128, 256, 512, 1024], flavors=TIER12 + CHAR)
 
 
 @pytest.mark.parametrize("dtype", [np.float64, np.float32])
 def test_config2_full_length(dtype):
     for N in (1 << 11, 1 << 16):  # full 10000 steps against the oracle
         w = si.config(2, N=N)
-        check(w, w.nsteps, [32, 256, 1024], dtype=dtype, flavors=((sw.FLAVOR_TIER, 2),))
+        check(w, w.nsteps, [32, 256, 1024], dtype=dtype, flavors=((sw.FLAVOR_TIER, 2),) + CHAR)
 
 
 @pytest.mark.parametrize("dtype", [np.float64, np.float32])
@@ -161,7 +174,7 @@ def test_config2_large_N(dtype):
     # oracle over a reduced step count covering > 2 swept cycles + remainder; full run swept == per_step
     for N in (1 << 20, 1 << 22):
         w = si.config(2, N=N)
-        check(w, 1100, [256, 1024], dtype=dtype, flavors=((sw.FLAVOR_TIER, 2),))
+        check(w, 1100, [256, 1024], dtype=dtype, flavors=((sw.FLAVOR_TIER, 2),) + CHAR)
     w = si.config(2, N=1 << 20)
     ps, _ = gpu_run(w, w.nsteps, sw.PER_STEP, dtype=dtype)
     sx, _ = gpu_run(w, w.nsteps, sw.SWEPT, 256, dtype=dtype)
@@ -170,9 +183,9 @@ def test_config2_large_N(dtype):
 
 def test_config3_ks():
     w = si.config(3, N=1 << 14)  # full 20000 steps
-    check(w, w.nsteps, [64, 256, 1024], flavors=((sw.FLAVOR_TIER, 2),))
+    check(w, w.nsteps, [64, 256, 1024], flavors=((sw.FLAVOR_TIER, 2),) + CHAR)
     w = si.config(3, N=1 << 20)
-    check(w, 300, [256], flavors=((sw.FLAVOR_TIER, 2),))
+    check(w, 300, [256], flavors=((sw.FLAVOR_TIER, 2),) + CHAR)
     ps, _ = gpu_run(w, 4000, sw.PER_STEP)
     sx, _ = gpu_run(w, 4000, sw.SWEPT, 512)
     assert np.array_equal(ps, sx) and np.all(np.isfinite(ps)) and np.max(np.abs(ps)) < 10
@@ -182,9 +195,9 @@ def test_config3_ks():
 def test_config4_euler(rk2):
     for N in (1 << 11, 1 << 14):  # full 5000 steps
         w = si.config(4, N=N, rk2=rk2)
-        check(w, w.nsteps, [64, 256], flavors=((sw.FLAVOR_TIER, 2),))
+        check(w, w.nsteps, [64, 256], flavors=((sw.FLAVOR_TIER, 2),) + CHAR)
     w = si.config(4, N=1 << 20, rk2=rk2)
-    check(w, 70, [256], flavors=((sw.FLAVOR_TIER, 2),))
+    check(w, 70, [256], flavors=((sw.FLAVOR_TIER, 2),) + CHAR)
 
 
 def test_config5_sampled_grid():
@@ -196,8 +209,13 @@ def test_config5_sampled_grid():
             if N == 1 << 11:
                 assert np.array_equal(ps, oracle.run_workload(w, nsteps=steps))
             for n in (32, 128, 512, 1024):
-                sx, _ = gpu_run(w, steps, sw.SWEPT, n)
-                assert np.array_equal(ps, sx), (problem, N, n)
+                for fl, grp in ((sw.FLAVOR_TIER, 0), (sw.FLAVOR_CHAR, 16), (sw.FLAVOR_CHAR, 32)):
+                    try:
+                        sx, _ = gpu_run(w, steps, sw.SWEPT, n, fl, grp)
+                    except sw.SweptError as e:
+                        assert "not admissible" in str(e)
+                        continue
+                    assert np.array_equal(ps, sx), (problem, N, n, fl, grp)
 
 
 def test_autotune_picks_admissible_width_and_keeps_state():
