@@ -42,6 +42,69 @@ __device__ __forceinline__ float shfl_up_<float>(float v, int width) {
   return __shfl_up_sync(0xffffffffu, v, 1, width);
 }
 
+// One super-step of a lane: fetch the 2h-line halo (shuffle, or the staged edge for group lane 0), update the
+// B lines of this lane (2h sub-columns, each a dependent chain of B/2h points), stream the top lines out
+// (group lane L-1).  GUARD = some lanes of the warp are outside their m super-columns (ramp up / down).
+template <class Prob, int B, int L, int KIND, bool GUARD>
+__device__ __forceinline__ void char_step(typename Prob::R (&v)[Prob::C][B],
+                                          typename Prob::R (&hal)[Prob::C][2 * Prob::H],
+                                          const typename Prob::R (&halp)[Prob::C][2 * Prob::H],
+                                          typename Prob::R*& io, int& inc, const int s, const int gl, const int RS,
+                                          const Consts<typename Prob::R>& kc) {
+  using R = typename Prob::R;
+  constexpr int H = Prob::H, C = Prob::C;
+  constexpr int n = B * L, m = n / (2 * H), BP = B / (2 * H);
+  const int sc = s - gl;  // this lane's super-column
+#pragma unroll
+  for (int c = 0; c < C; ++c)
+#pragma unroll
+    for (int e = 0; e < 2 * H; ++e) hal[c][e] = shfl_up_<R>(v[c][B - 1 - e], L);
+  if (gl == 0 && (!GUARD || s < m)) {
+#pragma unroll
+    for (int c = 0; c < C; ++c)
+#pragma unroll
+      for (int e = 0; e < 2 * H; ++e) hal[c][e] = io[c * RS + e];
+  }
+  if (!GUARD || (sc >= 0 && sc < m)) {
+#pragma unroll
+    for (int rho = 0; rho < 2 * H; ++rho) {
+      R carry[C];  // previous value of line i-2h (tier t-2 of the point being computed)
+#pragma unroll
+      for (int c = 0; c < C; ++c) carry[c] = halp[c][rho];
+#pragma unroll
+      for (int aa = 0; aa < BP; ++aa) {
+        const int i = 2 * H - 1 - rho + 2 * H * aa;  // line updated in this sub-column
+        const int t = sc + gl * BP + aa + 1;         // its relative tier
+        const int odd = t & 1;
+        const bool act = KIND == KIND_UP ? (t > m) : (KIND == KIND_DOWN ? (t <= m) : true);
+        R win[C][2 * H + 1], bs[C][1], o[C][1];
+#pragma unroll
+        for (int c = 0; c < C; ++c) {
+#pragma unroll
+          for (int k = 0; k <= 2 * H; ++k)
+            win[c][k] = (i - k >= 0) ? v[c][(i - k >= 0) ? i - k : 0] : hal[c][(i - k >= 0) ? 0 : k - i - 1];
+          bs[c][0] = (Prob::SIGMA == 2 && !odd) ? carry[c] : win[c][H];
+        }
+        Prob::template stage<1>(win, bs, o, odd, kc);
+#pragma unroll
+        for (int c = 0; c < C; ++c) {
+          carry[c] = v[c][i];
+          if (act) v[c][i] = o[c][0];
+        }
+      }
+    }
+    // upper-left edge: the top 2h lines of the last lane leave the tile
+    if (KIND != KIND_DOWN && gl == L - 1) {
+#pragma unroll
+      for (int c = 0; c < C; ++c)
+#pragma unroll
+        for (int e = 0; e < 2 * H; ++e) io[c * RS + e] = v[c][B - 1 - e];
+    }
+  }
+  io += inc;
+  inc = 2 * H - inc;
+}
+
 template <class Prob, int B, int L, int KIND>
 __global__ void __launch_bounds__(128) swept_char_kernel(const TierArgs<typename Prob::R> a) {
   using R = typename Prob::R;
@@ -50,6 +113,7 @@ __global__ void __launch_bounds__(128) swept_char_kernel(const TierArgs<typename
   constexpr int m = n / (2 * H);    // super-columns per tile = tiers per half diamond
   constexpr int BP = B / (2 * H);   // points per lane per sub-column (chain length)
   static_assert(B % (2 * H) == 0, "lines per lane must be a multiple of 2h");
+  static_assert(L % 2 == 0 && m % 2 == 0 && m >= L, "step pairing needs even L, even m >= L");
   extern __shared__ __align__(128) unsigned char smem_raw[];
   const int T = blockDim.x;
   const int chunk = T * B;  // points staged by this CTA (T/L adjacent tiles)
@@ -101,7 +165,7 @@ __global__ void __launch_bounds__(128) swept_char_kernel(const TierArgs<typename
   const int ctr = PAD + (tid / L) * n + n / 2;  // smem slot of x' = 0 of this thread's tile
   auto slot = [&](int row, int c, int xp) -> R& { return rows[(row * C + c) * RS + ctr + xp]; };
 
-  R v[C][B], hal[C][2 * H], halp[C][2 * H];
+  R v[C][B], halA[C][2 * H], halB[C][2 * H];
   // initial line values: the point of line q just below the square (super-column -1), which is the latest
   // (or second latest) tier stored at x' = -(h tq + r + 1); Up: the anti-diagonal = tier-0 data
 #pragma unroll
@@ -122,61 +186,29 @@ __global__ void __launch_bounds__(128) swept_char_kernel(const TierArgs<typename
 #pragma unroll
   for (int c = 0; c < C; ++c)
 #pragma unroll
-    for (int e = 0; e < 2 * H; ++e) hal[c][e] = halp[c][e] = (R)0;
+    for (int e = 0; e < 2 * H; ++e) halA[c][e] = halB[c][e] = (R)0;
   __syncwarp();
 
-  for (int s = 0; s < m + L - 1; ++s) {
-    const int sc = s - gl;  // this lane's super-column
-    // halo: top 2h lines of the lower neighbour lane (it finished super-column sc one step ago);
-    // group lane 0 reads the staged lower-right edge: line -1-e at super-column sc is (x' = h sc + e, tier sc)
-    {
-      const int scc = sc < 0 ? 0 : (sc >= m ? m - 1 : sc);
-#pragma unroll
-      for (int c = 0; c < C; ++c)
-#pragma unroll
-        for (int e = 0; e < 2 * H; ++e) {
-          halp[c][e] = hal[c][e];
-          const R up = shfl_up_<R>(v[c][B - 1 - e], L);
-          hal[c][e] = up;
-          if (gl == 0) hal[c][e] = slot(scc & 1, c, H * scc + e);
-        }
-    }
-    if (sc >= 0 && sc < m) {
-#pragma unroll
-      for (int rho = 0; rho < 2 * H; ++rho) {
-        R carry[C];  // previous value of line i-2h (tier t-2 of the point being computed)
-#pragma unroll
-        for (int c = 0; c < C; ++c) carry[c] = halp[c][rho];
-#pragma unroll
-        for (int aa = 0; aa < BP; ++aa) {
-          const int i = 2 * H - 1 - rho + 2 * H * aa;  // line updated in this sub-column
-          const int t = sc + gl * BP + aa + 1;         // its relative tier
-          const int odd = t & 1;
-          const bool act = KIND == KIND_UP ? (t > m) : (KIND == KIND_DOWN ? (t <= m) : true);
-          R win[C][2 * H + 1], bs[C][1], o[C][1];
-#pragma unroll
-          for (int c = 0; c < C; ++c) {
-#pragma unroll
-            for (int k = 0; k <= 2 * H; ++k) win[c][k] = (i - k >= 0) ? v[c][(i - k >= 0) ? i - k : 0]
-                                                                      : hal[c][(i - k >= 0) ? 0 : k - i - 1];
-            bs[c][0] = (Prob::SIGMA == 2 && !odd) ? carry[c] : win[c][H];
-          }
-          Prob::template stage<1>(win, bs, o, odd, a.k);
-#pragma unroll
-          for (int c = 0; c < C; ++c) {
-            carry[c] = v[c][i];
-            if (act) v[c][i] = o[c][0];
-          }
-        }
-      }
-      // upper-left edge: the top 2h lines of the last lane leave the tile (x' = -n/2 + h sc + e, tier m+sc)
-      if (KIND != KIND_DOWN && gl == L - 1) {
-#pragma unroll
-        for (int c = 0; c < C; ++c)
-#pragma unroll
-          for (int e = 0; e < 2 * H; ++e) slot(sc & 1, c, -n / 2 + H * sc + e) = v[c][B - 1 - e];
-      }
-    }
+  // Loop I/O goes through one per-thread pointer: element (row sc&1, x' = base + h sc) with
+  //   reader (group lane 0)    base = 0      : line -1-e at super-column sc is (x' = h sc + e,        tier sc)
+  //   writer (group lane L-1)  base = -n/2   : its top line e leaves at       (x' = -n/2 + h sc + e, tier m+sc)
+  // advanced by h and toggled between the two rows every step (inc alternates h + C RS, h - C RS).
+  const int sc0 = -gl;
+  R* io = rows + ((sc0 & 1) * C) * RS + ctr + (gl == 0 ? 0 : -n / 2) + H * sc0;
+  int inc = H + ((sc0 & 1) ? -C * RS : C * RS);
+
+  int s = 0;
+  for (; s < L; s += 2) {  // ramp up: lane gl starts at step gl
+    char_step<Prob, B, L, KIND, true>(v, halA, halB, io, inc, s, gl, RS, a.k);
+    char_step<Prob, B, L, KIND, true>(v, halB, halA, io, inc, s + 1, gl, RS, a.k);
+  }
+  for (; s < m; s += 2) {  // steady state: every lane is inside its m super-columns
+    char_step<Prob, B, L, KIND, false>(v, halA, halB, io, inc, s, gl, RS, a.k);
+    char_step<Prob, B, L, KIND, false>(v, halB, halA, io, inc, s + 1, gl, RS, a.k);
+  }
+  for (; s < m + L; s += 2) {  // ramp down (the last step, s = m+L-1, is empty and keeps the pairing)
+    char_step<Prob, B, L, KIND, true>(v, halA, halB, io, inc, s, gl, RS, a.k);
+    char_step<Prob, B, L, KIND, true>(v, halB, halA, io, inc, s + 1, gl, RS, a.k);
   }
   __syncwarp();
   // upper-right edge (Down: the full time level): last value of every line
