@@ -16,7 +16,12 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 BUILD = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libswept_b200.so")
-SOURCES = ["swept_api.cu", "probes.cu", "kernels_heat.cu", "kernels_ks.cu", "kernels_euler.cu"]
+# (source, object stem, extra defines); the Euler swept kernels are compiled in six parallel slices
+SOURCES = [("swept_api.cu", "swept_api", []), ("probes.cu", "probes", []),
+           ("kernels_heat.cu", "kernels_heat", []), ("kernels_ks.cu", "kernels_ks", []),
+           ("kernels_euler.cu", "kernels_euler", [])]
+SOURCES += [("kernels_euler_inst.cu", f"kernels_euler_i{i}r{r}", [f"-DSWEPT_INST={i}", f"-DSWEPT_RK2={r}"])
+            for i in (2, 1, 0) for r in (0, 1)]
 NVCC_FLAGS = ["-std=c++17", "-O3", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "-fmad=false", "-prec-div=true", "-prec-sqrt=true", "-ftz=false",
               "-Xcompiler", "-fPIC"]
@@ -43,19 +48,20 @@ def build(force: bool = False, verbose: bool = False) -> str:
     os.makedirs(BUILD, exist_ok=True)
     nvcc = _nvcc()
 
-    def compile_one(src: str) -> str:
-        obj = os.path.join(BUILD, src.replace(".cu", ".o"))
-        cmd = [nvcc, *NVCC_FLAGS, "-c", os.path.join(CSRC, src), "-o", obj]
+    def compile_one(item) -> str:
+        src, stem, defs = item
+        obj = os.path.join(BUILD, stem + ".o")
+        cmd = [nvcc, *NVCC_FLAGS, *defs, "-c", os.path.join(CSRC, src), "-o", obj]
         if verbose:
             cmd.insert(1, "-Xptxas=-v")
         r = subprocess.run(cmd, capture_output=True, text=True)
         if r.returncode != 0:
-            raise RuntimeError(f"nvcc failed for {src}:\n{r.stdout}\n{r.stderr}")
+            raise RuntimeError(f"nvcc failed for {stem}:\n{r.stdout}\n{r.stderr}")
         if verbose:
             sys.stderr.write(r.stderr)
         return obj
 
-    with cf.ThreadPoolExecutor(max_workers=len(SOURCES)) as ex:
+    with cf.ThreadPoolExecutor(max_workers=min(len(SOURCES), os.cpu_count() or 4)) as ex:
         objs = list(ex.map(compile_one, SOURCES))
     tmp = LIB + f".tmp{os.getpid()}"
     r = subprocess.run([nvcc, "-shared", "-o", tmp, *objs], capture_output=True, text=True)

@@ -1,6 +1,15 @@
-// kernels_euler.cu — Euler equations / Sod tube (App. D) kernel instantiations, FP64.
+// kernels_euler.cu — Euler equations / Sod tube (App. D) host dispatch, FP64.
+// The swept kernels themselves are instantiated in kernels_euler_inst.cu, compiled once per
+// (flavour, integrator) slice so that the slices build in parallel (see build.py).
 #include "kernels_impl.cuh"
 namespace swept {
+extern template int tier_T<Euler<double, 0>, 4>(const TileLaunch&);
+extern template int tier_T<Euler<double, 1>, 4>(const TileLaunch&);
+extern template int char_L<Euler<double, 0>, 8>(const TileLaunch&);
+extern template int char_L<Euler<double, 1>, 8>(const TileLaunch&);
+extern template int char_L<Euler<double, 0>, 16>(const TileLaunch&);
+extern template int char_L<Euler<double, 1>, 16>(const TileLaunch&);
+
 int launch_per_step_euler(int dtype, int rk2, const PerStepLaunch& a) {
   if (dtype != 0) return NO_KERNEL;
   return rk2 == 0 ? per_step_T<Euler<double, 0>, 2>(a) : per_step_T<Euler<double, 1>, 2>(a);

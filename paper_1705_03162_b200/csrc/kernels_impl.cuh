@@ -75,7 +75,7 @@ inline bool tier_ok(int n, int P, int pmax) {
 }
 
 template <class Prob, int PMAX>
-inline int tier_T(const TileLaunch& a) {
+int tier_T(const TileLaunch& a) {
   if (!tier_ok<Prob>(a.n, a.P, PMAX)) return NO_KERNEL;
   switch (a.P) {
     case 1: return tier_kind<Prob, 1>(a);
@@ -134,7 +134,7 @@ inline bool char_ok(int64_t N, int n, int L) {
 }
 
 template <class Prob, int B>
-inline int char_L(const TileLaunch& a) {
+int char_L(const TileLaunch& a) {
   switch (a.P) {
     case 8: return char_kind<Prob, B, 8>(a);
     case 16: return char_kind<Prob, B, 16>(a);
@@ -144,7 +144,7 @@ inline int char_L(const TileLaunch& a) {
 }
 
 template <class Prob, int BMAX>
-inline int char_T(const TileLaunch& a) {
+int char_T(const TileLaunch& a) {
   if (!char_ok<Prob, BMAX>(a.N, a.n, a.P)) return NO_KERNEL;
   switch (a.n / a.P) {
     case 8: return char_L<Prob, 8>(a);
