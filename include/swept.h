@@ -138,17 +138,22 @@ const char* swept_last_error(void);
 
 /* One phase of the swept schedule: kind 0 Up, 1 SplitDiamond, 2 WholeDiamond, 3 Down,
  * 4 per-step remainder.  `shift` = offset of the tiling in points (0 or n/2), `tier0` = global sub-timestep
- * index at which the phase's relative tier 0 sits, `ntiers` = tiers it computes at its tallest column. */
+ * index at which the phase's relative tier 0 sits, `ntiers` = tiers it computes at its tallest column,
+ * `n` = tile width of the phase (0 for the per-step remainder). */
 typedef struct {
   int32_t kind;
   int32_t shift;
   int64_t tier0;
   int64_t ntiers;
+  int32_t n;
+  int32_t reserved;
 } swept_phase;
 
-/* swept_plan — the phase list swept_run would execute for nsub = sigma*nsteps sub-timesteps with tile width
- * n and stencil half-width h.  Writes at most max_phases entries, returns the number of phases needed
- * (or a negative error code). */
+/* swept_plan — the phase list swept_run executes for nsub = sigma*nsteps sub-timesteps with tile width n and
+ * stencil half-width h: one Up / D diamonds / Down cycle of width n covering the largest T = (D+1) n/(2h) <= nsub
+ * (PAPER.md:83), then further cycles of width n/2, n/4, ... >= 32 for what is left (reading G5),
+ * then a per-step remainder.  (swept_run additionally skips widths for which N has no kernel.)
+ * Writes at most max_phases entries, returns the number of phases needed (or a negative error code). */
 int64_t swept_plan(int64_t nsub, int32_t n, int32_t h, swept_phase* out, int64_t max_phases);
 
 /* ---- measurement helpers --------------------------------------------------------------------------- */

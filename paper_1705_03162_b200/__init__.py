@@ -35,7 +35,8 @@ class swept_params(Structure):
 
 
 class swept_phase(Structure):
-    _fields_ = [("kind", c_int32), ("shift", c_int32), ("tier0", c_int64), ("ntiers", c_int64)]
+    _fields_ = [("kind", c_int32), ("shift", c_int32), ("tier0", c_int64), ("ntiers", c_int64),
+                ("n", c_int32), ("reserved", c_int32)]
 
 
 class SweptError(RuntimeError):
@@ -184,7 +185,7 @@ def swept_plan(nsub: int, n: int, h: int):
         raise SweptError(f"swept_plan: {swept_last_error()}")
     arr = (swept_phase * max(cnt, 1))()
     lib.swept_plan(nsub, n, h, arr, cnt)
-    return [(int(a.kind), int(a.shift), int(a.tier0), int(a.ntiers)) for a in arr[:cnt]]
+    return [(int(a.kind), int(a.shift), int(a.tier0), int(a.ntiers), int(a.n)) for a in arr[:cnt]]
 
 
 def swept_probe_fp64(device: int = -1) -> float:

@@ -42,6 +42,20 @@ def _deps_mtime() -> float:
     return max(t, os.path.getmtime(__file__))
 
 
+def _includes(path: str, seen: set) -> set:
+    """Transitive closure of the quoted #include files of `path` (for per-object staleness)."""
+    if path in seen or not os.path.exists(path):
+        return seen
+    seen.add(path)
+    with open(path) as f:
+        for line in f:
+            line = line.strip()
+            if line.startswith("#include \""):
+                inc = line.split('"')[1]
+                _includes(os.path.normpath(os.path.join(os.path.dirname(path), inc)), seen)
+    return seen
+
+
 def build(force: bool = False, verbose: bool = False) -> str:
     if not force and os.path.exists(LIB) and os.path.getmtime(LIB) >= _deps_mtime():
         return LIB
@@ -51,6 +65,10 @@ def build(force: bool = False, verbose: bool = False) -> str:
     def compile_one(item) -> str:
         src, stem, defs = item
         obj = os.path.join(BUILD, stem + ".o")
+        deps = _includes(os.path.join(CSRC, src), set()) | {os.path.abspath(__file__)}
+        if not force and not verbose and os.path.exists(obj) and \
+                os.path.getmtime(obj) >= max(os.path.getmtime(d) for d in deps):
+            return obj
         cmd = [nvcc, *NVCC_FLAGS, *defs, "-c", os.path.join(CSRC, src), "-o", obj]
         if verbose:
             cmd.insert(1, "-Xptxas=-v")

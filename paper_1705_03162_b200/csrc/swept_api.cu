@@ -198,22 +198,39 @@ int run_per_step(swept_state* s, int64_t steps, int threads) {
 }
 
 // ---- swept phase plan -------------------------------------------------------------------------------
-int64_t make_plan(int64_t nsub, int n, int h, std::vector<swept_phase>* out) {
-  if (n < 4 * h || (n & (n - 1)) || nsub < 0) return SWEPT_EINVAL;
-  const int64_t m = n / (2 * h);
+// One Up / D diamonds / Down cycle per admissible tile width, widest first (reading G5 of DESIGN.md §3): the
+// sub-timesteps a cycle of width w cannot cover (fewer than m_w = w/(2h)) go to the next narrower width, and
+// what is left below the narrowest one is finished with per-step launches.  Between cycles the state is a
+// plain time level, so every cycle starts with an UpTriangle from row 0.
+int64_t make_plan(int64_t nsub, const std::vector<int>& widths, int h, std::vector<swept_phase>* out) {
+  if (nsub < 0 || widths.empty()) return SWEPT_EINVAL;
   int64_t done = 0;
-  if (nsub >= m) {
-    const int64_t D = nsub / m - 1;
-    out->push_back({KIND_UP, 0, 0, m - 1});
+  for (int n : widths) {
+    if (n < 4 * h || (n & (n - 1))) return SWEPT_EINVAL;
+    const int64_t m = n / (2 * h);
+    const int64_t left = nsub - done;
+    if (left < m) continue;
+    const int64_t D = left / m - 1;
+    out->push_back({KIND_UP, 0, done, m - 1, n, 0});
     for (int64_t k = 1; k <= D; ++k) {
       const bool split = (k & 1) != 0;
-      out->push_back({split ? KIND_SPLIT : KIND_WHOLE, split ? n / 2 : 0, (k - 1) * m, 2 * m - 1});
+      out->push_back({split ? KIND_SPLIT : KIND_WHOLE, split ? n / 2 : 0, done + (k - 1) * m, 2 * m - 1, n, 0});
     }
-    out->push_back({KIND_DOWN, (D & 1) ? 0 : n / 2, D * m, m});
-    done = (D + 1) * m;
+    out->push_back({KIND_DOWN, (D & 1) ? 0 : n / 2, done + D * m, m, n, 0});
+    done += (D + 1) * m;
   }
-  if (nsub > done) out->push_back({KIND_REMAINDER, 0, done, nsub - done});
+  if (nsub > done) out->push_back({KIND_REMAINDER, 0, done, nsub - done, 0, 0});
   return (int64_t)out->size();
+}
+
+constexpr int MIN_LEVEL_WIDTH = 32;  // narrowest tile of the remainder cycles
+
+int tier_default_P(const swept_state* s, int n) {
+  const int pmax = 4, tmax = s->problem == SWEPT_EULER ? 256 : 1024;
+  int P = std::min(pmax, std::max(1, n / 256));
+  while (P < pmax && n / P > tmax) P *= 2;
+  if (P == 3) P = 2;
+  return P;
 }
 
 void default_tile(const swept_state* s, int* n_io, int* flavor_io, int* P_io) {
@@ -237,16 +254,39 @@ void default_tile(const swept_state* s, int* n_io, int* flavor_io, int* P_io) {
     P = 0;
   }
   if (P == 0) {
-    if (flavor == SWEPT_FLAVOR_TIER) {
-      const int pmax = 4, tmax = s->problem == SWEPT_EULER ? 256 : 1024;
-      P = std::min(pmax, std::max(1, n / 256));
-      while (P < pmax && n / P > tmax) P *= 2;
-      if (P == 3) P = 2;
-    }
+    if (flavor == SWEPT_FLAVOR_TIER) P = tier_default_P(s, n);
   }
   *n_io = n;
   *flavor_io = flavor;
   *P_io = P;
+}
+
+// kernel configuration of a remainder cycle of width n, as close as possible to the top-level (flavor, P)
+bool level_config(const swept_state* s, int n_top, int flavor_top, int P_top, int n, int* flavor, int* P) {
+  if (n == n_top) {
+    *flavor = flavor_top;
+    *P = P_top;
+    return tile_ok(s, flavor_top, n, P_top);
+  }
+  if (flavor_top == SWEPT_FLAVOR_CHAR) {
+    const int B_top = n_top / P_top;
+    for (int B : {B_top, 16, 8, 32}) {
+      if (n % B) continue;
+      if (tile_ok(s, SWEPT_FLAVOR_CHAR, n, n / B)) {
+        *flavor = SWEPT_FLAVOR_CHAR;
+        *P = n / B;
+        return true;
+      }
+    }
+  }
+  for (int Pt : {tier_default_P(s, n), 1, 2, 4}) {
+    if (tile_ok(s, SWEPT_FLAVOR_TIER, n, Pt)) {
+      *flavor = SWEPT_FLAVOR_TIER;
+      *P = Pt;
+      return true;
+    }
+  }
+  return false;
 }
 
 int run_swept(swept_state* s, int64_t nsteps, int n, int flavor, int P) {
@@ -256,8 +296,17 @@ int run_swept(swept_state* s, int64_t nsteps, int n, int flavor, int P) {
   if (!tile_ok(s, flavor, n, P))
     return fail(s->N % n ? SWEPT_EINVAL : SWEPT_EUNSUPPORTED,
                 "tile_width=%d (flavor %d, P=%d) not admissible for N=%lld", n, flavor, P, (long long)s->N);
+  // widths of the cycles: n, then every narrower power of two that has a kernel for this N
+  std::vector<int> widths;
+  std::map<int, std::pair<int, int>> cfg;
+  for (int w = n; w >= MIN_LEVEL_WIDTH && w >= 8 * sh.h; w /= 2) {
+    int fl = 0, Pl = 0;
+    if (!level_config(s, n, flavor, P, w, &fl, &Pl)) continue;
+    widths.push_back(w);
+    cfg[w] = {fl, Pl};
+  }
   std::vector<swept_phase> plan;
-  const int64_t np = make_plan(nsteps * sh.sigma, n, sh.h, &plan);
+  const int64_t np = make_plan(nsteps * sh.sigma, widths, sh.h, &plan);
   if (np < 0) return fail(SWEPT_EINVAL, "cannot plan tile_width=%d", n);
   int r0 = -1, r1 = -1;  // slabs holding the current two-row state
   for (const swept_phase& ph : plan) {
@@ -267,11 +316,11 @@ int run_swept(swept_state* s, int64_t nsteps, int n, int flavor, int P) {
     }
     swept::TileLaunch a{};
     a.kind = ph.kind;
-    a.n = n;
+    a.n = ph.n;
     a.shift = ph.shift;
     a.ntiers = (int)ph.ntiers;
-    a.P = P;
-    a.flavor = flavor;
+    a.flavor = cfg[ph.n].first;
+    a.P = cfg[ph.n].second;
     int o0, o1;
     if (ph.kind == KIND_UP) {
       o0 = (s->cur + 1) & 3;
@@ -461,8 +510,11 @@ int swept_run(swept_state* s, int64_t nsteps, int32_t tile_width, int variant) {
 
 int64_t swept_plan(int64_t nsub, int32_t n, int32_t h, swept_phase* out, int64_t max_phases) {
   if (h != 1 && h != 2) return fail(SWEPT_EINVAL, "h must be 1 or 2");
+  if (n < 8 * h || (n & (n - 1))) return fail(SWEPT_EINVAL, "tile width %d not plannable for h=%d", n, h);
+  std::vector<int> widths;
+  for (int w = n; w == n || (w >= MIN_LEVEL_WIDTH && w >= 8 * h); w /= 2) widths.push_back(w);
   std::vector<swept_phase> plan;
-  const int64_t np = make_plan(nsub, n, h, &plan);
+  const int64_t np = make_plan(nsub, widths, h, &plan);
   if (np < 0) return fail(SWEPT_EINVAL, "tile width %d not plannable for h=%d", n, h);
   if (out)
     for (int64_t i = 0; i < np && i < max_phases; ++i) out[i] = plan[(size_t)i];

@@ -29,7 +29,7 @@ def simulate(N, n, h, sigma, nsub):
     bufs[0][0] = [0] * N  # tier 0 everywhere in row 0
     cur, updates, launches = 0, 0, 0
     field_tier = 0
-    for kind, shift, tier0, ntiers in plan:
+    for kind, shift, tier0, ntiers, n_ph in plan:
         if kind == REM:
             assert tier0 == field_tier and ntiers % sigma == 0
             field_tier += ntiers
@@ -37,6 +37,8 @@ def simulate(N, n, h, sigma, nsub):
             launches += ntiers
             continue
         launches += 1
+        assert n_ph <= n and n % n_ph == 0
+        n = n_ph  # remainder cycles use narrower tiles (reading G5)
         src, dst = bufs[cur], bufs[1 - cur]
         new_dst = [list(dst[0]), list(dst[1])]
         assert N % n == 0 and shift in (0, n // 2)
@@ -104,6 +106,22 @@ def test_remainder_policy_g5(nsub):
     assert (len(rem) == 1 and rem[0][3] == nsub % m) if nsub % m else not rem
 
 
+@pytest.mark.parametrize("N,n,h,sigma,nsub", [(256, 128, 1, 1, 64 + 32 + 16 + 5), (256, 128, 1, 1, 3 * 64 + 16),
+                                              (256, 256, 2, 2, 64 + 2 * 16 + 8 + 6), (512, 128, 2, 2, 5 * 32 + 30),
+                                              (128, 128, 1, 1, 1000)])
+def test_multi_level_remainder_g5(N, n, h, sigma, nsub):
+    # what a cycle of width n cannot cover goes to cycles of width n/2, n/4, ... >= 32, then per-step
+    plan, launches = simulate(N, n, h, sigma, nsub)
+    widths = [p[4] for p in plan if p[0] != REM]
+    assert widths == sorted(widths, reverse=True) and widths[0] == n
+    rem = sum(p[3] for p in plan if p[0] == REM)
+    assert rem < 32 // (2 * h), "only less than the narrowest tile's m sub-timesteps go per-step"
+    for w in set(widths):  # every cycle is Up, diamonds, Down
+        kinds = [p[0] for p in plan if p[4] == w and p[0] != REM]
+        assert kinds[0] == UP and kinds[-1] == DOWN and all(k in (SPLIT, WHOLE) for k in kinds[1:-1])
+    assert launches < nsub or nsub < 32 // (2 * h)
+
+
 def test_paper_counts():
     # the triangle of a 512-point node holds 65 792 values (incl. the initial row), h = 1
     n, h = 512, 1
@@ -117,7 +135,7 @@ def test_paper_counts():
     assert sw.swept_plan(64 * 10, 64, 1)[1][3] == 63
     # launch counts: heat N=2^20 n=256, 50 000 steps: D + 2 launches (~392)
     plan = sw.swept_plan(50000, 256, 1)
-    assert sum(1 for p in plan if p[0] != REM) == 50000 // 128 + 1 == 391
+    assert sum(1 for p in plan if p[4] == 256) == 50000 // 128 + 1 == 391
 
 
 def test_plan_rejects_bad_arguments():
