@@ -28,7 +28,7 @@ def test_every_declared_symbol_is_exported():
 def test_params_struct_matches_header():
     # 4 x 4-byte + 2 doubles + 4 pointers
     assert ctypes.sizeof(sw.swept_params) == 16 + 16 + 32
-    assert ctypes.sizeof(sw.swept_phase) == 24
+    assert ctypes.sizeof(sw.swept_phase) == 32  # 2 x int32, 2 x int64, 2 x int32
 
 
 def test_no_cpu_fallback():
