@@ -120,6 +120,23 @@ def read_peaks():
 
 
 # ----------------------------------------------------------------------------------------------------
+def max_over_ranks(ms: float, dist, device) -> float:
+    """Replicas only: the job's time is the slowest rank's device time.  `dist` is
+    torch.distributed (initialised) or None for a single process."""
+    if dist is None:
+        return float(ms)
+    import torch
+    t = torch.tensor([ms], device=device, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def replica_value(updates_per_step: int, steps: int, world: int, max_ms: float) -> float:
+    """Whole-job throughput: every rank advanced `updates_per_step * steps` point-timesteps."""
+    return world * updates_per_step * steps / (max_ms * 1e-3)
+
+
+# ----------------------------------------------------------------------------------------------------
 def oracle_sample(w, budget_s: float = 12.0):
     """Time the oracle, as it stands, on a bounded sample of workload `w` (same N, fewer steps)."""
     import oracle
@@ -252,6 +269,8 @@ def main():
 
     for _ in range(args.warmup):
         one_step()
+    state.phase_times()
+    state.set_phase_timing(True)  # CUDA-event pair around every swept launch, on the library's stream
     barrier()
     with ClockSampler(local) as clk:
         t_wall0 = time.perf_counter()
@@ -262,12 +281,11 @@ def main():
     step_ms = [a.elapsed_time(b) for a, b in e_pairs]
     total_ms = sum(step_ms)
     launches_per_step = state.last_launches
-    if dist is not None:
-        t = torch.tensor([total_ms], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        total_ms = float(t.item())
+    phase = state.phase_times()  # per-kind device time of this rank's launches inside the timed region
+    state.set_phase_timing(False)
+    total_ms = max_over_ranks(total_ms, dist, "cuda")
     updates_per_step = w.N * nsteps
-    value = world * updates_per_step * args.steps / (total_ms * 1e-3)
+    value = replica_value(updates_per_step, args.steps, world, total_ms)
 
     # ---- end to end through the C ABI with host buffers (pinned), copies inside the timed region
     host_in = torch.from_numpy(np.ascontiguousarray(w.u0)).pin_memory()
@@ -287,11 +305,8 @@ def main():
         if r >= 2:
             e2e_ms.append(a.elapsed_time(b))
     e2e_total = sum(e2e_ms)
-    if dist is not None:
-        t = torch.tensor([e2e_total], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e_total = float(t.item())
-    e2e_value = world * updates_per_step * args.steps / (e2e_total * 1e-3)
+    e2e_total = max_over_ranks(e2e_total, dist, "cuda")
+    e2e_value = replica_value(updates_per_step, args.steps, world, e2e_total)
     final_field = host_out.numpy().copy()
 
     if rank != 0:
@@ -308,21 +323,35 @@ def main():
     peak_tflops = sms * FP64_LANES_PER_CLK_PER_SM * 2 * sm_max * 1e6 / 1e12
     probe = sw.swept_probe_fp64()
     plan = sw.swept_plan(nsteps * state.sigma, tile, state.h)
-    n_tile_launches = sum(1 for p in plan if p[0] != 4)
-    n_diamonds = sum(1 for p in plan if p[0] in (1, 2))
+    m_top = tile // (2 * state.h)
+    # dominant kernel = the Split/WholeDiamond launches of the top-level cycle: N * m updates per launch,
+    # 3 FP64-pipe instructions per update (DADD, DMUL, DFMA) = 6 FMA-equivalent flops
+    d_ms = phase["SplitDiamond"][0] + phase["WholeDiamond"][0]
+    d_cnt = phase["SplitDiamond"][1] + phase["WholeDiamond"][1]
+    n_diamonds_top = sum(1 for p in plan if p[0] in (1, 2) and p[4] == tile)
+    n_diamonds_all = sum(1 for p in plan if p[0] in (1, 2))
     fp64_instr_per_update = 3
-    ach_tflops = fp64_instr_per_update * 2 * (updates_per_step * args.steps / (total_ms * 1e-3)) / 1e12 \
-        * (1 if world == 1 else 1.0 / world)
+    if d_cnt and n_diamonds_all == n_diamonds_top:
+        avg_launch_ms = d_ms / d_cnt
+        ach_tflops = fp64_instr_per_update * 2 * w.N * m_top / (avg_launch_ms * 1e-3) / 1e12
+        how = "CUDA events around every Split/WholeDiamond launch of the timed region (swept_phase_times)"
+    else:  # flavours without per-launch phases, or diamonds of several widths: whole-step figure
+        avg_launch_ms = total_ms / args.steps
+        ach_tflops = fp64_instr_per_update * 2 * updates_per_step / (avg_launch_ms * 1e-3) / 1e12
+        how = "whole swept_run (all phases) timed with CUDA events"
+    step_tflops = fp64_instr_per_update * 2 * updates_per_step / (total_ms / args.steps * 1e-3) / 1e12
     roofline = {"bound": "alu", "achieved": ach_tflops, "peak": peak_tflops, "unit": "TFLOP/s",
                 "frac": ach_tflops / peak_tflops, "traffic": None,
-                "kernel": "swept Split/WholeDiamond (heat FP64)",
-                "note": "FMA-equivalent FP64 flops = 2 x 3 FP64-pipe instructions per update; peak = "
-                        f"{sms} SM x 64 lanes x 2 x {sm_max:.0f} MHz (nominal unit count, max clock); "
-                        "probe = live DFMA-chain measurement",
+                "kernel": "swept Split/WholeDiamond (heat FP64)", "timed_by": how,
+                "note": "FMA-equivalent FP64 flops = 2 x 3 FP64-pipe instructions per update, N*m updates per "
+                        f"launch (m = {m_top}); peak = {sms} SM x 64 lanes x 2 x {sm_max:.0f} MHz (nominal unit "
+                        "count, max clock); probe = live DFMA-chain measurement",
                 "peak_probe_tflops": probe * 2 / 1e12,
                 "frac_of_probe": ach_tflops / (probe * 2 / 1e12) if probe else None,
-                "avg_launch_ms": total_ms / args.steps / max(n_tile_launches, 1),
-                "diamond_launches_per_step": n_diamonds}
+                "avg_launch_ms": avg_launch_ms, "diamond_launches_timed": d_cnt,
+                "whole_step_tflops": step_tflops, "whole_step_frac": step_tflops / peak_tflops,
+                "phase_ms_per_step": {k: v[0] / args.steps for k, v in phase.items()},
+                "phase_launches_per_step": {k: v[1] / args.steps for k, v in phase.items()}}
     try:
         with open(os.path.join(ROOT, "profiles", "traffic.json")) as f:
             roofline["traffic"] = json.load(f).get("heat_diamond_dram_bytes_per_launch")

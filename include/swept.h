@@ -129,6 +129,17 @@ int64_t swept_steps_done(const swept_state* s);
 /* swept_last_launches — number of kernel launches (graph nodes included) issued by the last swept_run. */
 int64_t swept_last_launches(const swept_state* s);
 
+/* swept_set_phase_timing — on != 0: every later swept_run brackets each swept launch (and the per-step
+ * remainder as a whole) with a pair of CUDA events recorded on the state's stream, so that the duration of
+ * each kernel kind can be measured live, inside a timed region, without a profiler.  Off by default. */
+int swept_set_phase_timing(swept_state* s, int on);
+
+/* swept_phase_times — synchronise the stream and return, per phase kind (index 0 Up, 1 SplitDiamond,
+ * 2 WholeDiamond, 3 Down, 4 per-step remainder), the summed device time in milliseconds and the number of
+ * kernel launches recorded since timing was switched on or since the previous call; then reset the record.
+ * ms and launches are caller-owned HOST arrays of 5 entries. */
+int swept_phase_times(swept_state* s, double* ms, int64_t* launches);
+
 void swept_destroy(swept_state* s);
 
 /* swept_last_error — thread-local message of the last failing call on this thread. */

@@ -80,6 +80,8 @@ def load():
     lib.swept_plan.argtypes = [c_int64, c_int32, c_int32, POINTER(swept_phase), c_int64]
     lib.swept_probe_fp64.argtypes = [c_int, c_void_p, POINTER(c_double)]
     lib.swept_probe_launch.argtypes = [c_int, c_void_p, c_int, POINTER(c_double)]
+    lib.swept_set_phase_timing.argtypes = [c_void_p, c_int]
+    lib.swept_phase_times.argtypes = [c_void_p, POINTER(c_double), POINTER(c_int64)]
     lib.swept_tuned.argtypes = [c_void_p, c_int, POINTER(c_int32), POINTER(c_int32), POINTER(c_int32)]
     _lib = lib
     return lib
@@ -170,6 +172,17 @@ def swept_tuned(state: int, variant: int):
     return int(n.value), int(fl.value), int(g.value)
 
 
+def swept_set_phase_timing(state: int, on: bool) -> None:
+    _check(load().swept_set_phase_timing(state, 1 if on else 0))
+
+
+def swept_phase_times(state: int):
+    """{kind name: (milliseconds, launches)} recorded since timing was switched on / the previous call."""
+    ms, cnt = (c_double * 5)(), (c_int64 * 5)()
+    _check(load().swept_phase_times(state, ms, cnt))
+    return {KIND_NAMES[k]: (float(ms[k]), int(cnt[k])) for k in range(5)}
+
+
 def swept_set_stream(state: int, stream: int) -> None:
     _check(load().swept_set_stream(state, stream))
 
@@ -242,6 +255,13 @@ class Swept:
     def autotune(self, variant: int = SWEPT) -> int:
         swept_set_stream(self._h, _current_stream())
         return swept_autotune(self._h, variant)
+
+    def set_phase_timing(self, on: bool) -> None:
+        swept_set_phase_timing(self._h, on)
+
+    def phase_times(self):
+        swept_set_stream(self._h, _current_stream())
+        return swept_phase_times(self._h)
 
     def tuned(self, variant: int = SWEPT):
         return swept_tuned(self._h, variant)

@@ -73,6 +73,11 @@ struct swept_state {
   int tuned_width[2] = {0, 0};
   int tuned_flavor = 0, tuned_P = 0;
   std::map<GraphKey, cudaGraphExec_t> graphs;
+  // live per-kind timing (swept_set_phase_timing): event pairs recorded around launches
+  struct Timed { int kind; int64_t launches; cudaEvent_t e0, e1; };
+  bool timing = false;
+  std::vector<Timed> timed;
+  std::vector<cudaEvent_t> event_pool;
   size_t elem() const { return dtype == SWEPT_F64 ? 8 : 4; }
 };
 
@@ -113,6 +118,34 @@ int launch_tile(swept_state* s, swept::TileLaunch& a) {
   if (rc != 0) return fail(SWEPT_ECUDA, "swept launch: %s", cudaGetErrorString((cudaError_t)rc));
   return 0;
 }
+
+cudaEvent_t take_event(swept_state* s) {
+  cudaEvent_t e = nullptr;
+  if (!s->event_pool.empty()) {
+    e = s->event_pool.back();
+    s->event_pool.pop_back();
+  } else {
+    cudaEventCreate(&e);
+  }
+  return e;
+}
+
+// RAII bracket: records e0 now and e1 at scope exit when phase timing is on
+struct TimedScope {
+  swept_state* s;
+  size_t idx = 0;
+  bool on;
+  TimedScope(swept_state* s_, int kind, int64_t launches) : s(s_), on(s_->timing) {
+    if (!on) return;
+    swept_state::Timed t{kind, launches, take_event(s), take_event(s)};
+    cudaEventRecord(t.e0, s->stream);
+    idx = s->timed.size();
+    s->timed.push_back(t);
+  }
+  ~TimedScope() {
+    if (on) cudaEventRecord(s->timed[idx].e1, s->stream);
+  }
+};
 
 bool tile_ok(const swept_state* s, int flavor, int n, int P) {
   if (n <= 0 || s->N % n != 0) return false;
@@ -242,19 +275,34 @@ void default_tile(const swept_state* s, int* n_io, int* flavor_io, int* P_io) {
       P = s->tuned_P;
     }
   }
+  // untuned defaults (measured on B200): heat and KS run fastest with the register-resident
+  // CHAR flavour on wide tiles, Euler (about 250 live registers per point) with the TIER flavour
+  const bool want_char = flavor == SWEPT_FLAVOR_CHAR || (flavor == SWEPT_FLAVOR_AUTO && s->problem != SWEPT_EULER);
   if (n == 0) {
-    for (int cand : {256, 512, 128, 1024, 64, 32, 2048, 4096})
-      if (s->N % cand == 0) {
-        n = cand;
-        break;
-      }
+    if (want_char) {
+      for (int cand : {1024, 512, 256, 128, 64})
+        for (int L : {32, 16, 8})
+          if (n == 0 && (P == 0 || P == L) && tile_ok(s, SWEPT_FLAVOR_CHAR, cand, L)) n = cand;
+    }
+    if (n == 0 && flavor != SWEPT_FLAVOR_CHAR)
+      for (int cand : {512, 256, 128, 1024, 64, 32, 2048, 4096})
+        if (n == 0 && s->N % cand == 0) n = cand;
   }
   if (flavor == SWEPT_FLAVOR_AUTO) {
     flavor = SWEPT_FLAVOR_TIER;
     P = 0;
+    if (want_char)
+      for (int L : {32, 16, 8})
+        if (flavor == SWEPT_FLAVOR_TIER && tile_ok(s, SWEPT_FLAVOR_CHAR, n, L)) {
+          flavor = SWEPT_FLAVOR_CHAR;
+          P = L;
+        }
   }
   if (P == 0) {
     if (flavor == SWEPT_FLAVOR_TIER) P = tier_default_P(s, n);
+    else
+      for (int L : {32, 16, 8})
+        if (P == 0 && tile_ok(s, SWEPT_FLAVOR_CHAR, n, L)) P = L;
   }
   *n_io = n;
   *flavor_io = flavor;
@@ -311,6 +359,7 @@ int run_swept(swept_state* s, int64_t nsteps, int n, int flavor, int P) {
   int r0 = -1, r1 = -1;  // slabs holding the current two-row state
   for (const swept_phase& ph : plan) {
     if (ph.kind == KIND_REMAINDER) {
+      TimedScope ts(s, KIND_REMAINDER, ph.ntiers);
       if (int rc = run_per_step(s, ph.ntiers / sh.sigma, 0)) return rc;
       continue;
     }
@@ -339,7 +388,10 @@ int run_swept(swept_state* s, int64_t nsteps, int n, int flavor, int P) {
     }
     a.out0 = s->slab[o0];
     a.out1 = s->slab[o1];
-    if (int rc = launch_tile(s, a)) return rc;
+    {
+      TimedScope ts(s, ph.kind, 1);
+      if (int rc = launch_tile(s, a)) return rc;
+    }
     s->last_launches += 1;
     r0 = o0;
     r1 = o1;
@@ -440,6 +492,8 @@ void swept_destroy(swept_state* s) {
   cudaStreamSynchronize(s->stream);
   for (auto& kv : s->graphs) cudaGraphExecDestroy(kv.second);
   if (s->capture_stream) cudaStreamDestroy(s->capture_stream);
+  for (auto& t : s->timed) { cudaEventDestroy(t.e0); cudaEventDestroy(t.e1); }
+  for (cudaEvent_t e : s->event_pool) cudaEventDestroy(e);
   for (int i = 0; i < 4; ++i) {
     if (!s->slab[i]) continue;
     if (s->free_) s->free_(s->alloc_ctx, s->slab[i]);
@@ -451,6 +505,31 @@ void swept_destroy(swept_state* s) {
 int swept_set_stream(swept_state* s, void* stream) {
   if (!s) return fail(SWEPT_EINVAL, "null state");
   s->stream = (cudaStream_t)stream;
+  return 0;
+}
+
+int swept_set_phase_timing(swept_state* s, int on) {
+  if (!s) return fail(SWEPT_EINVAL, "null state");
+  s->timing = on != 0;
+  return 0;
+}
+
+int swept_phase_times(swept_state* s, double* ms, int64_t* launches) {
+  if (!s || !ms || !launches) return fail(SWEPT_EINVAL, "null argument");
+  if (int rc = set_device(s)) return rc;
+  CUDA_TRY(cudaStreamSynchronize(s->stream));
+  for (int k = 0; k < 5; ++k) { ms[k] = 0; launches[k] = 0; }
+  for (auto& t : s->timed) {
+    float f = 0;
+    if (cudaEventElapsedTime(&f, t.e0, t.e1) == cudaSuccess && t.kind >= 0 && t.kind < 5) {
+      ms[t.kind] += f;
+      launches[t.kind] += t.launches;
+    }
+    s->event_pool.push_back(t.e0);
+    s->event_pool.push_back(t.e1);
+  }
+  s->timed.clear();
+  cudaGetLastError();
   return 0;
 }
 
