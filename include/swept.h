@@ -43,6 +43,7 @@ enum { SWEPT_PER_STEP = 0, SWEPT_SWEPT = 1 };               /* variant          
 enum { SWEPT_F64 = 0, SWEPT_F32 = 1 };                      /* dtype                             */
 enum { SWEPT_RK2_MIDPOINT = 0, SWEPT_RK2_HEUN = 1 };        /* KS/Euler integrator (
                                                                Heun is BASELINE.json config 4)   */
+enum { SWEPT_NKINDS = 6 };                                   /* phase kinds reported by swept_phase_times */
 enum { SWEPT_OK = 0, SWEPT_EINVAL = -1, SWEPT_EUNSUPPORTED = -2, SWEPT_ECUDA = -3, SWEPT_ENOMEM = -4 };
 
 /* swept kernel flavours (how a tile is evaluated on chip; results are identical) */
@@ -50,8 +51,11 @@ enum {
   SWEPT_FLAVOR_AUTO = 0,  /* library picks (autotuned value if swept_autotune was run)                 */
   SWEPT_FLAVOR_TIER = 1,  /* one CTA per tile, two-row working array in shared memory, one block barrier
                              per tier (the paper's "Shared" arrangement, re-sized)        */
-  SWEPT_FLAVOR_CHAR = 2   /* register-resident sweep along characteristics: a lane group per tile,
+  SWEPT_FLAVOR_CHAR = 2,  /* register-resident sweep along characteristics: a lane group per tile,
                              halo exchange by warp shuffles only, no block barrier       */
+  SWEPT_FLAVOR_FLOW = 3   /* the CHAR sweep inside ONE persistent launch per Up..Down cycle: tiles are
+                             tasks, rows are chained by per-tile flags instead of kernel boundaries
+                             (DESIGN.md §5.5).  heat and KS, n = 256, 512, 1024   */
 };
 
 /* Optional device allocator hooks (so that PyTorch's caching allocator owns the memory).
@@ -135,9 +139,9 @@ int64_t swept_last_launches(const swept_state* s);
 int swept_set_phase_timing(swept_state* s, int on);
 
 /* swept_phase_times — synchronise the stream and return, per phase kind (index 0 Up, 1 SplitDiamond,
- * 2 WholeDiamond, 3 Down, 4 per-step remainder), the summed device time in milliseconds and the number of
- * kernel launches recorded since timing was switched on or since the previous call; then reset the record.
- * ms and launches are caller-owned HOST arrays of 5 entries. */
+ * 2 WholeDiamond, 3 Down, 4 per-step remainder, 5 whole FLOW cycle), the summed device time in milliseconds
+ * and the number of kernel launches recorded since timing was switched on or since the previous call; then
+ * reset the record.  ms and launches are caller-owned HOST arrays of SWEPT_NKINDS (6) entries. */
 int swept_phase_times(swept_state* s, double* ms, int64_t* launches);
 
 void swept_destroy(swept_state* s);

@@ -21,8 +21,8 @@ HEAT, KS, EULER = 0, 1, 2
 PER_STEP, SWEPT = 0, 1
 F64, F32 = 0, 1
 RK2_MIDPOINT, RK2_HEUN = 0, 1
-FLAVOR_AUTO, FLAVOR_TIER, FLAVOR_CHAR = 0, 1, 2
-KIND_NAMES = {0: "UpTriangle", 1: "SplitDiamond", 2: "WholeDiamond", 3: "DownTriangle", 4: "PerStepRemainder"}
+FLAVOR_AUTO, FLAVOR_TIER, FLAVOR_CHAR, FLAVOR_FLOW = 0, 1, 2, 3
+KIND_NAMES = {0: "UpTriangle", 1: "SplitDiamond", 2: "WholeDiamond", 3: "DownTriangle", 4: "PerStepRemainder", 5: "FlowCycle"}
 
 _ALLOC_FN = CFUNCTYPE(c_void_p, c_void_p, c_uint64)
 _FREE_FN = CFUNCTYPE(None, c_void_p, c_void_p)
@@ -178,9 +178,9 @@ def swept_set_phase_timing(state: int, on: bool) -> None:
 
 def swept_phase_times(state: int):
     """{kind name: (milliseconds, launches)} recorded since timing was switched on / the previous call."""
-    ms, cnt = (c_double * 5)(), (c_int64 * 5)()
+    ms, cnt = (c_double * 6)(), (c_int64 * 6)()
     _check(load().swept_phase_times(state, ms, cnt))
-    return {KIND_NAMES[k]: (float(ms[k]), int(cnt[k])) for k in range(5)}
+    return {KIND_NAMES[k]: (float(ms[k]), int(cnt[k])) for k in range(6)}
 
 
 def swept_set_stream(state: int, stream: int) -> None:

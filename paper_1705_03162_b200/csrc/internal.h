@@ -31,6 +31,19 @@ struct TileLaunch {
   cudaStream_t stream;
 };
 
+// FLOW flavour: one whole Up / diamonds / Down cycle of tile width n in a single persistent launch
+struct FlowLaunch {
+  const void* init;  // full time level at the start of the cycle
+  void* buf[2][2];   // [buffer][row]; row r of the cycle writes buffer r & 1
+  int64_t N;
+  int n, rows;       // tile width; rows = D + 2
+  int* flags;        // rows * N/n ints, zeroed by the caller (stream-ordered)
+  unsigned* ticket;  // zeroed by the caller
+  int warps;         // warps per CTA (0 = default)
+  const double* consts;
+  cudaStream_t stream;
+};
+
 // dtype: 0 f64, 1 f32.  rk2: 0 midpoint, 1 Heun.  Return cudaError_t as int, or -1000 if the
 // combination has no kernel.
 int launch_per_step_heat(int dtype, const PerStepLaunch& a);
@@ -40,6 +53,8 @@ int launch_tile_heat(int dtype, const TileLaunch& a);
 int launch_tile_ks(int dtype, int rk2, const TileLaunch& a);
 int launch_tile_euler(int dtype, int rk2, const TileLaunch& a);
 // does a kernel exist for (flavor, n, P)?  (host-only query used by the autotuner and argument checks)
+int launch_flow_heat(int dtype, const FlowLaunch& a);
+int launch_flow_ks(int dtype, int rk2, const FlowLaunch& a);
 bool tile_config_ok_heat(int dtype, int flavor, int64_t N, int n, int P);
 bool tile_config_ok_ks(int dtype, int flavor, int64_t N, int n, int P);
 bool tile_config_ok_euler(int dtype, int flavor, int64_t N, int n, int P);

@@ -1,9 +1,11 @@
 // kernels_impl.cuh — templated host launchers shared by kernels_{heat,ks,euler}.cu.
 #pragma once
+#include <cstdlib>
 #include "internal.h"
 #include "per_step.cuh"
 #include "swept_tier.cuh"
 #include "swept_char.cuh"
+#include "swept_flow.cuh"
 #include "../../include/swept.h"
 
 namespace swept {
@@ -150,6 +152,58 @@ int char_T(const TileLaunch& a) {
     case 8: return char_L<Prob, 8>(a);
     case 16: if (BMAX >= 16) return char_L<Prob, (BMAX >= 16 ? 16 : 8)>(a); break;
     case 32: if (BMAX >= 32) return char_L<Prob, (BMAX >= 32 ? 32 : 8)>(a); break;
+  }
+  return NO_KERNEL;
+}
+
+
+// ---- FLOW flavour: persistent launch, L = 32 lanes per tile, B = n / 32 lines per lane -----------------
+template <class Prob, int BMAX>
+inline bool flow_ok(int64_t N, int n) {
+  if (n % 32 || N % n) return false;
+  const int B = n / 32;
+  if (B != 8 && B != 16 && B != 32) return false;
+  return B <= BMAX && B % (2 * Prob::H) == 0 && n / (2 * Prob::H) >= 32;
+}
+
+template <class Prob, int B>
+inline int flow_go(const FlowLaunch& a) {
+  using R = typename Prob::R;
+  const int warps = (a.warps >= 1 && a.warps <= 4) ? a.warps : 4;
+  const int threads = warps * 32;
+  FlowArgs<R> f;
+  f.init = (const R*)a.init;
+  for (int i = 0; i < 2; ++i)
+    for (int j = 0; j < 2; ++j) f.buf[i][j] = (R*)a.buf[i][j];
+  f.N = a.N; f.K = (int)(a.N / a.n); f.rows = a.rows; f.flags = a.flags; f.ticket = a.ticket;
+  f.k = round_consts<R>(a.consts);
+  const size_t smem = flow_smem_bytes<Prob>(warps, a.n);
+  auto kern = swept_flow_kernel<Prob, B>;
+  cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  if (e != cudaSuccess) return (int)e;
+  // never launch more CTAs than can be co-resident: waiting tasks must not keep their parents off the machine
+  int dev = 0, sms = 0, occ = 0;
+  cudaGetDevice(&dev);
+  cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+  e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, threads, smem);
+  if (e != cudaSuccess) return (int)e;
+  if (occ < 1) return (int)cudaErrorLaunchOutOfResources;
+  if (const char* cap = getenv("SWEPT_FLOW_CTAS_PER_SM"))  // experiment knob: fewer resident (waiting) warps
+    if (atoi(cap) >= 1 && atoi(cap) < occ) occ = atoi(cap);
+  const int64_t ntasks = (int64_t)f.rows * f.K;
+  int64_t grid = (int64_t)occ * sms;
+  if (grid > (ntasks + warps - 1) / warps) grid = (ntasks + warps - 1) / warps;
+  kern<<<(unsigned)grid, threads, smem, a.stream>>>(f);
+  return (int)cudaGetLastError();
+}
+
+template <class Prob, int BMAX>
+int flow_T(const FlowLaunch& a) {
+  if (!flow_ok<Prob, BMAX>(a.N, a.n)) return NO_KERNEL;
+  switch (a.n / 32) {
+    case 8: return flow_go<Prob, 8>(a);
+    case 16: if (BMAX >= 16) return flow_go<Prob, (BMAX >= 16 ? 16 : 8)>(a); break;
+    case 32: if (BMAX >= 32) return flow_go<Prob, (BMAX >= 32 ? 32 : 8)>(a); break;
   }
   return NO_KERNEL;
 }

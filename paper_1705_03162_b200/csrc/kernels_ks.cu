@@ -9,6 +9,7 @@ bool tile_config_ok_ks(int dtype, int flavor, int64_t N, int n, int P) {
   if (dtype != 0) return false;
   if (flavor == SWEPT_FLAVOR_TIER) return tier_ok<KS<double, 0>>(n, P, 4);
   if (flavor == SWEPT_FLAVOR_CHAR) return char_ok<KS<double, 0>, 32>(N, n, P);
+  if (flavor == SWEPT_FLAVOR_FLOW) return flow_ok<KS<double, 0>, 32>(N, n);
   return false;
 }
 int launch_tile_ks(int dtype, int rk2, const TileLaunch& a) {
@@ -16,5 +17,9 @@ int launch_tile_ks(int dtype, int rk2, const TileLaunch& a) {
   if (a.flavor == SWEPT_FLAVOR_TIER) return rk2 == 0 ? tier_T<KS<double, 0>, 4>(a) : tier_T<KS<double, 1>, 4>(a);
   if (a.flavor == SWEPT_FLAVOR_CHAR) return rk2 == 0 ? char_T<KS<double, 0>, 32>(a) : char_T<KS<double, 1>, 32>(a);
   return NO_KERNEL;
+}
+int launch_flow_ks(int dtype, int rk2, const FlowLaunch& a) {
+  if (dtype != 0) return NO_KERNEL;
+  return rk2 == 0 ? flow_T<KS<double, 0>, 32>(a) : flow_T<KS<double, 1>, 32>(a);
 }
 }  // namespace swept

@@ -39,7 +39,7 @@ int fail(int code, const char* fmt, ...) {
                   cudaGetErrorString(e_));                                                  \
   } while (0)
 
-constexpr int KIND_UP = 0, KIND_SPLIT = 1, KIND_WHOLE = 2, KIND_DOWN = 3, KIND_REMAINDER = 4;
+constexpr int KIND_UP = 0, KIND_SPLIT = 1, KIND_WHOLE = 2, KIND_DOWN = 3, KIND_REMAINDER = 4, KIND_FLOW = 5;
 
 struct ProblemShape {
   int h, sigma, C;
@@ -78,6 +78,9 @@ struct swept_state {
   bool timing = false;
   std::vector<Timed> timed;
   std::vector<cudaEvent_t> event_pool;
+  // FLOW flavour scratch: ticket counter + one flag per tile of a cycle
+  int* flow_scratch = nullptr;
+  size_t flow_scratch_ints = 0;
   size_t elem() const { return dtype == SWEPT_F64 ? 8 : 4; }
 };
 
@@ -119,6 +122,35 @@ int launch_tile(swept_state* s, swept::TileLaunch& a) {
   return 0;
 }
 
+int launch_flow(swept_state* s, swept::FlowLaunch& a) {
+  a.N = s->N;
+  a.consts = s->consts;
+  a.stream = s->stream;
+  const size_t need = (size_t)a.rows * (size_t)(s->N / a.n) + 4;
+  if (need > s->flow_scratch_ints) {
+    if (s->flow_scratch) {
+      CUDA_TRY(cudaStreamSynchronize(s->stream));
+      CUDA_TRY(cudaFree(s->flow_scratch));
+      s->flow_scratch = nullptr;
+      s->flow_scratch_ints = 0;
+    }
+    CUDA_TRY(cudaMalloc((void**)&s->flow_scratch, need * sizeof(int)));
+    s->flow_scratch_ints = need;
+  }
+  CUDA_TRY(cudaMemsetAsync(s->flow_scratch, 0, need * sizeof(int), s->stream));
+  a.ticket = (unsigned*)s->flow_scratch;
+  a.flags = s->flow_scratch + 4;
+  int rc;
+  switch (s->problem) {
+    case SWEPT_HEAT: rc = swept::launch_flow_heat(s->dtype, a); break;
+    case SWEPT_KS: rc = swept::launch_flow_ks(s->dtype, s->rk2, a); break;
+    default: rc = NO_KERNEL; break;
+  }
+  if (rc == NO_KERNEL) return fail(SWEPT_EUNSUPPORTED, "no FLOW kernel for this problem / n=%d", a.n);
+  if (rc != 0) return fail(SWEPT_ECUDA, "flow launch: %s", cudaGetErrorString((cudaError_t)rc));
+  return 0;
+}
+
 cudaEvent_t take_event(swept_state* s) {
   cudaEvent_t e = nullptr;
   if (!s->event_pool.empty()) {
@@ -149,6 +181,7 @@ struct TimedScope {
 
 bool tile_ok(const swept_state* s, int flavor, int n, int P) {
   if (n <= 0 || s->N % n != 0) return false;
+  if (flavor == SWEPT_FLAVOR_FLOW && (s->problem == SWEPT_EULER || P < 0 || P > 4)) return false;
   switch (s->problem) {
     case SWEPT_HEAT: return swept::tile_config_ok_heat(s->dtype, flavor, s->N, n, P);
     case SWEPT_KS: return swept::tile_config_ok_ks(s->dtype, flavor, s->N, n, P);
@@ -284,6 +317,9 @@ void default_tile(const swept_state* s, int* n_io, int* flavor_io, int* P_io) {
         for (int L : {32, 16, 8})
           if (n == 0 && (P == 0 || P == L) && tile_ok(s, SWEPT_FLAVOR_CHAR, cand, L)) n = cand;
     }
+    if (n == 0 && flavor == SWEPT_FLAVOR_FLOW)
+      for (int cand : {512, 1024, 256})
+        if (n == 0 && tile_ok(s, SWEPT_FLAVOR_FLOW, cand, 0)) n = cand;
     if (n == 0 && flavor != SWEPT_FLAVOR_CHAR)
       for (int cand : {512, 256, 128, 1024, 64, 32, 2048, 4096})
         if (n == 0 && s->N % cand == 0) n = cand;
@@ -300,7 +336,7 @@ void default_tile(const swept_state* s, int* n_io, int* flavor_io, int* P_io) {
   }
   if (P == 0) {
     if (flavor == SWEPT_FLAVOR_TIER) P = tier_default_P(s, n);
-    else
+    else if (flavor == SWEPT_FLAVOR_CHAR)
       for (int L : {32, 16, 8})
         if (P == 0 && tile_ok(s, SWEPT_FLAVOR_CHAR, n, L)) P = L;
   }
@@ -315,6 +351,19 @@ bool level_config(const swept_state* s, int n_top, int flavor_top, int P_top, in
     *flavor = flavor_top;
     *P = P_top;
     return tile_ok(s, flavor_top, n, P_top);
+  }
+  if (flavor_top == SWEPT_FLAVOR_FLOW) {
+    if (tile_ok(s, SWEPT_FLAVOR_FLOW, n, P_top)) {
+      *flavor = SWEPT_FLAVOR_FLOW;
+      *P = P_top;
+      return true;
+    }
+    for (int L : {32, 16, 8})
+      if (tile_ok(s, SWEPT_FLAVOR_CHAR, n, L)) {
+        *flavor = SWEPT_FLAVOR_CHAR;
+        *P = L;
+        return true;
+      }
   }
   if (flavor_top == SWEPT_FLAVOR_CHAR) {
     const int B_top = n_top / P_top;
@@ -357,7 +406,30 @@ int run_swept(swept_state* s, int64_t nsteps, int n, int flavor, int P) {
   const int64_t np = make_plan(nsteps * sh.sigma, widths, sh.h, &plan);
   if (np < 0) return fail(SWEPT_EINVAL, "cannot plan tile_width=%d", n);
   int r0 = -1, r1 = -1;  // slabs holding the current two-row state
-  for (const swept_phase& ph : plan) {
+  for (size_t ip = 0; ip < plan.size(); ++ip) {
+    const swept_phase& ph = plan[ip];
+    if (ph.kind == KIND_UP && cfg[ph.n].first == SWEPT_FLAVOR_FLOW) {
+      // the whole cycle Up .. Down of this width in one persistent launch
+      size_t jp = ip;
+      while (plan[jp].kind != KIND_DOWN) ++jp;
+      swept::FlowLaunch f{};
+      f.n = ph.n;
+      f.rows = (int)(jp - ip + 1);
+      f.warps = cfg[ph.n].second;
+      f.init = s->slab[s->cur];
+      // buffer 0 = the two slabs after cur, buffer 1 = the third one and cur itself (swept_flow.cuh: hazards)
+      const int a0 = (s->cur + 1) & 3, a1 = (s->cur + 2) & 3, b0 = (s->cur + 3) & 3, b1 = s->cur;
+      f.buf[0][0] = s->slab[a0]; f.buf[0][1] = s->slab[a1];
+      f.buf[1][0] = s->slab[b0]; f.buf[1][1] = s->slab[b1];
+      {
+        TimedScope ts(s, KIND_FLOW, 1);
+        if (int rc = launch_flow(s, f)) return rc;
+      }
+      s->last_launches += 1;
+      s->cur = ((f.rows - 1) & 1) ? b0 : a0;  // the Down row wrote row 0 of its buffer
+      ip = jp;
+      continue;
+    }
     if (ph.kind == KIND_REMAINDER) {
       TimedScope ts(s, KIND_REMAINDER, ph.ntiers);
       if (int rc = run_per_step(s, ph.ntiers / sh.sigma, 0)) return rc;
@@ -494,6 +566,7 @@ void swept_destroy(swept_state* s) {
   if (s->capture_stream) cudaStreamDestroy(s->capture_stream);
   for (auto& t : s->timed) { cudaEventDestroy(t.e0); cudaEventDestroy(t.e1); }
   for (cudaEvent_t e : s->event_pool) cudaEventDestroy(e);
+  if (s->flow_scratch) cudaFree(s->flow_scratch);
   for (int i = 0; i < 4; ++i) {
     if (!s->slab[i]) continue;
     if (s->free_) s->free_(s->alloc_ctx, s->slab[i]);
@@ -518,10 +591,10 @@ int swept_phase_times(swept_state* s, double* ms, int64_t* launches) {
   if (!s || !ms || !launches) return fail(SWEPT_EINVAL, "null argument");
   if (int rc = set_device(s)) return rc;
   CUDA_TRY(cudaStreamSynchronize(s->stream));
-  for (int k = 0; k < 5; ++k) { ms[k] = 0; launches[k] = 0; }
+  for (int k = 0; k < SWEPT_NKINDS; ++k) { ms[k] = 0; launches[k] = 0; }
   for (auto& t : s->timed) {
     float f = 0;
-    if (cudaEventElapsedTime(&f, t.e0, t.e1) == cudaSuccess && t.kind >= 0 && t.kind < 5) {
+    if (cudaEventElapsedTime(&f, t.e0, t.e1) == cudaSuccess && t.kind >= 0 && t.kind < SWEPT_NKINDS) {
       ms[t.kind] += f;
       launches[t.kind] += t.launches;
     }
@@ -573,7 +646,7 @@ int swept_run_flavor(swept_state* s, int64_t nsteps, int32_t tile_width, int var
     rc = run_per_step(s, nsteps, tw);
   } else if (variant == SWEPT_SWEPT) {
     int fl = flavor & 0xff, P = (flavor >> 8) & 0xff;  // bits 8..15: explicit P / lane-group size (0 = default)
-    if (fl != SWEPT_FLAVOR_AUTO && fl != SWEPT_FLAVOR_TIER && fl != SWEPT_FLAVOR_CHAR)
+    if (fl != SWEPT_FLAVOR_AUTO && fl != SWEPT_FLAVOR_TIER && fl != SWEPT_FLAVOR_CHAR && fl != SWEPT_FLAVOR_FLOW)
       return fail(SWEPT_EINVAL, "unknown flavor %d", fl);
     rc = run_swept(s, nsteps, tile_width, fl, P);
   } else {
@@ -632,6 +705,8 @@ int swept_autotune(swept_state* s, int variant, int32_t* best_tile_width) {
       for (int fl : {SWEPT_FLAVOR_TIER, SWEPT_FLAVOR_CHAR})
         for (int P : {1, 2, 4, 8, 16, 32})
           if (tile_ok(s, fl, n, P)) cands.push_back({n, fl, P});
+    for (int n : {256, 512, 1024})
+      if (tile_ok(s, SWEPT_FLAVOR_FLOW, n, 0)) cands.push_back({n, SWEPT_FLAVOR_FLOW, 0});
   }
   int rc_final = 0;
   for (const Cand& c : cands) {

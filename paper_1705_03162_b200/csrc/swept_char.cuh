@@ -105,15 +105,91 @@ __device__ __forceinline__ void char_step(typename Prob::R (&v)[Prob::C][B],
   inc = 2 * H - inc;
 }
 
+// The sweep of ONE tile by its group of L lanes (all of one warp): initial line values from the staged rows,
+// m + L - 1 skewed super-steps, final line values back to the staged rows (in place).
+//   rows : staged two-row state, component c of row r at rows[(r*C + c)*RS + slot]
+//   ctr  : slot of x' = 0 (the tile centre);  gl : lane within the group
+template <class Prob, int B, int L, int KIND>
+__device__ __forceinline__ void char_sweep_tile(typename Prob::R* rows, const int RS, const int ctr, const int gl,
+                                                const Consts<typename Prob::R>& kc) {
+  using R = typename Prob::R;
+  constexpr int H = Prob::H, C = Prob::C;
+  constexpr int n = B * L;          // tile width
+  constexpr int m = n / (2 * H);    // super-columns per tile = tiers per half diamond
+  static_assert(B % (2 * H) == 0, "lines per lane must be a multiple of 2h");
+  static_assert(L % 2 == 0 && m % 2 == 0 && m >= L, "step pairing needs even L, even m >= L");
+  auto slot = [&](int row, int c, int xp) -> R& { return rows[(row * C + c) * RS + ctr + xp]; };
+
+  R v[C][B], halA[C][2 * H], halB[C][2 * H];
+  // initial line values: the point of line q just below the square (super-column -1), which is the latest
+  // (or second latest) tier stored at x' = -(h tq + r + 1); Up: the anti-diagonal = tier-0 data
+#pragma unroll
+  for (int i = 0; i < B; ++i) {
+    const int q = gl * B + i;
+    int xp, row;
+    if (KIND == KIND_UP) {
+      xp = n / 2 - 1 - q;
+      row = 0;
+    } else {
+      const int tq = q / (2 * H), r = i % (2 * H);
+      xp = -(H * tq + r + 1);
+      row = tq & 1;
+    }
+#pragma unroll
+    for (int c = 0; c < C; ++c) v[c][i] = slot(row, c, xp);
+  }
+#pragma unroll
+  for (int c = 0; c < C; ++c)
+#pragma unroll
+    for (int e = 0; e < 2 * H; ++e) halA[c][e] = halB[c][e] = (R)0;
+  __syncwarp();
+
+  // Loop I/O goes through one per-thread pointer: element (row sc&1, x' = base + h sc) with
+  //   reader (group lane 0)    base = 0      : line -1-e at super-column sc is (x' = h sc + e,        tier sc)
+  //   writer (group lane L-1)  base = -n/2   : its top line e leaves at       (x' = -n/2 + h sc + e, tier m+sc)
+  // advanced by h and toggled between the two rows every step (inc alternates h + C RS, h - C RS).
+  const int sc0 = -gl;
+  R* io = rows + ((sc0 & 1) * C) * RS + ctr + (gl == 0 ? 0 : -n / 2) + H * sc0;
+  int inc = H + ((sc0 & 1) ? -C * RS : C * RS);
+
+  int s = 0;
+  for (; s < L; s += 2) {  // ramp up: lane gl starts at step gl
+    char_step<Prob, B, L, KIND, true>(v, halA, halB, io, inc, s, gl, RS, kc);
+    char_step<Prob, B, L, KIND, true>(v, halB, halA, io, inc, s + 1, gl, RS, kc);
+  }
+  for (; s < m; s += 2) {  // steady state: every lane is inside its m super-columns
+    char_step<Prob, B, L, KIND, false>(v, halA, halB, io, inc, s, gl, RS, kc);
+    char_step<Prob, B, L, KIND, false>(v, halB, halA, io, inc, s + 1, gl, RS, kc);
+  }
+  for (; s < m + L; s += 2) {  // ramp down (the last step, s = m+L-1, is empty and keeps the pairing)
+    char_step<Prob, B, L, KIND, true>(v, halA, halB, io, inc, s, gl, RS, kc);
+    char_step<Prob, B, L, KIND, true>(v, halB, halA, io, inc, s + 1, gl, RS, kc);
+  }
+  __syncwarp();
+  // upper-right edge (Down: the full time level): last value of every line
+#pragma unroll
+  for (int i = 0; i < B; ++i) {
+    const int q = gl * B + i;
+    int xp, row;
+    if (KIND == KIND_DOWN) {
+      xp = n / 2 - 1 - q;
+      row = 0;
+    } else {
+      const int tq = q / (2 * H), r = i % (2 * H);
+      xp = n / 2 - 1 - H * tq - r;
+      row = tq & 1;
+    }
+#pragma unroll
+    for (int c = 0; c < C; ++c) slot(row, c, xp) = v[c][i];
+  }
+
+}
+
 template <class Prob, int B, int L, int KIND>
 __global__ void __launch_bounds__(128) swept_char_kernel(const TierArgs<typename Prob::R> a) {
   using R = typename Prob::R;
   constexpr int H = Prob::H, C = Prob::C, PAD = Pad16<R>::value;
   constexpr int n = B * L;          // tile width
-  constexpr int m = n / (2 * H);    // super-columns per tile = tiers per half diamond
-  constexpr int BP = B / (2 * H);   // points per lane per sub-column (chain length)
-  static_assert(B % (2 * H) == 0, "lines per lane must be a multiple of 2h");
-  static_assert(L % 2 == 0 && m % 2 == 0 && m >= L, "step pairing needs even L, even m >= L");
   extern __shared__ __align__(128) unsigned char smem_raw[];
   const int T = blockDim.x;
   const int chunk = T * B;  // points staged by this CTA (T/L adjacent tiles)
@@ -161,72 +237,7 @@ __global__ void __launch_bounds__(128) swept_char_kernel(const TierArgs<typename
   mbar_wait(mbar, 0);
   __syncthreads();
 
-  const int gl = tid % L;                       // lane within the tile's group
-  const int ctr = PAD + (tid / L) * n + n / 2;  // smem slot of x' = 0 of this thread's tile
-  auto slot = [&](int row, int c, int xp) -> R& { return rows[(row * C + c) * RS + ctr + xp]; };
-
-  R v[C][B], halA[C][2 * H], halB[C][2 * H];
-  // initial line values: the point of line q just below the square (super-column -1), which is the latest
-  // (or second latest) tier stored at x' = -(h tq + r + 1); Up: the anti-diagonal = tier-0 data
-#pragma unroll
-  for (int i = 0; i < B; ++i) {
-    const int q = gl * B + i;
-    int xp, row;
-    if (KIND == KIND_UP) {
-      xp = n / 2 - 1 - q;
-      row = 0;
-    } else {
-      const int tq = q / (2 * H), r = i % (2 * H);
-      xp = -(H * tq + r + 1);
-      row = tq & 1;
-    }
-#pragma unroll
-    for (int c = 0; c < C; ++c) v[c][i] = slot(row, c, xp);
-  }
-#pragma unroll
-  for (int c = 0; c < C; ++c)
-#pragma unroll
-    for (int e = 0; e < 2 * H; ++e) halA[c][e] = halB[c][e] = (R)0;
-  __syncwarp();
-
-  // Loop I/O goes through one per-thread pointer: element (row sc&1, x' = base + h sc) with
-  //   reader (group lane 0)    base = 0      : line -1-e at super-column sc is (x' = h sc + e,        tier sc)
-  //   writer (group lane L-1)  base = -n/2   : its top line e leaves at       (x' = -n/2 + h sc + e, tier m+sc)
-  // advanced by h and toggled between the two rows every step (inc alternates h + C RS, h - C RS).
-  const int sc0 = -gl;
-  R* io = rows + ((sc0 & 1) * C) * RS + ctr + (gl == 0 ? 0 : -n / 2) + H * sc0;
-  int inc = H + ((sc0 & 1) ? -C * RS : C * RS);
-
-  int s = 0;
-  for (; s < L; s += 2) {  // ramp up: lane gl starts at step gl
-    char_step<Prob, B, L, KIND, true>(v, halA, halB, io, inc, s, gl, RS, a.k);
-    char_step<Prob, B, L, KIND, true>(v, halB, halA, io, inc, s + 1, gl, RS, a.k);
-  }
-  for (; s < m; s += 2) {  // steady state: every lane is inside its m super-columns
-    char_step<Prob, B, L, KIND, false>(v, halA, halB, io, inc, s, gl, RS, a.k);
-    char_step<Prob, B, L, KIND, false>(v, halB, halA, io, inc, s + 1, gl, RS, a.k);
-  }
-  for (; s < m + L; s += 2) {  // ramp down (the last step, s = m+L-1, is empty and keeps the pairing)
-    char_step<Prob, B, L, KIND, true>(v, halA, halB, io, inc, s, gl, RS, a.k);
-    char_step<Prob, B, L, KIND, true>(v, halB, halA, io, inc, s + 1, gl, RS, a.k);
-  }
-  __syncwarp();
-  // upper-right edge (Down: the full time level): last value of every line
-#pragma unroll
-  for (int i = 0; i < B; ++i) {
-    const int q = gl * B + i;
-    int xp, row;
-    if (KIND == KIND_DOWN) {
-      xp = n / 2 - 1 - q;
-      row = 0;
-    } else {
-      const int tq = q / (2 * H), r = i % (2 * H);
-      xp = n / 2 - 1 - H * tq - r;
-      row = tq & 1;
-    }
-#pragma unroll
-    for (int c = 0; c < C; ++c) slot(row, c, xp) = v[c][i];
-  }
+  char_sweep_tile<Prob, B, L, KIND>(rows, RS, PAD + (tid / L) * n + n / 2, tid % L, a.k);
 
   fence_proxy_async_smem();
   __syncthreads();

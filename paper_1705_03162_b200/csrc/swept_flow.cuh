@@ -1,0 +1,171 @@
+// swept_flow.cuh — swept kernels, flavour FLOW: one whole swept cycle (UpTriangle, D Split/WholeDiamond rows,
+// DownTriangle; §4.2-4.3) in ONE persistent launch, the rows chained by per-tile dependencies.
+//
+// The paper synchronises the rows of tiles by returning to the host between launches ("kernel calls are
+// implicitly synchronized by returning control to the queue") and names a cheaper device-side
+// synchronisation as future work.  What a tile of row r really needs is only the two tiles of
+// row r-1 it overlaps (the edges it receives), not the whole row.  So here every tile of the
+// cycle is a task (row-major ticket order, one atomic ticket counter); a WARP takes a ticket, waits until the
+// two parent tiles have published their edges (one flag per tile, release/acquire at GPU scope), stages the
+// tile's two rows from global memory into its private shared-memory slice, sweeps the tile exactly as the
+// CHAR flavour does (swept_char.cuh: registers + shuffles, L = 32 lanes, B = n/32 lines per lane), writes the
+// rows back and raises its flag.  This removes the launch gaps, the load / compute / store serialisation of a
+// whole row, and the load imbalance of 2^k equal tiles on 148 SMs (a fast SM simply takes the next ticket).
+//
+// Global state: the same two-row layout as the other flavours.  Row r of the cycle
+// reads buffer (r-1)&1 and writes buffer r&1 (two rows each; the Up row reads the initial time level `init`,
+// the Down row writes only row 0 = the full time level).  Tiling of row r is shifted by n/2 when r is odd
+// (Up = row 0 aligned; the paper's half-tile shift).
+//
+// Hazards.  RAW: tile (r,k) reads [S-h, S+n+h) of buffer (r-1)&1, which lies inside the ranges of the two tiles
+// of row r-1 that overlap [S, S+n) — its parents — and both have published (flag) before it loads.  WAR: tile
+// (r,k) overwrites [S, S+n) of buffer r&1, last written by row r-2 and read by row r-1; the only tiles of row r-1
+// whose reads (range plus h-wide halo) touch [S, S+n) are again the two parents, which finished reading before
+// they published.  The Up row's input `init` may be one of the slabs of buffer 1: row 1 overwrites a range of it
+// only after both Up tiles that read that range have published.  Deadlock freedom: tickets are taken in
+// row-major order and a task only waits for tasks with smaller tickets, which are held by warps that are
+// already running — the launch never exceeds the number of co-resident CTAs (host side: occupancy query).
+#pragma once
+#include "common.cuh"
+#include "functors.cuh"
+#include "swept_char.cuh"
+
+namespace swept {
+
+template <class R>
+struct FlowArgs {
+  const R* init;  // full time level at the start of the cycle (C components, stride N)
+  R* buf[2][2];   // [buffer][row]
+  int64_t N;
+  int K;          // tiles per row = N / n
+  int rows;       // D + 2
+  int* flags;     // rows * K, zero on entry; flags[r * K + k] = 1 once tile (r, k) is in global memory
+  unsigned* ticket;  // zero on entry
+  Consts<R> k;
+};
+
+__device__ __forceinline__ int ld_acquire_gpu(const int* p) {
+  int v;
+  asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+  return v;
+}
+// polling load: relaxed at GPU scope (no L1 invalidation per poll); the acquire fence follows once the flag is seen
+__device__ __forceinline__ int ld_relaxed_gpu(const int* p) {
+  int v;
+  asm volatile("ld.relaxed.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+  return v;
+}
+__device__ __forceinline__ void fence_acq_rel_gpu() { asm volatile("fence.acq_rel.gpu;" ::: "memory"); }
+__device__ __forceinline__ void st_release_gpu(int* p, int v) {
+  asm volatile("st.release.gpu.global.s32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
+}
+
+// 16-byte copies global <-> shared of `count` elements starting at global element g0 (periodic in N; g0 and the
+// wrap point are multiples of the vector width), by the 32 lanes of a warp.  Loads bypass L1 (ld.global.cg):
+// the data was written by other SMs during this launch.
+template <class R>
+__device__ __forceinline__ void warp_load_row(R* dst, const R* __restrict__ src, int64_t g0, int count, int64_t N,
+                                              int lane) {
+  constexpr int V = 16 / (int)sizeof(R);
+  for (int i = lane * V; i < count; i += 32 * V) {
+    int64_t g = g0 + i;
+    if (g >= N) g -= N;
+    const int4 t = __ldcg(reinterpret_cast<const int4*>(src + g));
+    *reinterpret_cast<int4*>(dst + i) = t;
+  }
+}
+template <class R>
+__device__ __forceinline__ void warp_store_row(R* __restrict__ dst, const R* src, int64_t g0, int count, int64_t N,
+                                               int lane) {
+  constexpr int V = 16 / (int)sizeof(R);
+  for (int i = lane * V; i < count; i += 32 * V) {
+    int64_t g = g0 + i;
+    if (g >= N) g -= N;
+    *reinterpret_cast<int4*>(dst + g) = *reinterpret_cast<const int4*>(src + i);
+  }
+}
+
+template <class Prob, int B>
+__global__ void __launch_bounds__(128) swept_flow_kernel(const FlowArgs<typename Prob::R> a) {
+  using R = typename Prob::R;
+  constexpr int H = Prob::H, C = Prob::C, PAD = Pad16<R>::value, L = 32;
+  constexpr int n = B * L;
+  constexpr int RS = n + 2 * PAD;
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  R* rows = reinterpret_cast<R*>(smem_raw) + (size_t)warp * 2 * C * RS;
+  const int64_t N = a.N;
+  const unsigned ntasks = (unsigned)a.rows * (unsigned)a.K;
+
+  for (;;) {
+    unsigned t = 0;
+    if (lane == 0) t = atomicAdd(a.ticket, 1u);
+    t = __shfl_sync(0xffffffffu, t, 0);
+    if (t >= ntasks) break;
+    const int r = (int)(t / (unsigned)a.K), k = (int)(t % (unsigned)a.K);
+    const int64_t S = (int64_t)k * n + ((r & 1) ? n / 2 : 0);  // < N + n/2; copies wrap
+    if (r > 0) {
+      // parents: the tiles of row r-1 overlapping [S, S+n)
+      const int p0 = (r & 1) ? k : (k == 0 ? a.K - 1 : k - 1);
+      const int p1 = (r & 1) ? (k + 1 == a.K ? 0 : k + 1) : k;
+      const int* f = a.flags + (size_t)(r - 1) * a.K;
+      unsigned ns = 64;
+      while (ld_relaxed_gpu(f + p0) == 0 || ld_relaxed_gpu(f + p1) == 0) {
+        __nanosleep(ns);
+        if (ns < 2048) ns *= 2;
+      }
+      fence_acq_rel_gpu();
+    }
+    // ---- stage the tile: both rows over [S-h, S+n+h) (Up: row 0 of the initial level, no halo)
+    if (r == 0) {
+#pragma unroll
+      for (int c = 0; c < C; ++c) warp_load_row<R>(rows + c * RS + PAD, a.init + (int64_t)c * N, S, n, N, lane);
+      for (int i = lane; i < C * RS; i += 32) rows[C * RS + i] = (R)0;  // tier -1 does not exist
+    } else {
+      const R* in0 = (r & 1) ? a.buf[0][0] : a.buf[1][0];
+      const R* in1 = (r & 1) ? a.buf[0][1] : a.buf[1][1];
+#pragma unroll
+      for (int c = 0; c < C; ++c) {
+        warp_load_row<R>(rows + c * RS + PAD, in0 + (int64_t)c * N, S, n, N, lane);
+        warp_load_row<R>(rows + (C + c) * RS + PAD, in1 + (int64_t)c * N, S, n, N, lane);
+      }
+      if (lane < 2 * C * 2 * H) {
+        const int rr = lane / (C * 2 * H), c = (lane / (2 * H)) % C, j = lane % (2 * H);
+        int64_t g = (j < H) ? (S - H + j) : (S + n + (j - H));  // S < N, so one wrap suffices
+        if (g < 0) g += N;
+        if (g >= N) g -= N;
+        const int s = (j < H) ? (PAD - H + j) : (PAD + n + (j - H));
+        rows[(rr * C + c) * RS + s] = __ldcg((rr ? in1 : in0) + (int64_t)c * N + g);
+      }
+    }
+    __syncwarp();
+    // ---- sweep (identical arithmetic and order to the CHAR flavour)
+    if (r == 0) char_sweep_tile<Prob, B, L, KIND_UP>(rows, RS, PAD + n / 2, lane, a.k);
+    else if (r == a.rows - 1) char_sweep_tile<Prob, B, L, KIND_DOWN>(rows, RS, PAD + n / 2, lane, a.k);
+    else char_sweep_tile<Prob, B, L, KIND_WHOLE>(rows, RS, PAD + n / 2, lane, a.k);
+    __syncwarp();
+    // ---- publish
+    R* out0 = (r & 1) ? a.buf[1][0] : a.buf[0][0];
+    R* out1 = (r & 1) ? a.buf[1][1] : a.buf[0][1];
+#pragma unroll
+    for (int c = 0; c < C; ++c) {
+      warp_store_row<R>(out0 + (int64_t)c * N, rows + c * RS + PAD, S, n, N, lane);
+      if (r != a.rows - 1)  // Down leaves only row 0: the full time level
+        warp_store_row<R>(out1 + (int64_t)c * N, rows + (C + c) * RS + PAD, S, n, N, lane);
+    }
+    __syncwarp();
+    if (lane == 0) {
+      __threadfence();
+      st_release_gpu(a.flags + t, 1);
+    }
+    __syncwarp();  // the slice is reused by the next task of this warp
+  }
+}
+
+template <class Prob>
+inline size_t flow_smem_bytes(int warps, int n) {
+  using R = typename Prob::R;
+  return (size_t)warps * 2 * Prob::C * ((size_t)n + 2 * Pad16<R>::value) * sizeof(R);
+}
+
+}  // namespace swept

@@ -36,10 +36,11 @@ def gpu_run(w, nsteps, variant, tile_width=0, flavor=sw.FLAVOR_AUTO, group=0, dt
 
 
 CHAR = tuple((sw.FLAVOR_CHAR, L) for L in (8, 16, 32))
+FLOW = ((sw.FLAVOR_FLOW, 0),)   # heat / KS, n in {256, 512, 1024}; "not admissible" elsewhere
 TIER12 = ((sw.FLAVOR_TIER, 1), (sw.FLAVOR_TIER, 2))
 
 
-def check(w, nsteps, tile_widths, dtype=np.float64, flavors=((sw.FLAVOR_TIER, 0),) + CHAR, exact=True):
+def check(w, nsteps, tile_widths, dtype=np.float64, flavors=((sw.FLAVOR_TIER, 0),) + CHAR + FLOW, exact=True):
     C = w.components
     ref = oracle.run_workload(w, nsteps=nsteps, dtype=dtype)
     ps, _ = gpu_run(w, nsteps, sw.PER_STEP, dtype=dtype)
@@ -54,7 +55,7 @@ def check(w, nsteps, tile_widths, dtype=np.float64, flavors=((sw.FLAVOR_TIER, 0)
             try:
                 sx, _ = gpu_run(w, nsteps, sw.SWEPT, n, fl, grp, dtype=dtype)
             except sw.SweptError as e:
-                if "not admissible" in str(e):  # e.g. CHAR needs n/L in {8,16,32} and 32*B | N
+                if "not admissible" in str(e) or "no FLOW kernel" in str(e):  # e.g. CHAR needs n/L in {8,16,32}
                     continue
                 raise
             ran += 1
@@ -69,7 +70,7 @@ def check(w, nsteps, tile_widths, dtype=np.float64, flavors=((sw.FLAVOR_TIER, 0)
 def test_heat_small(N, nsteps):
     w = si.heat_sines(N, 8, 11, nsteps)
     widths = [n for n in (32, 64, 128, 256) if N % n == 0]
-    check(w, nsteps, widths, flavors=TIER12 + CHAR)
+    check(w, nsteps, widths, flavors=TIER12 + CHAR + FLOW)
 
 
 @pytest.mark.parametrize("rk2", [si.RK2_MIDPOINT, si.RK2_HEUN])
@@ -77,14 +78,14 @@ def test_heat_small(N, nsteps):
 def test_ks_small(N, nsteps, rk2):
     w = si.ks_cos(N, 5, nsteps)
     w.rk2 = rk2
-    check(w, nsteps, [32, 64, 128, 256], flavors=TIER12 + ((sw.FLAVOR_TIER, 4),) + CHAR)
+    check(w, nsteps, [32, 64, 128, 256], flavors=TIER12 + ((sw.FLAVOR_TIER, 4),) + CHAR + FLOW)
 
 
 @pytest.mark.parametrize("rk2", [si.RK2_MIDPOINT, si.RK2_HEUN])
 @pytest.mark.parametrize("N,nsteps", [(256, 3), (512, 150)])
 def test_euler_small(N, nsteps, rk2):
     w = si.euler_double_sod(N, nsteps, rk2=rk2)
-    check(w, nsteps, [32, 64, 128, 256], flavors=TIER12 + CHAR)
+    check(w, nsteps, [32, 64, 128, 256], flavors=TIER12 + CHAR + FLOW)
 
 
 def test_euler_random_data():
@@ -103,7 +104,7 @@ def test_single_tile_wraps_onto_itself():
 
 def test_heat_fp32():
     w = si.heat_sines(1024, 16, 21, 500)
-    check(w, 500, [32, 128, 256, 1024], dtype=np.float32, flavors=((sw.FLAVOR_TIER, 1), (sw.FLAVOR_TIER, 4)) + CHAR)
+    check(w, 500, [32, 128, 256, 1024], dtype=np.float32, flavors=((sw.FLAVOR_TIER, 1), (sw.FLAVOR_TIER, 4)) + CHAR + FLOW)
 
 
 def test_wide_tiles():
@@ -111,6 +112,25 @@ def test_wide_tiles():
     check(w, 3000, [2048, 4096], flavors=((sw.FLAVOR_TIER, 4),))
     w = si.ks_cos(8192, 5, 700)
     check(w, 700, [2048, 4096], flavors=((sw.FLAVOR_TIER, 4),))
+
+
+@pytest.mark.parametrize("warps", [1, 2, 4])
+def test_flow_flavour_many_cycles_and_small_grids(warps):
+    # FLOW: one persistent launch per Up..Down cycle, rows chained by per-tile flags.  K = N/n = 1, 2 and
+    # many tiles per row; D = 0 (Up + Down only), odd and even D; remainder levels; both RK2 flavours
+    for w, widths in ((si.heat_sines(1024, 8, 3, 1500), (256, 512, 1024)),
+                      (si.heat_sines(1 << 15, 8, 4, 700), (256, 512, 1024)),
+                      (si.ks_cos(2048, 6, 333), (256, 512, 1024)),
+                      (si.ks_cos(1 << 14, 7, 200), (256, 512))):
+        ref = oracle.run_workload(w)
+        for n in widths:
+            got, launches = gpu_run(w, w.nsteps, sw.SWEPT, n, sw.FLAVOR_FLOW, warps)
+            assert np.array_equal(got, ref), (w.name, n, warps)
+    w = si.heat_sines(4096, 8, 2, 0)
+    s = sw.Swept.from_workload(w)
+    s.run(128 * 5, 256, sw.SWEPT, sw.FLAVOR_FLOW)     # exactly 5 rows of m = 128: one launch
+    assert s.last_launches == 1
+    s.close()
 
 
 def test_per_step_non_power_of_two_N():
@@ -159,14 +179,14 @@ def test_error_codes():
 # ---------------------------------------------------------------- the five configs
 def test_config1_full():
     w = si.config(1)  # heat FP64 N=2048, 20000 steps
-    check(w, w.nsteps, [32, 64, 128, 256, 512, 1024], flavors=TIER12 + CHAR)
+    check(w, w.nsteps, [32, 64, 128, 256, 512, 1024], flavors=TIER12 + CHAR + FLOW)
 
 
 @pytest.mark.parametrize("dtype", [np.float64, np.float32])
 def test_config2_full_length(dtype):
     for N in (1 << 11, 1 << 16):  # full 10000 steps against the oracle
         w = si.config(2, N=N)
-        check(w, w.nsteps, [32, 256, 1024], dtype=dtype, flavors=((sw.FLAVOR_TIER, 2),) + CHAR)
+        check(w, w.nsteps, [32, 256, 1024], dtype=dtype, flavors=((sw.FLAVOR_TIER, 2),) + CHAR + FLOW)
 
 
 @pytest.mark.parametrize("dtype", [np.float64, np.float32])
@@ -174,7 +194,7 @@ def test_config2_large_N(dtype):
     # oracle over a reduced step count covering > 2 swept cycles + remainder; full run swept == per_step
     for N in (1 << 20, 1 << 22):
         w = si.config(2, N=N)
-        check(w, 1100, [256, 1024], dtype=dtype, flavors=((sw.FLAVOR_TIER, 2),) + CHAR)
+        check(w, 1100, [256, 1024], dtype=dtype, flavors=((sw.FLAVOR_TIER, 2),) + CHAR + FLOW)
     w = si.config(2, N=1 << 20)
     ps, _ = gpu_run(w, w.nsteps, sw.PER_STEP, dtype=dtype)
     sx, _ = gpu_run(w, w.nsteps, sw.SWEPT, 256, dtype=dtype)
@@ -183,9 +203,9 @@ def test_config2_large_N(dtype):
 
 def test_config3_ks():
     w = si.config(3, N=1 << 14)  # full 20000 steps
-    check(w, w.nsteps, [64, 256, 1024], flavors=((sw.FLAVOR_TIER, 2),) + CHAR)
+    check(w, w.nsteps, [64, 256, 1024], flavors=((sw.FLAVOR_TIER, 2),) + CHAR + FLOW)
     w = si.config(3, N=1 << 20)
-    check(w, 300, [256], flavors=((sw.FLAVOR_TIER, 2),) + CHAR)
+    check(w, 300, [256], flavors=((sw.FLAVOR_TIER, 2),) + CHAR + FLOW)
     ps, _ = gpu_run(w, 4000, sw.PER_STEP)
     sx, _ = gpu_run(w, 4000, sw.SWEPT, 512)
     assert np.array_equal(ps, sx) and np.all(np.isfinite(ps)) and np.max(np.abs(ps)) < 10
@@ -195,9 +215,9 @@ def test_config3_ks():
 def test_config4_euler(rk2):
     for N in (1 << 11, 1 << 14):  # full 5000 steps
         w = si.config(4, N=N, rk2=rk2)
-        check(w, w.nsteps, [64, 256], flavors=((sw.FLAVOR_TIER, 2),) + CHAR)
+        check(w, w.nsteps, [64, 256], flavors=((sw.FLAVOR_TIER, 2),) + CHAR + FLOW)
     w = si.config(4, N=1 << 20, rk2=rk2)
-    check(w, 70, [256], flavors=((sw.FLAVOR_TIER, 2),) + CHAR)
+    check(w, 70, [256], flavors=((sw.FLAVOR_TIER, 2),) + CHAR + FLOW)
 
 
 def test_config5_sampled_grid():
@@ -209,11 +229,11 @@ def test_config5_sampled_grid():
             if N == 1 << 11:
                 assert np.array_equal(ps, oracle.run_workload(w, nsteps=steps))
             for n in (32, 128, 512, 1024):
-                for fl, grp in ((sw.FLAVOR_TIER, 0), (sw.FLAVOR_CHAR, 16), (sw.FLAVOR_CHAR, 32)):
+                for fl, grp in ((sw.FLAVOR_TIER, 0), (sw.FLAVOR_CHAR, 16), (sw.FLAVOR_CHAR, 32), (sw.FLAVOR_FLOW, 0)):
                     try:
                         sx, _ = gpu_run(w, steps, sw.SWEPT, n, fl, grp)
                     except sw.SweptError as e:
-                        assert "not admissible" in str(e)
+                        assert "not admissible" in str(e) or "no FLOW kernel" in str(e)
                         continue
                     assert np.array_equal(ps, sx), (problem, N, n, fl, grp)
 
