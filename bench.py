@@ -331,7 +331,20 @@ def main():
     n_diamonds_top = sum(1 for p in plan if p[0] in (1, 2) and p[4] == tile)
     n_diamonds_all = sum(1 for p in plan if p[0] in (1, 2))
     fp64_instr_per_update = 3
-    if d_cnt and n_diamonds_all == n_diamonds_top:
+    flow_ms, flow_cnt = phase["FlowCycle"]
+    kernel_name = "swept Split/WholeDiamond (heat FP64)"
+    if flow_cnt:
+        # FLOW flavour: the dominant kernel is the persistent launch that runs whole Up..Down cycles; the
+        # sub-timesteps it covers = sum over the cycles of widths 256/512/1024 of (D+1) * m (swept_plan)
+        t_flow = 0
+        for p in plan:
+            if p[4] in (256, 512, 1024) and p[0] in (1, 2, 3):   # each diamond row and the Down row close m tiers
+                t_flow += p[4] // (2 * state.h)
+        avg_launch_ms = flow_ms / flow_cnt
+        ach_tflops = fp64_instr_per_update * 2 * w.N * t_flow * args.steps / (flow_ms * 1e-3) / 1e12
+        kernel_name = "swept_flow_kernel: persistent launch running whole Up..Down cycles (heat FP64)"
+        how = "CUDA events around every FLOW launch of the timed region (swept_phase_times)"
+    elif d_cnt and n_diamonds_all == n_diamonds_top:
         avg_launch_ms = d_ms / d_cnt
         ach_tflops = fp64_instr_per_update * 2 * w.N * m_top / (avg_launch_ms * 1e-3) / 1e12
         how = "CUDA events around every Split/WholeDiamond launch of the timed region (swept_phase_times)"
@@ -342,7 +355,7 @@ def main():
     step_tflops = fp64_instr_per_update * 2 * updates_per_step / (total_ms / args.steps * 1e-3) / 1e12
     roofline = {"bound": "alu", "achieved": ach_tflops, "peak": peak_tflops, "unit": "TFLOP/s",
                 "frac": ach_tflops / peak_tflops, "traffic": None,
-                "kernel": "swept Split/WholeDiamond (heat FP64)", "timed_by": how,
+                "kernel": kernel_name, "timed_by": how,
                 "note": "FMA-equivalent FP64 flops = 2 x 3 FP64-pipe instructions per update, N*m updates per "
                         f"launch (m = {m_top}); peak = {sms} SM x 64 lanes x 2 x {sm_max:.0f} MHz (nominal unit "
                         "count, max clock); probe = live DFMA-chain measurement",

@@ -121,7 +121,7 @@ const void* swept_device_ptr(swept_state* s);
 int swept_autotune(swept_state* s, int variant, int32_t* best_tile_width);
 
 /* swept_tuned — what swept_autotune remembered for `variant`: tile width, swept flavour and its group
- * parameter (TIER: points per thread; CHAR: lanes per tile); zeros if autotune has not run. */
+ * parameter (TIER: points per thread; CHAR: lanes per tile; FLOW: resident CTAs per SM); zeros if autotune has not run. */
 int swept_tuned(const swept_state* s, int variant, int32_t* tile_width, int32_t* flavor, int32_t* group);
 
 /* swept_set_stream — change the stream used by subsequent calls (cudaStream_t). */

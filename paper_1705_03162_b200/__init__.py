@@ -151,7 +151,7 @@ def swept_write(state: int, host_buf: np.ndarray) -> None:
 
 def swept_run(state: int, nsteps: int, tile_width: int, variant: int, flavor: int = FLAVOR_AUTO,
               group: int = 0) -> None:
-    """``group``: TIER points per thread / CHAR lanes per tile (0 = library default)."""
+    """``group``: TIER points per thread / CHAR lanes per tile / FLOW resident CTAs per SM (0 = library default)."""
     _check(load().swept_run_flavor(state, nsteps, tile_width, variant, flavor | (group << 8)))
 
 

@@ -39,7 +39,7 @@ struct FlowLaunch {
   int n, rows;       // tile width; rows = D + 2
   int* flags;        // rows * N/n ints, zeroed by the caller (stream-ordered)
   unsigned* ticket;  // zeroed by the caller
-  int warps;         // warps per CTA (0 = default)
+  int ctas_per_sm;   // resident CTAs (of 4 warps) per SM; 0 = default policy
   const double* consts;
   cudaStream_t stream;
 };

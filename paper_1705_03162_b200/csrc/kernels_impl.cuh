@@ -1,6 +1,5 @@
 // kernels_impl.cuh — templated host launchers shared by kernels_{heat,ks,euler}.cu.
 #pragma once
-#include <cstdlib>
 #include "internal.h"
 #include "per_step.cuh"
 #include "swept_tier.cuh"
@@ -169,8 +168,8 @@ inline bool flow_ok(int64_t N, int n) {
 template <class Prob, int B>
 inline int flow_go(const FlowLaunch& a) {
   using R = typename Prob::R;
-  const int warps = (a.warps >= 1 && a.warps <= 4) ? a.warps : 4;
-  const int threads = warps * 32;
+  constexpr int warps = 4;  // one per scheduler
+  constexpr int threads = warps * 32;
   FlowArgs<R> f;
   f.init = (const R*)a.init;
   for (int i = 0; i < 2; ++i)
@@ -188,10 +187,19 @@ inline int flow_go(const FlowLaunch& a) {
   e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, threads, smem);
   if (e != cudaSuccess) return (int)e;
   if (occ < 1) return (int)cudaErrorLaunchOutOfResources;
-  if (const char* cap = getenv("SWEPT_FLOW_CTAS_PER_SM"))  // experiment knob: fewer resident (waiting) warps
-    if (atoi(cap) >= 1 && atoi(cap) < occ) occ = atoi(cap);
   const int64_t ntasks = (int64_t)f.rows * f.K;
-  int64_t grid = (int64_t)occ * sms;
+  // Resident warps.  All warps run at the same pace, so the tile a warp takes next has its parents still in
+  // flight when the resident warps span a whole row (K tiles): waiting warps then only poll.  Default: about
+  // 7/8 K warps for the 3-point problem, K/2 for the 5-point ones (their tiles have more parallelism inside a
+  // warp and more registers); `ctas_per_sm` (autotuned) overrides.
+  int64_t per_sm = a.ctas_per_sm;
+  if (per_sm <= 0) {
+    const int64_t want = (Prob::H == 1 ? (int64_t)f.K * 7 / 8 : (int64_t)f.K / 2) / warps;  // CTAs
+    per_sm = (want + sms / 2) / sms;
+  }
+  if (per_sm < 1) per_sm = 1;
+  if (per_sm > occ) per_sm = occ;
+  int64_t grid = per_sm * sms;
   if (grid > (ntasks + warps - 1) / warps) grid = (ntasks + warps - 1) / warps;
   kern<<<(unsigned)grid, threads, smem, a.stream>>>(f);
   return (int)cudaGetLastError();

@@ -181,7 +181,7 @@ struct TimedScope {
 
 bool tile_ok(const swept_state* s, int flavor, int n, int P) {
   if (n <= 0 || s->N % n != 0) return false;
-  if (flavor == SWEPT_FLAVOR_FLOW && (s->problem == SWEPT_EULER || P < 0 || P > 4)) return false;
+  if (flavor == SWEPT_FLAVOR_FLOW && (s->problem == SWEPT_EULER || P < 0 || P > 16)) return false;
   switch (s->problem) {
     case SWEPT_HEAT: return swept::tile_config_ok_heat(s->dtype, flavor, s->N, n, P);
     case SWEPT_KS: return swept::tile_config_ok_ks(s->dtype, flavor, s->N, n, P);
@@ -415,7 +415,7 @@ int run_swept(swept_state* s, int64_t nsteps, int n, int flavor, int P) {
       swept::FlowLaunch f{};
       f.n = ph.n;
       f.rows = (int)(jp - ip + 1);
-      f.warps = cfg[ph.n].second;
+      f.ctas_per_sm = cfg[ph.n].second;
       f.init = s->slab[s->cur];
       // buffer 0 = the two slabs after cur, buffer 1 = the third one and cur itself (swept_flow.cuh: hazards)
       const int a0 = (s->cur + 1) & 3, a1 = (s->cur + 2) & 3, b0 = (s->cur + 3) & 3, b1 = s->cur;
@@ -706,14 +706,16 @@ int swept_autotune(swept_state* s, int variant, int32_t* best_tile_width) {
         for (int P : {1, 2, 4, 8, 16, 32})
           if (tile_ok(s, fl, n, P)) cands.push_back({n, fl, P});
     for (int n : {256, 512, 1024})
-      if (tile_ok(s, SWEPT_FLAVOR_FLOW, n, 0)) cands.push_back({n, SWEPT_FLAVOR_FLOW, 0});
+      for (int ctas : {1, 2, 3, 4, 6})  // resident CTAs per SM (clamped to the occupancy limit at launch)
+        if (tile_ok(s, SWEPT_FLAVOR_FLOW, n, ctas)) cands.push_back({n, SWEPT_FLAVOR_FLOW, ctas});
   }
   int rc_final = 0;
   for (const Cand& c : cands) {
-    // enough steps for Up + >= 4 diamonds + Down at this width (and a few graph chunks for per-step)
+    // enough steps for Up + 14 diamonds + Down at this width, so that the Up/Down rows and the start-up of a
+    // persistent FLOW launch weigh as little as in a long run (and a few graph chunks for per-step)
     int64_t steps;
     if (variant == SWEPT_PER_STEP) steps = 512;
-    else steps = std::max<int64_t>(6 * (c.n / (2 * sh.h)) / sh.sigma, 64);
+    else steps = std::max<int64_t>(16 * (c.n / (2 * sh.h)) / sh.sigma, 64);
     double t_best = 1e300;
     for (int rep = 0; rep < 3; ++rep) {  // rep 0 warms up (graph capture, attribute setting)
       cudaMemcpyAsync(s->slab[s->cur], backup, s->slab_bytes, cudaMemcpyDeviceToDevice, s->stream);

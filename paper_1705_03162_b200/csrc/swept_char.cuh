@@ -42,6 +42,46 @@ __device__ __forceinline__ float shfl_up_<float>(float v, int width) {
   return __shfl_up_sync(0xffffffffu, v, 1, width);
 }
 
+// Advance the B lines of one lane by one super-column `sc` (0 <= sc < m): 2h sub-columns (p mod 2h fixed), each a
+// dependent chain of B/2h points.  hal = the 2h lines below the lane's block after the neighbour's super-column
+// sc, halp = the same one super-column earlier (own-point-two-tiers-back operand of the first chain links).
+template <class Prob, int B, int L, int KIND>
+__device__ __forceinline__ void char_update_lines(typename Prob::R (&v)[Prob::C][B],
+                                                  const typename Prob::R (&hal)[Prob::C][2 * Prob::H],
+                                                  const typename Prob::R (&halp)[Prob::C][2 * Prob::H], const int sc,
+                                                  const int gl, const Consts<typename Prob::R>& kc) {
+  using R = typename Prob::R;
+  constexpr int H = Prob::H, C = Prob::C;
+  constexpr int n = B * L, m = n / (2 * H), BP = B / (2 * H);
+#pragma unroll
+  for (int rho = 0; rho < 2 * H; ++rho) {
+    R carry[C];  // previous value of line i-2h (tier t-2 of the point being computed)
+#pragma unroll
+    for (int c = 0; c < C; ++c) carry[c] = halp[c][rho];
+#pragma unroll
+    for (int aa = 0; aa < BP; ++aa) {
+      const int i = 2 * H - 1 - rho + 2 * H * aa;  // line updated in this sub-column
+      const int t = sc + gl * BP + aa + 1;         // its relative tier
+      const int odd = t & 1;
+      const bool act = KIND == KIND_UP ? (t > m) : (KIND == KIND_DOWN ? (t <= m) : true);
+      R win[C][2 * H + 1], bs[C][1], o[C][1];
+#pragma unroll
+      for (int c = 0; c < C; ++c) {
+#pragma unroll
+        for (int k = 0; k <= 2 * H; ++k)
+          win[c][k] = (i - k >= 0) ? v[c][(i - k >= 0) ? i - k : 0] : hal[c][(i - k >= 0) ? 0 : k - i - 1];
+        bs[c][0] = (Prob::SIGMA == 2 && !odd) ? carry[c] : win[c][H];
+      }
+      Prob::template stage<1>(win, bs, o, odd, kc);
+#pragma unroll
+      for (int c = 0; c < C; ++c) {
+        carry[c] = v[c][i];
+        if (act) v[c][i] = o[c][0];
+      }
+    }
+  }
+}
+
 // One super-step of a lane: fetch the 2h-line halo (shuffle, or the staged edge for group lane 0), update the
 // B lines of this lane (2h sub-columns, each a dependent chain of B/2h points), stream the top lines out
 // (group lane L-1).  GUARD = some lanes of the warp are outside their m super-columns (ramp up / down).
@@ -66,33 +106,7 @@ __device__ __forceinline__ void char_step(typename Prob::R (&v)[Prob::C][B],
       for (int e = 0; e < 2 * H; ++e) hal[c][e] = io[c * RS + e];
   }
   if (!GUARD || (sc >= 0 && sc < m)) {
-#pragma unroll
-    for (int rho = 0; rho < 2 * H; ++rho) {
-      R carry[C];  // previous value of line i-2h (tier t-2 of the point being computed)
-#pragma unroll
-      for (int c = 0; c < C; ++c) carry[c] = halp[c][rho];
-#pragma unroll
-      for (int aa = 0; aa < BP; ++aa) {
-        const int i = 2 * H - 1 - rho + 2 * H * aa;  // line updated in this sub-column
-        const int t = sc + gl * BP + aa + 1;         // its relative tier
-        const int odd = t & 1;
-        const bool act = KIND == KIND_UP ? (t > m) : (KIND == KIND_DOWN ? (t <= m) : true);
-        R win[C][2 * H + 1], bs[C][1], o[C][1];
-#pragma unroll
-        for (int c = 0; c < C; ++c) {
-#pragma unroll
-          for (int k = 0; k <= 2 * H; ++k)
-            win[c][k] = (i - k >= 0) ? v[c][(i - k >= 0) ? i - k : 0] : hal[c][(i - k >= 0) ? 0 : k - i - 1];
-          bs[c][0] = (Prob::SIGMA == 2 && !odd) ? carry[c] : win[c][H];
-        }
-        Prob::template stage<1>(win, bs, o, odd, kc);
-#pragma unroll
-        for (int c = 0; c < C; ++c) {
-          carry[c] = v[c][i];
-          if (act) v[c][i] = o[c][0];
-        }
-      }
-    }
+    char_update_lines<Prob, B, L, KIND>(v, hal, halp, sc, gl, kc);
     // upper-left edge: the top 2h lines of the last lane leave the tile
     if (KIND != KIND_DOWN && gl == L - 1) {
 #pragma unroll
@@ -103,6 +117,56 @@ __device__ __forceinline__ void char_step(typename Prob::R (&v)[Prob::C][B],
   }
   io += inc;
   inc = 2 * H - inc;
+}
+
+// Line values of one lane <-> the staged rows of its tile (rows, RS, ctr as in char_sweep_tile).
+template <class Prob, int B, int L, int KIND>
+__device__ __forceinline__ void char_load_lines(typename Prob::R (&v)[Prob::C][B], const typename Prob::R* rows, const int RS,
+                                   const int ctr, const int gl) {
+  using R = typename Prob::R;
+  constexpr int H = Prob::H, C = Prob::C, n = B * L;
+  auto slot = [&](int row, int c, int xp) -> const R& { return rows[(row * C + c) * RS + ctr + xp]; };
+  // initial line values: the point of line q just below the square (super-column -1), which is the latest
+  // (or second latest) tier stored at x' = -(h tq + r + 1); Up: the anti-diagonal = tier-0 data
+#pragma unroll
+  for (int i = 0; i < B; ++i) {
+    const int q = gl * B + i;
+    int xp, row;
+    if (KIND == KIND_UP) {
+      xp = n / 2 - 1 - q;
+      row = 0;
+    } else {
+      const int tq = q / (2 * H), r = i % (2 * H);
+      xp = -(H * tq + r + 1);
+      row = tq & 1;
+    }
+#pragma unroll
+    for (int c = 0; c < C; ++c) v[c][i] = slot(row, c, xp);
+  }
+}
+
+template <class Prob, int B, int L, int KIND>
+__device__ __forceinline__ void char_store_lines(const typename Prob::R (&v)[Prob::C][B], typename Prob::R* rows, const int RS,
+                                   const int ctr, const int gl) {
+  using R = typename Prob::R;
+  constexpr int H = Prob::H, C = Prob::C, n = B * L;
+  auto slot = [&](int row, int c, int xp) -> R& { return rows[(row * C + c) * RS + ctr + xp]; };
+  // upper-right edge (Down: the full time level): last value of every line
+#pragma unroll
+  for (int i = 0; i < B; ++i) {
+    const int q = gl * B + i;
+    int xp, row;
+    if (KIND == KIND_DOWN) {
+      xp = n / 2 - 1 - q;
+      row = 0;
+    } else {
+      const int tq = q / (2 * H), r = i % (2 * H);
+      xp = n / 2 - 1 - H * tq - r;
+      row = tq & 1;
+    }
+#pragma unroll
+    for (int c = 0; c < C; ++c) slot(row, c, xp) = v[c][i];
+  }
 }
 
 // The sweep of ONE tile by its group of L lanes (all of one warp): initial line values from the staged rows,
@@ -121,23 +185,7 @@ __device__ __forceinline__ void char_sweep_tile(typename Prob::R* rows, const in
   auto slot = [&](int row, int c, int xp) -> R& { return rows[(row * C + c) * RS + ctr + xp]; };
 
   R v[C][B], halA[C][2 * H], halB[C][2 * H];
-  // initial line values: the point of line q just below the square (super-column -1), which is the latest
-  // (or second latest) tier stored at x' = -(h tq + r + 1); Up: the anti-diagonal = tier-0 data
-#pragma unroll
-  for (int i = 0; i < B; ++i) {
-    const int q = gl * B + i;
-    int xp, row;
-    if (KIND == KIND_UP) {
-      xp = n / 2 - 1 - q;
-      row = 0;
-    } else {
-      const int tq = q / (2 * H), r = i % (2 * H);
-      xp = -(H * tq + r + 1);
-      row = tq & 1;
-    }
-#pragma unroll
-    for (int c = 0; c < C; ++c) v[c][i] = slot(row, c, xp);
-  }
+  char_load_lines<Prob, B, L, KIND>(v, rows, RS, ctr, gl);
 #pragma unroll
   for (int c = 0; c < C; ++c)
 #pragma unroll
@@ -166,23 +214,7 @@ __device__ __forceinline__ void char_sweep_tile(typename Prob::R* rows, const in
     char_step<Prob, B, L, KIND, true>(v, halB, halA, io, inc, s + 1, gl, RS, kc);
   }
   __syncwarp();
-  // upper-right edge (Down: the full time level): last value of every line
-#pragma unroll
-  for (int i = 0; i < B; ++i) {
-    const int q = gl * B + i;
-    int xp, row;
-    if (KIND == KIND_DOWN) {
-      xp = n / 2 - 1 - q;
-      row = 0;
-    } else {
-      const int tq = q / (2 * H), r = i % (2 * H);
-      xp = n / 2 - 1 - H * tq - r;
-      row = tq & 1;
-    }
-#pragma unroll
-    for (int c = 0; c < C; ++c) slot(row, c, xp) = v[c][i];
-  }
-
+  char_store_lines<Prob, B, L, KIND>(v, rows, RS, ctr, gl);
 }
 
 template <class Prob, int B, int L, int KIND>

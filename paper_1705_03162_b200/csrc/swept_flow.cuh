@@ -44,11 +44,6 @@ struct FlowArgs {
   Consts<R> k;
 };
 
-__device__ __forceinline__ int ld_acquire_gpu(const int* p) {
-  int v;
-  asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
-  return v;
-}
 // polling load: relaxed at GPU scope (no L1 invalidation per poll); the acquire fence follows once the flag is seen
 __device__ __forceinline__ int ld_relaxed_gpu(const int* p) {
   int v;

@@ -114,7 +114,7 @@ def test_wide_tiles():
     check(w, 700, [2048, 4096], flavors=((sw.FLAVOR_TIER, 4),))
 
 
-@pytest.mark.parametrize("warps", [1, 2, 4])
+@pytest.mark.parametrize("warps", [0, 1, 3])  # resident CTAs per SM (0 = default policy)
 def test_flow_flavour_many_cycles_and_small_grids(warps):
     # FLOW: one persistent launch per Up..Down cycle, rows chained by per-tile flags.  K = N/n = 1, 2 and
     # many tiles per row; D = 0 (Up + Down only), odd and even D; remainder levels; both RK2 flavours
