@@ -365,9 +365,15 @@ def main():
                 "whole_step_tflops": step_tflops, "whole_step_frac": step_tflops / peak_tflops,
                 "phase_ms_per_step": {k: v[0] / args.steps for k, v in phase.items()},
                 "phase_launches_per_step": {k: v[1] / args.steps for k, v in phase.items()}}
-    try:
-        with open(os.path.join(ROOT, "profiles", "traffic.json")) as f:
-            roofline["traffic"] = json.load(f).get("heat_diamond_dram_bytes_per_launch")
+    try:  # DRAM bytes per launch of the dominant kernel, from the committed ncu --set full capture
+        import csv
+        with open(os.path.join(ROOT, "profiles", "traffic.csv")) as f:
+            want = "swept_flow_kernel" if flow_cnt else "swept_char_kernel"
+            for row in csv.DictReader(f):
+                if row["kernel"].startswith(want):
+                    roofline["traffic"] = int(row["dram_bytes_per_launch"])
+                    roofline["traffic_source"] = row["source"]
+                    break
     except Exception:
         pass
 
