@@ -390,6 +390,16 @@ def main():
                                        "not HBM-bound (SURVEY.md §7 H7)"},
                   "swept_over_per_step": (updates_per_step / (statistics.median(step_ms) * 1e-3)) / ps_value,
                   "launch_us": sw.swept_probe_launch(2000)}
+        try:  # launch-free per-step baseline (PS_RESIDENT): same sub-timesteps, one persistent launch
+            rs_ms = time_runs(torch, sw, state, w, nsteps, 0, sw.PER_STEP, sw.PS_RESIDENT, 0, reps=3, flush=flush)
+            detail["per_step_resident"] = {"value": updates_per_step / (min(rs_ms) * 1e-3), "ms": min(rs_ms),
+                                           "us_per_substep": min(rs_ms) * 1e3 / (nsteps * state.sigma),
+                                           "note": "field in registers, neighbour-only flags between CTAs "
+                                                   "(DESIGN.md §5.7); bound by the L2 round trips of the edge exchange"}
+            detail["swept_over_per_step_resident"] = (updates_per_step / (statistics.median(step_ms) * 1e-3)) \
+                / detail["per_step_resident"]["value"]
+        except sw.SweptError as e:
+            detail["per_step_resident"] = {"unsupported": str(e)}
         detail["problems"] = problem_table(torch, sw, flush, hbm)
 
     cpu_base, _, _ = oracle_sample(w) if not args.no_detail else ({"value": None, "unit": UNIT, "cores": 0, "kind": "oracle", "sample": "skipped (--no-detail)"}, 0, 0)

@@ -104,11 +104,23 @@ int swept_write_device(swept_state* s, const void* device_buf);
  * Asynchronous on the state's stream; launch errors surface at the next synchronising call. */
 int swept_run(swept_state* s, int64_t nsteps, int32_t tile_width, int variant);
 
-/* swept_run_flavor — swept_run with an explicit swept kernel flavour (SWEPT_FLAVOR_*). */
+/* per-step flavours */
+enum {
+  SWEPT_PS_LAUNCH = 0,   /* one launch per sub-timestep (CUDA-graph replay): the paper's "Classic" */
+  SWEPT_PS_RESIDENT = 1  /* the same sub-timesteps in ONE persistent cooperative launch: field in registers,
+                            neighbour-only synchronisation through global flags (PAPER.md:297-303 future work;
+                            DESIGN.md §5.7).  Needs N small enough for a co-resident grid (heat FP64: N <= 2^20
+                            on B200), else SWEPT_EUNSUPPORTED; tile_width is ignored                            */
+};
+
+/* swept_run_flavor — swept_run with an explicit kernel flavour in bits 0..7 of `flavor` (SWEPT_FLAVOR_* for
+ * variant SWEPT_SWEPT, SWEPT_PS_* for SWEPT_PER_STEP) and the flavour's group parameter in bits 8..15
+ * (TIER: points per thread; CHAR: lanes per tile; FLOW: resident CTAs per SM; 0 = default). */
 int swept_run_flavor(swept_state* s, int64_t nsteps, int32_t tile_width, int variant, int flavor);
 
 /* swept_read — synchronise the stream and copy the current field to HOST memory (same layout as
- * swept_write). */
+ * swept_write).  Errors of the asynchronous launches since the last synchronising call surface here
+ * (SWEPT_ECUDA), including a FLOW launch whose dependency wait timed out. */
 int swept_read(swept_state* s, void* host_buf);
 
 /* swept_device_ptr — DEVICE pointer to the current full time level (C*N REALs), valid until the next

@@ -22,6 +22,7 @@ PER_STEP, SWEPT = 0, 1
 F64, F32 = 0, 1
 RK2_MIDPOINT, RK2_HEUN = 0, 1
 FLAVOR_AUTO, FLAVOR_TIER, FLAVOR_CHAR, FLAVOR_FLOW = 0, 1, 2, 3
+PS_LAUNCH, PS_RESIDENT = 0, 1  # per-step flavours
 KIND_NAMES = {0: "UpTriangle", 1: "SplitDiamond", 2: "WholeDiamond", 3: "DownTriangle", 4: "PerStepRemainder", 5: "FlowCycle"}
 
 _ALLOC_FN = CFUNCTYPE(c_void_p, c_void_p, c_uint64)

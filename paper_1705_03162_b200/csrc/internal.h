@@ -44,6 +44,23 @@ struct FlowLaunch {
   cudaStream_t stream;
 };
 
+// resident per-step: all sub-timesteps in one persistent cooperative launch (per_step_resident.cuh)
+struct ResidentLaunch {
+  const void* in;
+  void* out;
+  int64_t N, nsteps;
+  void* xch;       // device scratch, resident_scratch_bytes() bytes, 16-byte aligned; first the flags
+  const double* consts;
+  cudaStream_t stream;
+};
+// scratch needed for at most `max_ctas` CTAs (flags + error word, then the exchange slots of the widest problem)
+// layout: one 128-byte line per CTA flag, one line for the error word, then 2 x max_ctas x 2 exchange lines
+inline size_t resident_flag_bytes(int max_ctas) { return (size_t)(max_ctas + 1) * 128; }
+inline size_t resident_scratch_bytes(int max_ctas) {
+  return resident_flag_bytes(max_ctas) + (size_t)2 * max_ctas * 2 * 128;
+}
+constexpr int RESIDENT_MAX_CTAS = 4096;
+
 // dtype: 0 f64, 1 f32.  rk2: 0 midpoint, 1 Heun.  Return cudaError_t as int, or -1000 if the
 // combination has no kernel.
 int launch_per_step_heat(int dtype, const PerStepLaunch& a);
@@ -53,6 +70,9 @@ int launch_tile_heat(int dtype, const TileLaunch& a);
 int launch_tile_ks(int dtype, int rk2, const TileLaunch& a);
 int launch_tile_euler(int dtype, int rk2, const TileLaunch& a);
 // does a kernel exist for (flavor, n, P)?  (host-only query used by the autotuner and argument checks)
+int launch_resident_heat(int dtype, const ResidentLaunch& a);
+int launch_resident_ks(int dtype, int rk2, const ResidentLaunch& a);
+int launch_resident_euler(int dtype, int rk2, const ResidentLaunch& a);
 int launch_flow_heat(int dtype, const FlowLaunch& a);
 int launch_flow_ks(int dtype, int rk2, const FlowLaunch& a);
 bool tile_config_ok_heat(int dtype, int flavor, int64_t N, int n, int P);

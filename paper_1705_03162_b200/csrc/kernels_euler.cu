@@ -28,4 +28,8 @@ int launch_tile_euler(int dtype, int rk2, const TileLaunch& a) {
     return rk2 == 0 ? char_T<Euler<double, 0>, 16>(a) : char_T<Euler<double, 1>, 16>(a);
   return NO_KERNEL;
 }
+int launch_resident_euler(int dtype, int rk2, const ResidentLaunch& a) {
+  if (dtype != 0) return NO_KERNEL;
+  return rk2 == 0 ? resident_T<Euler<double, 0>, 2>(a) : resident_T<Euler<double, 1>, 2>(a);
+}
 }  // namespace swept

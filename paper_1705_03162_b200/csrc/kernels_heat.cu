@@ -18,4 +18,7 @@ int launch_tile_heat(int dtype, const TileLaunch& a) {
 int launch_flow_heat(int dtype, const FlowLaunch& a) {
   return dtype == 0 ? flow_T<Heat<double>, 32>(a) : flow_T<Heat<float>, 32>(a);
 }
+int launch_resident_heat(int dtype, const ResidentLaunch& a) {
+  return dtype == 0 ? resident_T<Heat<double>, 16>(a) : resident_T<Heat<float>, 16>(a);
+}
 }  // namespace swept

@@ -2,6 +2,7 @@
 #pragma once
 #include "internal.h"
 #include "per_step.cuh"
+#include "per_step_resident.cuh"
 #include "swept_tier.cuh"
 #include "swept_char.cuh"
 #include "swept_flow.cuh"
@@ -155,6 +156,51 @@ int char_T(const TileLaunch& a) {
   return NO_KERNEL;
 }
 
+
+// ---- resident per-step: one cooperative launch, the field in registers ---------------------------------
+template <class Prob, int P>
+inline int resident_try(const ResidentLaunch& a, int threads, int pass) {
+  using R = typename Prob::R;
+  if (a.N % P) return NO_KERNEL;
+  const int64_t nthr = a.N / P;
+  if (nthr < threads) threads = (int)((nthr + 31) / 32 * 32);
+  const int64_t G = (nthr + threads - 1) / threads;
+  auto kern = per_step_resident_kernel<Prob, P>;
+  const size_t smem = resident_smem_bytes<Prob>(threads);
+  int dev = 0, sms = 0, occ = 0;
+  cudaGetDevice(&dev);
+  cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+  if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, threads, smem) != cudaSuccess || occ < 1) {
+    cudaGetLastError();
+    return NO_KERNEL;
+  }
+  // pass 0: a single CTA (no global exchange at all); 1: one CTA per SM; 2: any co-resident grid
+  if (G > RESIDENT_MAX_CTAS || G > (pass == 0 ? 1 : (int64_t)sms * (pass == 1 ? 1 : occ))) return NO_KERNEL;
+  ResidentArgs<R> r;
+  r.in = (const R*)a.in; r.out = (R*)a.out; r.N = a.N; r.nsteps = a.nsteps;
+  r.flags = (int*)a.xch;
+  r.err = r.flags + RESIDENT_MAX_CTAS * 32;
+  r.xch = (R*)((char*)a.xch + resident_flag_bytes(RESIDENT_MAX_CTAS));
+  r.k = round_consts<R>(a.consts);
+  void* args[] = {&r};
+  return (int)cudaLaunchCooperativeKernel((const void*)kern, dim3((unsigned)G), dim3((unsigned)threads), args, smem,
+                                          a.stream);
+}
+
+// smallest P (most lanes busy per point) whose grid fits one CTA per SM, else any co-resident grid
+template <class Prob, int PMAX>
+int resident_T(const ResidentLaunch& a) {
+  constexpr int TMAX = Prob::MAX_THREADS < 512 ? Prob::MAX_THREADS : 512;
+  for (int pass = 0; pass < 3; ++pass) {
+    int rc = NO_KERNEL;
+    if (rc == NO_KERNEL && Prob::H <= 2 && PMAX >= 2) rc = resident_try<Prob, 2>(a, TMAX, pass);
+    if (rc == NO_KERNEL && PMAX >= 4) rc = resident_try<Prob, (PMAX >= 4 ? 4 : 2)>(a, TMAX, pass);
+    if (rc == NO_KERNEL && PMAX >= 8) rc = resident_try<Prob, (PMAX >= 8 ? 8 : 2)>(a, TMAX, pass);
+    if (rc == NO_KERNEL && PMAX >= 16) rc = resident_try<Prob, (PMAX >= 16 ? 16 : 2)>(a, TMAX, pass);
+    if (rc != NO_KERNEL) return rc;
+  }
+  return NO_KERNEL;
+}
 
 // ---- FLOW flavour: persistent launch, L = 32 lanes per tile, B = n / 32 lines per lane -----------------
 template <class Prob, int BMAX>

@@ -22,4 +22,8 @@ int launch_flow_ks(int dtype, int rk2, const FlowLaunch& a) {
   if (dtype != 0) return NO_KERNEL;
   return rk2 == 0 ? flow_T<KS<double, 0>, 32>(a) : flow_T<KS<double, 1>, 32>(a);
 }
+int launch_resident_ks(int dtype, int rk2, const ResidentLaunch& a) {
+  if (dtype != 0) return NO_KERNEL;
+  return rk2 == 0 ? resident_T<KS<double, 0>, 8>(a) : resident_T<KS<double, 1>, 8>(a);
+}
 }  // namespace swept

@@ -81,6 +81,9 @@ struct swept_state {
   // FLOW flavour scratch: ticket counter + one flag per tile of a cycle
   int* flow_scratch = nullptr;
   size_t flow_scratch_ints = 0;
+  bool flow_pending_check = false;
+  void* resident_scratch = nullptr;  // flags + exchange slots of the resident per-step kernel
+  bool resident_pending_check = false;  // a FLOW launch has run since the error word was last read
   size_t elem() const { return dtype == SWEPT_F64 ? 8 : 4; }
 };
 
@@ -136,8 +139,11 @@ int launch_flow(swept_state* s, swept::FlowLaunch& a) {
     }
     CUDA_TRY(cudaMalloc((void**)&s->flow_scratch, need * sizeof(int)));
     s->flow_scratch_ints = need;
+    CUDA_TRY(cudaMemsetAsync(s->flow_scratch, 0, 4 * sizeof(int), s->stream));
   }
-  CUDA_TRY(cudaMemsetAsync(s->flow_scratch, 0, need * sizeof(int), s->stream));
+  // word 0 = ticket, word 1 = sticky error word (cleared when read), words 4.. = one flag per tile
+  CUDA_TRY(cudaMemsetAsync(s->flow_scratch, 0, sizeof(int), s->stream));
+  CUDA_TRY(cudaMemsetAsync(s->flow_scratch + 4, 0, (need - 4) * sizeof(int), s->stream));
   a.ticket = (unsigned*)s->flow_scratch;
   a.flags = s->flow_scratch + 4;
   int rc;
@@ -148,6 +154,26 @@ int launch_flow(swept_state* s, swept::FlowLaunch& a) {
   }
   if (rc == NO_KERNEL) return fail(SWEPT_EUNSUPPORTED, "no FLOW kernel for this problem / n=%d", a.n);
   if (rc != 0) return fail(SWEPT_ECUDA, "flow launch: %s", cudaGetErrorString((cudaError_t)rc));
+  s->flow_pending_check = true;
+  return 0;
+}
+
+// after a stream synchronisation: did any FLOW launch give up waiting for a dependency?
+int check_flow_error(swept_state* s) {
+  if (s->resident_pending_check && s->resident_scratch) {
+    s->resident_pending_check = false;
+    int err = 0;
+    int* word = (int*)s->resident_scratch + swept::RESIDENT_MAX_CTAS * 32;
+    CUDA_TRY(cudaMemcpy(&err, word, sizeof(int), cudaMemcpyDeviceToHost));
+    if (err) CUDA_TRY(cudaMemset(word, 0, sizeof(int)));
+    if (err) return fail(SWEPT_ECUDA, "resident per-step kernel: a CTA waited too long for its neighbour");
+  }
+  if (!s->flow_pending_check || !s->flow_scratch) return 0;
+  s->flow_pending_check = false;
+  int err = 0;
+  CUDA_TRY(cudaMemcpy(&err, s->flow_scratch + 1, sizeof(int), cudaMemcpyDeviceToHost));
+  if (err) CUDA_TRY(cudaMemset(s->flow_scratch + 1, 0, sizeof(int)));
+  if (err) return fail(SWEPT_ECUDA, "FLOW kernel: a tile waited too long for its parents (grid not co-resident?)");
   return 0;
 }
 
@@ -260,6 +286,33 @@ int run_per_step(swept_state* s, int64_t steps, int threads) {
     s->cur = cur;
     s->last_launches += left * sigma;
   }
+  return 0;
+}
+
+// ---- resident per-step: every sub-timestep in one persistent launch (per_step_resident.cuh) -----------
+int run_resident(swept_state* s, int64_t steps) {
+  if (steps <= 0) return 0;
+  if (!s->resident_scratch) {
+    CUDA_TRY(cudaMalloc(&s->resident_scratch, swept::resident_scratch_bytes(swept::RESIDENT_MAX_CTAS)));
+    CUDA_TRY(cudaMemsetAsync(s->resident_scratch, 0, swept::resident_flag_bytes(swept::RESIDENT_MAX_CTAS), s->stream));
+  }
+  // flags restart from zero every launch; the error word behind them is sticky until swept_read looks at it
+  CUDA_TRY(cudaMemsetAsync(s->resident_scratch, 0, (size_t)swept::RESIDENT_MAX_CTAS * 128, s->stream));
+  const int nxt = (s->cur + 1) & 3;
+  swept::ResidentLaunch a{s->slab[s->cur], s->slab[nxt], s->N, steps, s->resident_scratch, s->consts, s->stream};
+  int rc;
+  switch (s->problem) {
+    case SWEPT_HEAT: rc = swept::launch_resident_heat(s->dtype, a); break;
+    case SWEPT_KS: rc = swept::launch_resident_ks(s->dtype, s->rk2, a); break;
+    default: rc = swept::launch_resident_euler(s->dtype, s->rk2, a); break;
+  }
+  if (rc == NO_KERNEL)
+    return fail(SWEPT_EUNSUPPORTED, "N=%lld does not fit a co-resident register-resident grid for this problem",
+                (long long)s->N);
+  if (rc != 0) return fail(SWEPT_ECUDA, "resident per-step launch: %s", cudaGetErrorString((cudaError_t)rc));
+  s->cur = nxt;
+  s->last_launches += 1;
+  s->resident_pending_check = true;
   return 0;
 }
 
@@ -567,6 +620,7 @@ void swept_destroy(swept_state* s) {
   for (auto& t : s->timed) { cudaEventDestroy(t.e0); cudaEventDestroy(t.e1); }
   for (cudaEvent_t e : s->event_pool) cudaEventDestroy(e);
   if (s->flow_scratch) cudaFree(s->flow_scratch);
+  if (s->resident_scratch) cudaFree(s->resident_scratch);
   for (int i = 0; i < 4; ++i) {
     if (!s->slab[i]) continue;
     if (s->free_) s->free_(s->alloc_ctx, s->slab[i]);
@@ -627,7 +681,7 @@ int swept_read(swept_state* s, void* host_buf) {
   if (int rc = set_device(s)) return rc;
   CUDA_TRY(cudaMemcpyAsync(host_buf, s->slab[s->cur], s->slab_bytes, cudaMemcpyDeviceToHost, s->stream));
   CUDA_TRY(cudaStreamSynchronize(s->stream));
-  return 0;
+  return check_flow_error(s);
 }
 
 const void* swept_device_ptr(swept_state* s) { return s ? s->slab[s->cur] : nullptr; }
@@ -642,8 +696,14 @@ int swept_run_flavor(swept_state* s, int64_t nsteps, int32_t tile_width, int var
   s->last_launches = 0;
   int rc;
   if (variant == SWEPT_PER_STEP) {
-    int tw = tile_width ? tile_width : s->tuned_width[SWEPT_PER_STEP];
-    rc = run_per_step(s, nsteps, tw);
+    if ((flavor & 0xff) == SWEPT_PS_RESIDENT) {
+      rc = run_resident(s, nsteps);
+    } else if ((flavor & 0xff) != SWEPT_PS_LAUNCH) {
+      return fail(SWEPT_EINVAL, "unknown per-step flavor %d", flavor & 0xff);
+    } else {
+      int tw = tile_width ? tile_width : s->tuned_width[SWEPT_PER_STEP];
+      rc = run_per_step(s, nsteps, tw);
+    }
   } else if (variant == SWEPT_SWEPT) {
     int fl = flavor & 0xff, P = (flavor >> 8) & 0xff;  // bits 8..15: explicit P / lane-group size (0 = default)
     if (fl != SWEPT_FLAVOR_AUTO && fl != SWEPT_FLAVOR_TIER && fl != SWEPT_FLAVOR_CHAR && fl != SWEPT_FLAVOR_FLOW)

@@ -40,7 +40,7 @@ struct FlowArgs {
   int K;          // tiles per row = N / n
   int rows;       // D + 2
   int* flags;     // rows * K, zero on entry; flags[r * K + k] = 1 once tile (r, k) is in global memory
-  unsigned* ticket;  // zero on entry
+  unsigned* ticket;  // zero on entry; ticket[1] is an error word (set if a dependency wait timed out)
   Consts<R> k;
 };
 
@@ -104,10 +104,16 @@ __global__ void __launch_bounds__(128) swept_flow_kernel(const FlowArgs<typename
       const int p0 = (r & 1) ? k : (k == 0 ? a.K - 1 : k - 1);
       const int p1 = (r & 1) ? (k + 1 == a.K ? 0 : k + 1) : k;
       const int* f = a.flags + (size_t)(r - 1) * a.K;
-      unsigned ns = 64;
+      unsigned ns = 64, polls = 0;
       while (ld_relaxed_gpu(f + p0) == 0 || ld_relaxed_gpu(f + p1) == 0) {
         __nanosleep(ns);
         if (ns < 2048) ns *= 2;
+        // cannot happen while the grid is co-resident; bounded so that a scheduling surprise yields an error
+        // code (swept_read reports it) instead of a hung device: 2^22 polls x >= 2 us
+        if (++polls > (1u << 22)) {
+          if (lane == 0) atomicExch(a.ticket + 1, 1u);
+          break;
+        }
       }
       fence_acq_rel_gpu();
     }

@@ -133,6 +133,40 @@ def test_flow_flavour_many_cycles_and_small_grids(warps):
     s.close()
 
 
+def test_per_step_resident_matches_oracle():
+    # per-step sub-timesteps in one persistent cooperative launch (PS_RESIDENT): single CTA (no global exchange),
+    # several CTAs (neighbour flags), a ragged last CTA, N not a power of two, both RK2 flavours, FP32
+    cases = [(si.heat_sines(2048, 8, 3, 700), np.float64), (si.heat_sines(1 << 16, 8, 4, 300), np.float64),
+             (si.heat_sines(1 << 20, 16, 5, 150), np.float64), (si.heat_sines(3000, 4, 6, 200), np.float64),
+             (si.heat_sines(100000, 4, 7, 120), np.float64), (si.heat_sines(1 << 17, 8, 8, 200), np.float32),
+             (si.ks_cos(4096, 9, 150), np.float64), (si.ks_cos(1 << 18, 10, 60), np.float64),
+             (si.euler_double_sod(2048, 80), np.float64), (si.euler_double_sod(1 << 15, 40), np.float64)]
+    w = si.ks_cos(1 << 14, 11, 90)
+    w.rk2 = si.RK2_HEUN
+    cases.append((w, np.float64))
+    cases.append((si.euler_double_sod(4096, 50, rk2=si.RK2_MIDPOINT), np.float64))
+    for w, dtype in cases:
+        ref = oracle.run_workload(w, dtype=dtype)
+        got, launches = gpu_run(w, w.nsteps, sw.PER_STEP, 0, sw.PS_RESIDENT, dtype=dtype)
+        assert launches == 1
+        assert np.array_equal(got, ref), (w.name, w.N, dtype)
+    # continues from a swept run and into a launch-per-step run on the same state
+    w = si.heat_sines(8192, 8, 2, 0)
+    s = sw.Swept.from_workload(w)
+    s.run(300, 256, sw.SWEPT)
+    s.run(77, 0, sw.PER_STEP, sw.PS_RESIDENT)
+    s.run(23, 0, sw.PER_STEP)
+    got = s.read()
+    s.close()
+    assert np.array_equal(got, oracle.run_workload(w, nsteps=400))
+    # too large for a co-resident register-resident grid: a clean error, no fallback
+    w = si.heat_sines(1 << 26, 4, 2, 0)
+    s = sw.Swept.from_workload(w)
+    with pytest.raises(sw.SweptError):
+        s.run(10, 0, sw.PER_STEP, sw.PS_RESIDENT)
+    s.close()
+
+
 def test_per_step_non_power_of_two_N():
     # the paper's `& lastidx` wrap needs N = 2^k; ours does not
     for N in (1000, 1001, 1002):
