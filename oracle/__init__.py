@@ -50,6 +50,8 @@ def _load():
         vp = ctypes.c_void_p
         lib.oracle_heat_f64.argtypes = [vp, i64, i64, dbl, dbl, dbl]
         lib.oracle_heat_f32.argtypes = [vp, i64, i64, dbl, dbl, dbl]
+        lib.oracle_heat_bc_f64.argtypes = [vp, i64, i64, dbl, dbl, dbl, ci]
+        lib.oracle_heat_bc_f32.argtypes = [vp, i64, i64, dbl, dbl, dbl, ci]
         lib.oracle_ks_f64.argtypes = [vp, i64, i64, dbl, dbl, ci]
         lib.oracle_ks_f32.argtypes = [vp, i64, i64, dbl, dbl, ci]
         lib.oracle_euler_f64.argtypes = [vp, i64, i64, dbl, dbl, dbl, ci]
@@ -70,11 +72,12 @@ def set_num_threads(n: int) -> None:
 
 def run(problem: int, u0: np.ndarray, N: int, nsteps: int, dx: float, dt: float, *,
         alpha: float = 1.0, gamma: float = 1.4, rk2: int = RK2_MIDPOINT,
-        dtype=np.float64) -> np.ndarray:
+        dtype=np.float64, bc: int = 0) -> np.ndarray:
     """Advance ``u0`` (component-major, C*N values) by ``nsteps`` full timesteps; returns a new array.
 
     ``dtype`` float64 or float32 selects the arithmetic type of the whole computation (reading X15: the
     FP32 GPU path is gated against the FP32 instantiation of these same expression trees).
+    ``bc``: 0 periodic (the configs), 1 the paper's insulated ends for heat, Eq. (B.5) PAPER.md:328-331.
     """
     lib = _load()
     dtype = np.dtype(dtype)
@@ -84,8 +87,11 @@ def run(problem: int, u0: np.ndarray, N: int, nsteps: int, dx: float, dt: float,
         raise ValueError(f"expected {C * N} values, got {u.size}")
     sfx = "f64" if dtype == np.float64 else "f32"
     ptr = u.ctypes.data_as(ctypes.c_void_p)
+    if bc and problem != HEAT:
+        raise ValueError("boundary conditions other than periodic exist for the heat problem only (B.5)")
     if problem == HEAT:
-        rc = getattr(lib, "oracle_heat_" + sfx)(ptr, N, nsteps, dx, dt, alpha)
+        rc = getattr(lib, "oracle_heat_bc_" + sfx)(ptr, N, nsteps, dx, dt, alpha, bc) if bc else \
+            getattr(lib, "oracle_heat_" + sfx)(ptr, N, nsteps, dx, dt, alpha)
     elif problem == KS:
         rc = getattr(lib, "oracle_ks_" + sfx)(ptr, N, nsteps, dx, dt, rk2)
     elif problem == EULER:
@@ -100,4 +106,4 @@ def run(problem: int, u0: np.ndarray, N: int, nsteps: int, dx: float, dt: float,
 def run_workload(w, nsteps: int | None = None, dtype=np.float64) -> np.ndarray:
     """Run a ``swept_inputs.Workload`` (duck-typed: no import of that module needed)."""
     return run(w.problem, w.u0, w.N, w.nsteps if nsteps is None else nsteps, w.dx, w.dt,
-               alpha=w.alpha, gamma=w.gamma, rk2=w.rk2, dtype=dtype)
+               alpha=w.alpha, gamma=w.gamma, rk2=w.rk2, dtype=dtype, bc=getattr(w, "bc", 0))

@@ -27,7 +27,10 @@
 //       PARITY UNPINNED (any reading with the same 0/inf/NaN classes is the same scheme in exact
 //       arithmetic away from those classes).
 //   X6  RK2 flavour: midpoint (the paper's) and Heun (BASELINE.json config 4) both provided.
-//   X10 periodic boundaries for all three problems (BASELINE.json configs).
+//   X10 periodic boundaries for all three problems (BASELINE.json configs); the paper's own heat
+//       boundary condition, insulated ends (B.5) PAPER.md:328-331, is available as bc = 1:
+//       T_{-1} = T_1 and T_N = T_{N-2} for points 0..N-1 (mirror about the end POINTS; the paper's
+//       index "n+1" is read with points 0..n).
 //
 // Floating point: every expression below is a fixed tree of IEEE-754 operations.  Build with
 // -ffp-contract=off so the compiler never fuses a*b+c on its own; the fused operations that ARE
@@ -61,8 +64,16 @@ inline int64_t wrap(int64_t i, int64_t N) {
 
 // ---------------------------------------------------------------- heat, Eq. (B.4)
 // T_i^{m+1} = Fo (T_{i+1} + T_{i-1}) + (1 - 2 Fo) T_i
+// bc = 0: periodic neighbours.  bc = 1: insulated ends, Eq. (B.5): T_{-1} = T_1, T_N = T_{N-2}.
+inline int64_t heat_nb(int64_t i, int64_t N, int bc) {
+    if (bc == 0) return wrap(i, N);
+    if (i < 0) return -i;
+    if (i >= N) return 2 * (N - 1) - i;
+    return i;
+}
+
 template <class R>
-void heat_run(R* u, int64_t N, int64_t nsteps, double dx, double dt, double alpha) {
+void heat_run(R* u, int64_t N, int64_t nsteps, double dx, double dt, double alpha, int bc = 0) {
     const double Fo_d = alpha * dt / (dx * dx);  // Fourier number
     const R Fo = (R)Fo_d;
     const R c0 = (R)(1.0 - 2.0 * Fo_d);
@@ -72,7 +83,7 @@ void heat_run(R* u, int64_t N, int64_t nsteps, double dx, double dt, double alph
     for (int64_t s = 0; s < nsteps; ++s) {
 #pragma omp parallel for schedule(static) if (N >= OMP_MIN_N)
         for (int64_t i = 0; i < N; ++i) {
-            const R um = a[wrap(i - 1, N)], u0 = a[i], up = a[wrap(i + 1, N)];
+            const R um = a[heat_nb(i - 1, N, bc)], u0 = a[i], up = a[heat_nb(i + 1, N, bc)];
             const R sum = um + up;
             const R t = c0 * u0;
             b[i] = std::fma(Fo, sum, t);
@@ -254,6 +265,17 @@ int oracle_heat_f64(double* u, int64_t N, int64_t nsteps, double dx, double dt, 
 int oracle_heat_f32(float* u, int64_t N, int64_t nsteps, double dx, double dt, double alpha) {
     if (!u || N < 3 || nsteps < 0) return -1;
     heat_run<float>(u, N, nsteps, dx, dt, alpha);
+    return 0;
+}
+// heat with an explicit boundary condition: bc = 0 periodic, 1 insulated (B.5)
+int oracle_heat_bc_f64(double* u, int64_t N, int64_t nsteps, double dx, double dt, double alpha, int bc) {
+    if (!u || N < 3 || nsteps < 0 || bc < 0 || bc > 1) return -1;
+    heat_run<double>(u, N, nsteps, dx, dt, alpha, bc);
+    return 0;
+}
+int oracle_heat_bc_f32(float* u, int64_t N, int64_t nsteps, double dx, double dt, double alpha, int bc) {
+    if (!u || N < 3 || nsteps < 0 || bc < 0 || bc > 1) return -1;
+    heat_run<float>(u, N, nsteps, dx, dt, alpha, bc);
     return 0;
 }
 int oracle_ks_f64(double* u, int64_t N, int64_t nsteps, double dx, double dt, int rk2) {

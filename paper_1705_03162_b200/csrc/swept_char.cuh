@@ -93,7 +93,7 @@ __device__ __forceinline__ void char_step(typename Prob::R (&v)[Prob::C][B],
                                           const Consts<typename Prob::R>& kc) {
   using R = typename Prob::R;
   constexpr int H = Prob::H, C = Prob::C;
-  constexpr int n = B * L, m = n / (2 * H), BP = B / (2 * H);
+  constexpr int n = B * L, m = n / (2 * H);
   const int sc = s - gl;  // this lane's super-column
 #pragma unroll
   for (int c = 0; c < C; ++c)

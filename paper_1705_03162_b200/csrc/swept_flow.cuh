@@ -80,6 +80,10 @@ __device__ __forceinline__ void warp_store_row(R* __restrict__ dst, const R* src
   }
 }
 
+#ifndef FLOW_MAX_SLEEP
+#define FLOW_MAX_SLEEP 256
+#endif
+
 template <class Prob, int B>
 __global__ void __launch_bounds__(128) swept_flow_kernel(const FlowArgs<typename Prob::R> a) {
   using R = typename Prob::R;
@@ -104,10 +108,10 @@ __global__ void __launch_bounds__(128) swept_flow_kernel(const FlowArgs<typename
       const int p0 = (r & 1) ? k : (k == 0 ? a.K - 1 : k - 1);
       const int p1 = (r & 1) ? (k + 1 == a.K ? 0 : k + 1) : k;
       const int* f = a.flags + (size_t)(r - 1) * a.K;
-      unsigned ns = 64, polls = 0;
+      unsigned ns = 32, polls = 0;
       while (ld_relaxed_gpu(f + p0) == 0 || ld_relaxed_gpu(f + p1) == 0) {
         __nanosleep(ns);
-        if (ns < 2048) ns *= 2;
+        if (ns < FLOW_MAX_SLEEP) ns *= 2;
         // cannot happen while the grid is co-resident; bounded so that a scheduling surprise yields an error
         // code (swept_read reports it) instead of a hung device: 2^22 polls x >= 2 us
         if (++polls > (1u << 22)) {

@@ -43,6 +43,7 @@ class Workload:
     rk2: int = RK2_MIDPOINT
     name: str = ""
     meta: dict = field(default_factory=dict)
+    bc: int = 0  # 0 periodic (BASELINE.json configs); 1 = the paper's insulated heat ends, Eq. (B.5)
 
     @property
     def components(self) -> int:
@@ -66,6 +67,24 @@ def heat_sines(N: int, nmodes: int, seed: int, nsteps: int, r: float = 0.25, alp
     dt = r * dx * dx / alpha
     return Workload(HEAT, N, dx, dt, nsteps, u0, alpha=alpha, name=name or f"heat_N{N}",
                     meta={"amps": amps, "r": r})
+
+
+BC_PERIODIC, BC_PAPER = 0, 1
+
+
+def heat_insulated(N: int, nmodes: int, seed: int, nsteps: int, r: float = 0.25, name: str = "") -> Workload:
+    """The paper's own heat set-up: N points 0..N-1 with insulated ends (B.5), here with
+    u0_i = a_0 + sum_{k=1..K} a_k cos(pi k i / (N-1)), a_k ~ U(-1, 1) — cosines are the eigenmodes of the
+    mirrored stencil, so the closed form of the pin is g_k = 1 - 4 r sin^2(pi k / (2 (N-1))).  dx = 1/(N-1)."""
+    rng = np.random.default_rng(seed)
+    amps = rng.uniform(-1.0, 1.0, size=nmodes + 1)
+    i = np.arange(N, dtype=np.float64)
+    u0 = np.full(N, amps[0], dtype=np.float64)
+    for k in range(1, nmodes + 1):
+        u0 += amps[k] * np.cos(np.pi * k * i / (N - 1))
+    dx = 1.0 / (N - 1)
+    return Workload(HEAT, N, dx, r * dx * dx, nsteps, u0, name=name or f"heat_insulated_N{N}",
+                    meta={"amps": amps, "r": r}, bc=BC_PAPER)
 
 
 def ks_cos(N: int, seed: int, nsteps: int, dx: float = 0.5, dt: float = 0.005,
