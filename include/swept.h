@@ -43,6 +43,11 @@ enum { SWEPT_PER_STEP = 0, SWEPT_SWEPT = 1 };               /* variant          
 enum { SWEPT_F64 = 0, SWEPT_F32 = 1 };                      /* dtype                             */
 enum { SWEPT_RK2_MIDPOINT = 0, SWEPT_RK2_HEUN = 1 };        /* KS/Euler integrator (
                                                                Heun is BASELINE.json config 4)   */
+/* boundary conditions: periodic (all BASELINE.json configs) or the paper's own: insulated ends for heat,
+ * Eq. (B.5), T_{-1} = T_1 and T_N = T_{N-2} for points 0..N-1.  SWEPT_BC_PAPER is built for
+ * the heat problem, per-step (launch per sub-timestep) and swept TIER flavour, where the tile split across
+ * the boundary applies the condition at its centre; other combinations: SWEPT_EUNSUPPORTED. */
+enum { SWEPT_BC_PERIODIC = 0, SWEPT_BC_PAPER = 1 };
 enum { SWEPT_NKINDS = 6 };                                   /* phase kinds reported by swept_phase_times */
 enum { SWEPT_OK = 0, SWEPT_EINVAL = -1, SWEPT_EUNSUPPORTED = -2, SWEPT_ECUDA = -3, SWEPT_ENOMEM = -4 };
 
@@ -74,6 +79,8 @@ typedef struct {
   swept_alloc_fn alloc; /* NULL = cudaMalloc                                                         */
   swept_free_fn free;   /* NULL = cudaFree                                                           */
   void* alloc_ctx;      /* passed back to alloc/free                                                 */
+  int32_t bc;           /* SWEPT_BC_PERIODIC (default) or SWEPT_BC_PAPER                                */
+  int32_t reserved0;    /* 0                                                                           */
 } swept_params;
 
 /* swept_create — set up one problem: N periodic points, spacing dx, fixed timestep dt.

@@ -23,6 +23,7 @@ F64, F32 = 0, 1
 RK2_MIDPOINT, RK2_HEUN = 0, 1
 FLAVOR_AUTO, FLAVOR_TIER, FLAVOR_CHAR, FLAVOR_FLOW = 0, 1, 2, 3
 PS_LAUNCH, PS_RESIDENT = 0, 1  # per-step flavours
+BC_PERIODIC, BC_PAPER = 0, 1   # BC_PAPER: insulated heat ends, Eq. (B.5)
 KIND_NAMES = {0: "UpTriangle", 1: "SplitDiamond", 2: "WholeDiamond", 3: "DownTriangle", 4: "PerStepRemainder", 5: "FlowCycle"}
 
 _ALLOC_FN = CFUNCTYPE(c_void_p, c_void_p, c_uint64)
@@ -32,7 +33,8 @@ _FREE_FN = CFUNCTYPE(None, c_void_p, c_void_p)
 class swept_params(Structure):
     _fields_ = [("struct_size", c_uint32), ("dtype", c_int32), ("rk2", c_int32), ("device", c_int32),
                 ("alpha", c_double), ("gamma", c_double), ("stream", c_void_p),
-                ("alloc", _ALLOC_FN), ("free", _FREE_FN), ("alloc_ctx", c_void_p)]
+                ("alloc", _ALLOC_FN), ("free", _FREE_FN), ("alloc_ctx", c_void_p),
+                ("bc", c_int32), ("reserved0", c_int32)]
 
 
 class swept_phase(Structure):
@@ -127,11 +129,12 @@ def _current_stream() -> int:
 
 # ---- the C ABI, same names ----------------------------------------------------------------------------
 def swept_create(problem: int, N: int, dx: float, dt: float, *, dtype: int = F64, rk2: int = RK2_MIDPOINT,
-                 alpha: float = 1.0, gamma: float = 1.4, device: int = -1, use_torch: bool = True) -> int:
+                 alpha: float = 1.0, gamma: float = 1.4, device: int = -1, use_torch: bool = True,
+                 bc: int = BC_PERIODIC) -> int:
     lib = load()
     p = swept_params()
     p.struct_size = ctypes.sizeof(swept_params)
-    p.dtype, p.rk2, p.device, p.alpha, p.gamma = dtype, rk2, device, alpha, gamma
+    p.dtype, p.rk2, p.device, p.alpha, p.gamma, p.bc = dtype, rk2, device, alpha, gamma, bc
     if use_torch:
         import torch
         if not torch.cuda.is_available():
@@ -218,18 +221,19 @@ class Swept:
     """Convenience wrapper: one problem instance on the current CUDA device."""
 
     def __init__(self, problem: int, N: int, dx: float, dt: float, *, dtype=np.float64, rk2: int = RK2_MIDPOINT,
-                 alpha: float = 1.0, gamma: float = 1.4):
+                 alpha: float = 1.0, gamma: float = 1.4, bc: int = BC_PERIODIC):
         self.problem, self.N = problem, N
         self.np_dtype = np.dtype(dtype)
         self.C = 3 if problem == EULER else 1
         self.h = 1 if problem == HEAT else 2
         self.sigma = 1 if problem == HEAT else 2
         self._h = swept_create(problem, N, dx, dt, dtype=F64 if self.np_dtype == np.float64 else F32, rk2=rk2,
-                               alpha=alpha, gamma=gamma)
+                               alpha=alpha, gamma=gamma, bc=bc)
 
     @classmethod
     def from_workload(cls, w, dtype=np.float64) -> "Swept":
-        s = cls(w.problem, w.N, w.dx, w.dt, dtype=dtype, rk2=w.rk2, alpha=w.alpha, gamma=w.gamma)
+        s = cls(w.problem, w.N, w.dx, w.dt, dtype=dtype, rk2=w.rk2, alpha=w.alpha, gamma=w.gamma,
+                bc=getattr(w, "bc", BC_PERIODIC))
         s.write(w.u0)
         return s
 

@@ -15,6 +15,7 @@ struct PerStepLaunch {
   int P;        // points per thread (N % P == 0)
   const double* consts;  // 5 doubles, rounded once to REAL by the launcher
   cudaStream_t stream;
+  int bc = 0;   // 0 periodic, 1 insulated ends (heat only)
 };
 
 struct TileLaunch {
@@ -29,6 +30,7 @@ struct TileLaunch {
   int flavor;  // SWEPT_FLAVOR_TIER / SWEPT_FLAVOR_CHAR
   const double* consts;
   cudaStream_t stream;
+  int bc = 0;  // 0 periodic, 1 insulated ends (heat, TIER flavour only)
 };
 
 // FLOW flavour: one whole Up / diamonds / Down cycle of tile width n in a single persistent launch

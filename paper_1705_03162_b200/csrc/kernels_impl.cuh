@@ -24,7 +24,7 @@ inline int per_step_go(const PerStepLaunch& a) {
   const int threads = a.threads < Prob::MAX_THREADS ? a.threads : Prob::MAX_THREADS;
   const unsigned grid = (unsigned)((nthreads + threads - 1) / threads);
   per_step_kernel<Prob, P><<<grid, threads, 0, a.stream>>>((const R*)a.in, (const R*)a.base, (R*)a.out,
-                                                             a.N, a.odd, round_consts<R>(a.consts));
+                                                             a.N, a.odd, round_consts<R>(a.consts), a.bc);
   return (int)cudaGetLastError();
 }
 
@@ -45,6 +45,7 @@ inline int tier_go(const TileLaunch& a) {
   TierArgs<R> t;
   t.in0 = (const R*)a.in0; t.in1 = (const R*)a.in1; t.out0 = (R*)a.out0; t.out1 = (R*)a.out1;
   t.N = a.N; t.n = a.n; t.shift = a.shift; t.ntiers = a.ntiers; t.k = round_consts<R>(a.consts);
+  t.bc = a.bc;
   const size_t smem = tier_smem_bytes<Prob>(a.n);
   auto kern = swept_tier_kernel<Prob, P, KIND>;
   if (smem > 48 * 1024) {
@@ -103,6 +104,7 @@ inline int char_go(const TileLaunch& a) {
   TierArgs<R> t;
   t.in0 = (const R*)a.in0; t.in1 = (const R*)a.in1; t.out0 = (R*)a.out0; t.out1 = (R*)a.out1;
   t.N = a.N; t.n = a.n; t.shift = a.shift; t.ntiers = a.ntiers; t.k = round_consts<R>(a.consts);
+  t.bc = 0;
   const size_t smem = char_smem_bytes<Prob>(T, B);
   auto kern = swept_char_kernel<Prob, B, L, KIND>;
   if (smem > 48 * 1024) {

@@ -56,7 +56,7 @@ struct GraphKey {
 }  // namespace
 
 struct swept_state {
-  int problem = 0, dtype = 0, rk2 = 0, device = 0;
+  int problem = 0, dtype = 0, rk2 = 0, device = 0, bc = 0;
   int64_t N = 0;
   double dx = 0, dt = 0, alpha = 1, gamma = 1.4;
   double consts[5] = {0, 0, 0, 0, 0};
@@ -97,7 +97,7 @@ int set_device(const swept_state* s) {
 }
 
 int launch_per_step(swept_state* s, const void* in, const void* base, void* out, int odd, int threads, int P) {
-  swept::PerStepLaunch a{in, base, out, s->N, odd, threads, P, s->consts, s->stream};
+  swept::PerStepLaunch a{in, base, out, s->N, odd, threads, P, s->consts, s->stream, s->bc};
   int rc;
   switch (s->problem) {
     case SWEPT_HEAT: rc = swept::launch_per_step_heat(s->dtype, a); break;
@@ -113,6 +113,7 @@ int launch_tile(swept_state* s, swept::TileLaunch& a) {
   a.N = s->N;
   a.consts = s->consts;
   a.stream = s->stream;
+  a.bc = s->bc;
   int rc;
   switch (s->problem) {
     case SWEPT_HEAT: rc = swept::launch_tile_heat(s->dtype, a); break;
@@ -207,6 +208,7 @@ struct TimedScope {
 
 bool tile_ok(const swept_state* s, int flavor, int n, int P) {
   if (n <= 0 || s->N % n != 0) return false;
+  if (s->bc && flavor != SWEPT_FLAVOR_TIER) return false;  // walls are applied by the TIER flavour only
   if (flavor == SWEPT_FLAVOR_FLOW && (s->problem == SWEPT_EULER || P < 0 || P > 16)) return false;
   switch (s->problem) {
     case SWEPT_HEAT: return swept::tile_config_ok_heat(s->dtype, flavor, s->N, n, P);
@@ -292,6 +294,7 @@ int run_per_step(swept_state* s, int64_t steps, int threads) {
 // ---- resident per-step: every sub-timestep in one persistent launch (per_step_resident.cuh) -----------
 int run_resident(swept_state* s, int64_t steps) {
   if (steps <= 0) return 0;
+  if (s->bc) return fail(SWEPT_EUNSUPPORTED, "the resident per-step flavour is periodic only");
   if (!s->resident_scratch) {
     CUDA_TRY(cudaMalloc(&s->resident_scratch, swept::resident_scratch_bytes(swept::RESIDENT_MAX_CTAS)));
     CUDA_TRY(cudaMemsetAsync(s->resident_scratch, 0, swept::resident_flag_bytes(swept::RESIDENT_MAX_CTAS), s->stream));
@@ -363,7 +366,8 @@ void default_tile(const swept_state* s, int* n_io, int* flavor_io, int* P_io) {
   }
   // untuned defaults (measured on B200): heat and KS run fastest with the register-resident
   // CHAR flavour on wide tiles, Euler (about 250 live registers per point) with the TIER flavour
-  const bool want_char = flavor == SWEPT_FLAVOR_CHAR || (flavor == SWEPT_FLAVOR_AUTO && s->problem != SWEPT_EULER);
+  const bool want_char = flavor == SWEPT_FLAVOR_CHAR ||
+                         (flavor == SWEPT_FLAVOR_AUTO && s->problem != SWEPT_EULER && !s->bc);
   if (n == 0) {
     if (want_char) {
       for (int cand : {1024, 512, 256, 128, 64})
@@ -553,6 +557,11 @@ swept_state* swept_create(int problem, int64_t N, double dx, double dt, const sw
     fail(SWEPT_EUNSUPPORTED, "FP32 is provided for the heat problem only (BASELINE.json config 2)");
     return nullptr;
   }
+  if (q.bc != SWEPT_BC_PERIODIC && q.bc != SWEPT_BC_PAPER) { fail(SWEPT_EINVAL, "bad bc"); return nullptr; }
+  if (q.bc == SWEPT_BC_PAPER && problem != SWEPT_HEAT) {
+    fail(SWEPT_EUNSUPPORTED, "SWEPT_BC_PAPER is built for the heat problem only (insulated ends, Eq. B.5)");
+    return nullptr;
+  }
   if ((q.alloc == nullptr) != (q.free == nullptr)) { fail(SWEPT_EINVAL, "alloc and free must be given together"); return nullptr; }
   int dev = q.device;
   if (dev < 0) {
@@ -564,7 +573,7 @@ swept_state* swept_create(int problem, int64_t N, double dx, double dt, const sw
     if (e != cudaSuccess) { fail(SWEPT_ECUDA, "cudaSetDevice(%d): %s (no CPU fallback exists)", dev, cudaGetErrorString(e)); return nullptr; }
   }
   swept_state* s = new swept_state();
-  s->problem = problem; s->dtype = q.dtype; s->rk2 = q.rk2; s->device = dev;
+  s->problem = problem; s->dtype = q.dtype; s->rk2 = q.rk2; s->device = dev; s->bc = q.bc;
   s->N = N; s->dx = dx; s->dt = dt; s->alpha = q.alpha; s->gamma = q.gamma;
   s->stream = (cudaStream_t)q.stream;
   s->alloc = q.alloc; s->free_ = q.free; s->alloc_ctx = q.alloc_ctx;

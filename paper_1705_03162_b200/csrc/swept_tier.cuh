@@ -37,6 +37,7 @@ struct TierArgs {
   int n;       // tile width in points
   int shift;   // 0 or n/2
   int ntiers;  // tiers to compute
+  int bc;      // 0 periodic; 1 insulated ends (heat, Eq. (B.5)): T_{-k} = T_k, T_{N-1+k} = T_{N-1-k}
   Consts<R> k;
 };
 
@@ -58,7 +59,7 @@ __global__ void __launch_bounds__(Prob::MAX_THREADS) swept_tier_kernel(const Tie
   constexpr int H = Prob::H, C = Prob::C, PAD = Pad16<R>::value;
   extern __shared__ __align__(128) unsigned char smem_raw[];
   const int n = a.n;
-  const int RS = n + 2 * PAD;  // padded row stride: body starts 16 bytes in
+  const int RS = n + 4 * PAD;  // padded row stride: body starts 16 bytes in; room for the wall gap (see below)
   R* rows = reinterpret_cast<R*>(smem_raw);
   uint64_t* mbar = reinterpret_cast<uint64_t*>(smem_raw + (size_t)2 * C * RS * sizeof(R));
   const int64_t N = a.N;
@@ -68,6 +69,16 @@ __global__ void __launch_bounds__(Prob::MAX_THREADS) swept_tier_kernel(const Tie
   const int len1 = (int)((N - S) < (int64_t)n ? (N - S) : (int64_t)n);  // part before the periodic wrap
   const int len2 = n - len1;
   constexpr int NROWS_IN = (KIND == KIND_UP) ? 1 : 2;
+  // Non-periodic ends ("node 0 is split across the spatial boundary and must apply the boundary conditions at its
+  // center"): the tile that wraps holds the last n/2 and the first n/2 points of the domain with the
+  // two walls between them.  Its halves are staged 2*PAD slots apart and the gap holds each wall's h ghost values;
+  // tiles that end at a wall keep the ghosts in their halo slots.  A ghost is the mirror image of a point the tile
+  // itself updates, so whoever writes a point within h of a wall also writes its image (no extra barrier).
+  const bool bcm = a.bc != 0;
+  const int GAP = (bcm && len2 > 0) ? 2 * PAD : 0;
+  const int jl = !bcm ? -100000 : (len2 > 0 ? len1 : (S == 0 ? 0 : -100000));              // local index of point 0
+  const int jr = !bcm ? -100000 : (len2 > 0 ? len1 - 1 : (S + n == N ? n - 1 : -100000));  // ... of point N-1
+  auto slot_of = [&](int j) -> int { return PAD + j + (j >= len1 ? GAP : 0); };
 
   if (tid == 0) {
     mbar_init(mbar, 1);
@@ -83,7 +94,7 @@ __global__ void __launch_bounds__(Prob::MAX_THREADS) swept_tier_kernel(const Tie
       for (int c = 0; c < C; ++c) {
         R* dst = rows + (r * C + c) * RS + PAD;
         bulk_g2s(dst, src + (int64_t)c * N + S, (uint32_t)(len1 * sizeof(R)), mbar);
-        if (len2 > 0) bulk_g2s(dst + len1, src + (int64_t)c * N, (uint32_t)(len2 * sizeof(R)), mbar);
+        if (len2 > 0) bulk_g2s(dst + len1 + GAP, src + (int64_t)c * N, (uint32_t)(len2 * sizeof(R)), mbar);
       }
     }
   }
@@ -91,15 +102,25 @@ __global__ void __launch_bounds__(Prob::MAX_THREADS) swept_tier_kernel(const Tie
     // tier -1 does not exist: give row1 a defined value (its edge slots are stored but never used)
     for (int i = tid; i < C * RS; i += blockDim.x) rows[C * RS + i] = (R)0;
   } else {
-    // halo: H points either side of the tile, both rows, plain loads (periodic)
+    // halo: H points either side of the tile, both rows, plain loads (periodic, or mirrored at a wall)
     for (int i = tid; i < 2 * C * 2 * H; i += blockDim.x) {
       const int r = i / (C * 2 * H), c = (i / (2 * H)) % C, j = i % (2 * H);
       const R* src = (r == 0 ? a.in0 : a.in1) + (int64_t)c * N;
       int64_t g = (j < H) ? (S - H + j) : (S + n + (j - H));
-      if (g < 0) g += N;
-      if (g >= N) g -= N;
-      const int s = (j < H) ? (PAD - H + j) : (PAD + n + (j - H));
+      if (len2 > 0 && j >= H) g = len2 + (j - H);  // the wrapping tile continues at point n/2 (no wall there)
+      if (g < 0) g = bcm ? -g : g + N;
+      if (g >= N) g = bcm ? 2 * (N - 1) - g : g - N;
+      const int s = (j < H) ? (PAD - H + j) : (PAD + n + GAP + (j - H));
       rows[(r * C + c) * RS + s] = src[g];
+    }
+    if (GAP > 0) {  // ghosts of the two walls inside the wrapping tile: T_{N-1+k} = T_{N-1-k}, T_{-k} = T_k
+      for (int i = tid; i < 2 * C * 2 * H; i += blockDim.x) {
+        const int r = i / (C * 2 * H), c = (i / (2 * H)) % C, j = i % (2 * H);
+        const R* src = (r == 0 ? a.in0 : a.in1) + (int64_t)c * N;
+        const int k = (j < H) ? j + 1 : j - H + 1;
+        const int s = (j < H) ? slot_of(jr) + k : slot_of(jl) - k;
+        rows[(r * C + c) * RS + s] = (j < H) ? src[N - 1 - k] : src[k];
+      }
     }
   }
   mbar_wait(mbar, 0);
@@ -107,10 +128,11 @@ __global__ void __launch_bounds__(Prob::MAX_THREADS) swept_tier_kernel(const Tie
 
   const int m = n / (2 * H);
   const int j0 = tid * P;
+  const int sb = slot_of(j0);  // a thread's P points lie on one side of the wrap (n/2 is a multiple of P)
   for (int t = 1; t <= a.ntiers; ++t) {
     const int par = t & 1;  // phases start on even global tiers (m is even): odd = predictor
-    const R* src = rows + (1 - par) * C * RS + PAD;
-    R* dst = rows + par * C * RS + PAD;
+    const R* src = rows + (1 - par) * C * RS;
+    R* dst = rows + par * C * RS;
     int lo, hi;
     tier_range<KIND>(t, n, H, m, lo, hi);
     if (j0 < hi && j0 + P > lo) {
@@ -118,18 +140,29 @@ __global__ void __launch_bounds__(Prob::MAX_THREADS) swept_tier_kernel(const Tie
 #pragma unroll
       for (int c = 0; c < C; ++c)
 #pragma unroll
-        for (int q = 0; q < P + 2 * H; ++q) win[c][q] = src[c * RS + j0 - H + q];
+        for (int q = 0; q < P + 2 * H; ++q) win[c][q] = src[c * RS + sb - H + q];
 #pragma unroll
       for (int c = 0; c < C; ++c)
 #pragma unroll
         for (int j = 0; j < P; ++j)
-          bs[c][j] = (Prob::SIGMA == 2 && !par) ? dst[c * RS + j0 + j] : win[c][H + j];
+          bs[c][j] = (Prob::SIGMA == 2 && !par) ? dst[c * RS + sb + j] : win[c][H + j];
       Prob::template stage<P>(win, bs, o, par, a.k);
 #pragma unroll
       for (int j = 0; j < P; ++j)
         if (j0 + j >= lo && j0 + j < hi) {
 #pragma unroll
-          for (int c = 0; c < C; ++c) dst[c * RS + j0 + j] = o[c][j];
+          for (int c = 0; c < C; ++c) dst[c * RS + sb + j] = o[c][j];
+          if (bcm) {
+            const int dl = j0 + j - jl, dr = jr - (j0 + j);
+            if (dl > 0 && dl <= H) {
+#pragma unroll
+              for (int c = 0; c < C; ++c) dst[c * RS + slot_of(jl) - dl] = o[c][j];
+            }
+            if (dr > 0 && dr <= H) {
+#pragma unroll
+              for (int c = 0; c < C; ++c) dst[c * RS + slot_of(jr) + dr] = o[c][j];
+            }
+          }
         }
     }
     __syncthreads();
@@ -146,7 +179,7 @@ __global__ void __launch_bounds__(Prob::MAX_THREADS) swept_tier_kernel(const Tie
       for (int c = 0; c < C; ++c) {
         const R* s = rows + (r * C + c) * RS + PAD;
         bulk_s2g(dstg + (int64_t)c * N + S, s, (uint32_t)(len1 * sizeof(R)));
-        if (len2 > 0) bulk_s2g(dstg + (int64_t)c * N, s + len1, (uint32_t)(len2 * sizeof(R)));
+        if (len2 > 0) bulk_s2g(dstg + (int64_t)c * N, s + len1 + GAP, (uint32_t)(len2 * sizeof(R)));
       }
     }
     bulk_commit();
@@ -157,7 +190,7 @@ __global__ void __launch_bounds__(Prob::MAX_THREADS) swept_tier_kernel(const Tie
 template <class Prob>
 inline size_t tier_smem_bytes(int n) {
   using R = typename Prob::R;
-  return (size_t)2 * Prob::C * (n + 2 * Pad16<R>::value) * sizeof(R) + 16;
+  return (size_t)2 * Prob::C * (n + 4 * Pad16<R>::value) * sizeof(R) + 16;
 }
 
 }  // namespace swept

@@ -26,8 +26,8 @@ def test_every_declared_symbol_is_exported():
 
 
 def test_params_struct_matches_header():
-    # 4 x 4-byte + 2 doubles + 4 pointers
-    assert ctypes.sizeof(sw.swept_params) == 16 + 16 + 32
+    # 4 x 4-byte + 2 doubles + 4 pointers + 2 x 4-byte
+    assert ctypes.sizeof(sw.swept_params) == 16 + 16 + 32 + 8
     assert ctypes.sizeof(sw.swept_phase) == 32  # 2 x int32, 2 x int64, 2 x int32
 
 

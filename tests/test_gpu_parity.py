@@ -167,6 +167,43 @@ def test_per_step_resident_matches_oracle():
     s.close()
 
 
+def test_heat_insulated_ends_bc_paper():
+    # the paper's own heat boundary condition (B.5): per-step and swept (TIER flavour; the tile split across the
+    # boundary applies the walls at its centre) against the oracle, bit for bit
+    for N, steps in ((64, 100), (256, 333), (1024, 1500), (4096, 700)):
+        w = si.heat_insulated(N, 6, 31, steps)
+        ref = oracle.run_workload(w)
+        ps, _ = gpu_run(w, steps, sw.PER_STEP)
+        assert np.array_equal(ps, ref), ("per_step", N)
+        for n in (32, 64, 256, 1024):
+            if N % n:
+                continue
+            for P in (1, 2, 4):
+                try:
+                    sx, _ = gpu_run(w, steps, sw.SWEPT, n, sw.FLAVOR_TIER, P)
+                except sw.SweptError as e:
+                    assert "not admissible" in str(e)
+                    continue
+                assert np.array_equal(sx, ref), ("swept", N, n, P)
+        sx, _ = gpu_run(w, steps, sw.SWEPT)          # library default: must pick an admissible (TIER) configuration
+        assert np.array_equal(sx, ref)
+    w = si.heat_insulated(2048, 4, 32, 300)
+    assert np.array_equal(gpu_run(w, 300, sw.SWEPT, 128, dtype=np.float32)[0],
+                          oracle.run_workload(w, dtype=np.float32))
+    s = sw.Swept.from_workload(w)
+    for fl in (sw.FLAVOR_CHAR, sw.FLAVOR_FLOW):      # register flavours are periodic only: clean error
+        with pytest.raises(sw.SweptError):
+            s.run(10, 256, sw.SWEPT, fl)
+    with pytest.raises(sw.SweptError):
+        s.run(10, 0, sw.PER_STEP, sw.PS_RESIDENT)
+    best = s.autotune(sw.SWEPT)
+    s.run(300, 0, sw.SWEPT)
+    assert np.array_equal(s.read(), oracle.run_workload(w)) and best >= 32
+    s.close()
+    with pytest.raises(sw.SweptError):
+        sw.swept_create(sw.KS, 4096, 0.5, 0.005, bc=sw.BC_PAPER)
+
+
 def test_per_step_non_power_of_two_N():
     # the paper's `& lastidx` wrap needs N = 2^k; ours does not
     for N in (1000, 1001, 1002):
