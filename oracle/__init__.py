@@ -52,6 +52,7 @@ def _load():
         lib.oracle_heat_f32.argtypes = [vp, i64, i64, dbl, dbl, dbl]
         lib.oracle_heat_bc_f64.argtypes = [vp, i64, i64, dbl, dbl, dbl, ci]
         lib.oracle_heat_bc_f32.argtypes = [vp, i64, i64, dbl, dbl, dbl, ci]
+        lib.oracle_euler_bc_f64.argtypes = [vp, i64, i64, dbl, dbl, dbl, ci]
         lib.oracle_ks_f64.argtypes = [vp, i64, i64, dbl, dbl, ci]
         lib.oracle_ks_f32.argtypes = [vp, i64, i64, dbl, dbl, ci]
         lib.oracle_euler_f64.argtypes = [vp, i64, i64, dbl, dbl, dbl, ci]
@@ -77,7 +78,8 @@ def run(problem: int, u0: np.ndarray, N: int, nsteps: int, dx: float, dt: float,
 
     ``dtype`` float64 or float32 selects the arithmetic type of the whole computation (reading X15: the
     FP32 GPU path is gated against the FP32 instantiation of these same expression trees).
-    ``bc``: 0 periodic (the configs), 1 the paper's insulated ends for heat, Eq. (B.5) PAPER.md:328-331.
+    ``bc``: 0 periodic (the configs), 1 the paper's own ends: insulated for heat, Eq. (B.5) PAPER.md:328-331;
+    Dirichlet (the initial end states) for the Euler tube.
     """
     lib = _load()
     dtype = np.dtype(dtype)
@@ -87,15 +89,16 @@ def run(problem: int, u0: np.ndarray, N: int, nsteps: int, dx: float, dt: float,
         raise ValueError(f"expected {C * N} values, got {u.size}")
     sfx = "f64" if dtype == np.float64 else "f32"
     ptr = u.ctypes.data_as(ctypes.c_void_p)
-    if bc and problem != HEAT:
-        raise ValueError("boundary conditions other than periodic exist for the heat problem only (B.5)")
+    if bc and (problem == KS or (problem == EULER and dtype != np.float64)):
+        raise ValueError("non-periodic ends exist for heat (B.5) and FP64 Euler (PAPER.md:377) only")
     if problem == HEAT:
         rc = getattr(lib, "oracle_heat_bc_" + sfx)(ptr, N, nsteps, dx, dt, alpha, bc) if bc else \
             getattr(lib, "oracle_heat_" + sfx)(ptr, N, nsteps, dx, dt, alpha)
     elif problem == KS:
         rc = getattr(lib, "oracle_ks_" + sfx)(ptr, N, nsteps, dx, dt, rk2)
     elif problem == EULER:
-        rc = getattr(lib, "oracle_euler_" + sfx)(ptr, N, nsteps, dx, dt, gamma, rk2)
+        rc = lib.oracle_euler_bc_f64(ptr, N, nsteps, dx, dt, gamma, rk2) if bc else \
+            getattr(lib, "oracle_euler_" + sfx)(ptr, N, nsteps, dx, dt, gamma, rk2)
     else:
         raise ValueError("unknown problem")
     if rc != 0:

@@ -30,7 +30,8 @@
 //   X10 periodic boundaries for all three problems (BASELINE.json configs); the paper's own heat
 //       boundary condition, insulated ends (B.5) PAPER.md:328-331, is available as bc = 1:
 //       T_{-1} = T_1 and T_N = T_{N-2} for points 0..N-1 (mirror about the end POINTS; the paper's
-//       index "n+1" is read with points 0..n).
+//       index "n+1" is read with points 0..n).  Euler: Dirichlet ends, bc = 1: ghost cells
+//       -2, -1 / N, N+1 hold the initial state of the first / last cell at every stage.
 //
 // Floating point: every expression below is a fixed tree of IEEE-754 operations.  Build with
 // -ffp-contract=off so the compiler never fuses a*b+c on its own; the fused operations that ARE
@@ -225,6 +226,55 @@ void euler_stage(const R* V, const R* base, R* out, int64_t N, R hs, const Euler
     }
 }
 
+// Dirichlet ends ("The spatial boundary conditions are these values at their respective ends of
+// the tube"): cells -2, -1 hold the initial state of cell 0 and cells N, N+1 that of cell N-1, at every stage.
+// Implemented by running the very same euler_stage on arrays padded with those four ghost cells and made
+// "periodic" over N+4 cells: the wrap-around then only ever couples ghost cells with each other (a ghost's
+// update is discarded and the ghosts are re-imposed before every stage), and every interior cell j reads exactly
+// cells j-2..j+2 of the padded array.
+template <class R>
+void euler_run_dirichlet(R* q, int64_t N, int64_t nsteps, double dx, double dt, double gamma, int rk2) {
+    EulerConst<R> c;
+    c.gm1 = (R)(gamma - 1.0);
+    c.ggm1 = (R)(gamma * (gamma - 1.0));
+    const double lam_d = dt / dx;
+    const R lam = (R)lam_d, half_lam = (R)(0.5 * lam_d);
+    const int64_t M = N + 4;
+    const size_t m3 = (size_t)(3 * M);
+    std::vector<R> qa(m3), qs(m3), qn(m3), P((size_t)M), F(m3);
+    R left[3], right[3];
+    for (int cpt = 0; cpt < 3; ++cpt) {
+        left[cpt] = q[cpt * N];
+        right[cpt] = q[cpt * N + N - 1];
+        for (int64_t j = 0; j < N; ++j) qa[(size_t)(cpt * M + 2 + j)] = q[cpt * N + j];
+    }
+    auto impose = [&](R* v) {
+        for (int cpt = 0; cpt < 3; ++cpt) {
+            v[cpt * M + 0] = v[cpt * M + 1] = left[cpt];
+            v[cpt * M + M - 2] = v[cpt * M + M - 1] = right[cpt];
+        }
+    };
+    R* a = qa.data();
+    R* b = qn.data();
+    R* p = qs.data();
+    for (int64_t s = 0; s < nsteps; ++s) {
+        impose(a);
+        if (rk2 == 0) {
+            euler_stage(a, a, p, M, half_lam, c, P, F);
+            impose(p);
+            euler_stage(p, a, b, M, lam, c, P, F);
+        } else {
+            euler_stage(a, a, p, M, lam, c, P, F);
+            impose(p);
+            euler_stage(p, p, b, M, lam, c, P, F);
+            for (int64_t j = 0; j < (int64_t)m3; ++j) b[j] = (R)0.5 * (a[j] + b[j]);
+        }
+        R* tmp = a; a = b; b = tmp;
+    }
+    for (int cpt = 0; cpt < 3; ++cpt)
+        for (int64_t j = 0; j < N; ++j) q[cpt * N + j] = a[(size_t)(cpt * M + 2 + j)];
+}
+
 template <class R>
 void euler_run(R* q, int64_t N, int64_t nsteps, double dx, double dt, double gamma, int rk2) {
     EulerConst<R> c;
@@ -298,6 +348,12 @@ int oracle_euler_f32(float* q, int64_t N, int64_t nsteps, double dx, double dt, 
                      int rk2) {
     if (!q || N < 5 || nsteps < 0) return -1;
     euler_run<float>(q, N, nsteps, dx, dt, gamma, rk2);
+    return 0;
+}
+// Euler with Dirichlet ends = the initial states of the first and last cell
+int oracle_euler_bc_f64(double* q, int64_t N, int64_t nsteps, double dx, double dt, double gamma, int rk2) {
+    if (!q || N < 5 || nsteps < 0) return -1;
+    euler_run_dirichlet<double>(q, N, nsteps, dx, dt, gamma, rk2);
     return 0;
 }
 int oracle_num_threads(void) {

@@ -115,6 +115,20 @@ def euler_double_sod(N: int, nsteps: int, rk2: int = RK2_HEUN, gamma: float = 1.
     return Workload(EULER, N, dx, dt, nsteps, u0, gamma=gamma, rk2=rk2, name=name or f"euler_N{N}")
 
 
+def euler_sod(N: int, nsteps: int, rk2: int = RK2_MIDPOINT, gamma: float = 1.4, cfl: float = 0.4,
+              lam_ref: float = 2.2, name: str = "") -> Workload:
+    """The paper's own Sod tube (readings X8, X11): one diaphragm at N/2, (rho, u, p) = (1, 0, 1) left
+    and (0.125, 0, 0.1) right, Dirichlet ends (bc = BC_PAPER), midpoint RK2."""
+    j = np.arange(N)
+    lft = j < N // 2
+    rho = np.where(lft, 1.0, 0.125)
+    p = np.where(lft, 1.0, 0.1)
+    u0 = np.concatenate([rho, np.zeros(N), p / (gamma - 1.0)]).astype(np.float64)
+    dx = 1.0 / N
+    return Workload(EULER, N, dx, cfl * dx / lam_ref, nsteps, u0, gamma=gamma, rk2=rk2,
+                    name=name or f"euler_sod_N{N}", bc=BC_PAPER)
+
+
 def config(k: int, N: int | None = None, nsteps: int | None = None, problem: int | None = None,
            rk2: int | None = None) -> Workload:
     """BASELINE.json config k (1-based, as numbered in SURVEY.md §8(d)); N / nsteps may be overridden
