@@ -44,9 +44,11 @@ enum { SWEPT_F64 = 0, SWEPT_F32 = 1 };                      /* dtype            
 enum { SWEPT_RK2_MIDPOINT = 0, SWEPT_RK2_HEUN = 1 };        /* KS/Euler integrator (
                                                                Heun is BASELINE.json config 4)   */
 /* boundary conditions: periodic (all BASELINE.json configs) or the paper's own: insulated ends for heat,
- * Eq. (B.5), T_{-1} = T_1 and T_N = T_{N-2} for points 0..N-1.  SWEPT_BC_PAPER is built for
- * the heat problem, per-step (launch per sub-timestep) and swept TIER flavour, where the tile split across
- * the boundary applies the condition at its centre; other combinations: SWEPT_EUNSUPPORTED. */
+ * Eq. (B.5), T_{-1} = T_1 and T_N = T_{N-2} for points 0..N-1; Dirichlet ends for the Euler
+ * tube: cells -2, -1 and N, N+1 hold the states that swept_write found in the first and last
+ * cell.  SWEPT_BC_PAPER is built for per-step (launch per sub-timestep) and the swept TIER flavour, where the
+ * tile split across the boundary applies the condition at its centre; KS (periodic in the
+ * paper) and the other flavours: SWEPT_EUNSUPPORTED. */
 enum { SWEPT_BC_PERIODIC = 0, SWEPT_BC_PAPER = 1 };
 enum { SWEPT_NKINDS = 6 };                                   /* phase kinds reported by swept_phase_times */
 enum { SWEPT_OK = 0, SWEPT_EINVAL = -1, SWEPT_EUNSUPPORTED = -2, SWEPT_ECUDA = -3, SWEPT_ENOMEM = -4 };

@@ -35,6 +35,15 @@ struct Consts {
   R a0, a1, a2, a3, a4;  // meaning per problem, see each functor
 };
 
+// Boundary treatment handed to the kernels (include/swept.h SWEPT_BC_*): 0 periodic; 1 mirror about the end points
+// (insulated heat ends, Eq. (B.5)); 2 Dirichlet: ghost cells hold the end states l / r at every
+// stage (Euler tube).
+enum { BC_WRAP = 0, BC_MIRROR = 1, BC_FIXED = 2 };
+template <class R>
+struct BcVals {
+  R l[3], r[3];
+};
+
 // ---------------------------------------------------------------------------------------------
 // Heat, FTCS, Eq. (B.4):  T_i^{m+1} = Fo (T_{i+1} + T_{i-1}) + (1 - 2 Fo) T_i
 //   a0 = Fo = alpha dt / dx^2,  a1 = 1 - 2 Fo

@@ -15,7 +15,8 @@ struct PerStepLaunch {
   int P;        // points per thread (N % P == 0)
   const double* consts;  // 5 doubles, rounded once to REAL by the launcher
   cudaStream_t stream;
-  int bc = 0;   // 0 periodic, 1 insulated ends (heat only)
+  int bc = 0;   // kernel boundary mode: 0 wrap, 1 mirror (heat B.5), 2 fixed end states (Euler tube)
+  const double* bcv = nullptr;  // bc == 2: left[3], right[3] end states
 };
 
 struct TileLaunch {
@@ -30,7 +31,8 @@ struct TileLaunch {
   int flavor;  // SWEPT_FLAVOR_TIER / SWEPT_FLAVOR_CHAR
   const double* consts;
   cudaStream_t stream;
-  int bc = 0;  // 0 periodic, 1 insulated ends (heat, TIER flavour only)
+  int bc = 0;  // kernel boundary mode (TIER flavour only): 0 wrap, 1 mirror, 2 fixed end states
+  const double* bcv = nullptr;
 };
 
 // FLOW flavour: one whole Up / diamonds / Down cycle of tile width n in a single persistent launch

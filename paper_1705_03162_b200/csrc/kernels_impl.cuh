@@ -17,6 +17,16 @@ inline Consts<R> round_consts(const double* c) {
   return k;
 }
 
+template <class R>
+inline BcVals<R> round_bcvals(const double* v) {
+  BcVals<R> b;
+  for (int c = 0; c < 3; ++c) {
+    b.l[c] = v ? (R)v[c] : (R)0;
+    b.r[c] = v ? (R)v[3 + c] : (R)0;
+  }
+  return b;
+}
+
 template <class Prob, int P>
 inline int per_step_go(const PerStepLaunch& a) {
   using R = typename Prob::R;
@@ -24,7 +34,8 @@ inline int per_step_go(const PerStepLaunch& a) {
   const int threads = a.threads < Prob::MAX_THREADS ? a.threads : Prob::MAX_THREADS;
   const unsigned grid = (unsigned)((nthreads + threads - 1) / threads);
   per_step_kernel<Prob, P><<<grid, threads, 0, a.stream>>>((const R*)a.in, (const R*)a.base, (R*)a.out,
-                                                             a.N, a.odd, round_consts<R>(a.consts), a.bc);
+                                                             a.N, a.odd, round_consts<R>(a.consts), a.bc,
+                                                             round_bcvals<R>(a.bcv));
   return (int)cudaGetLastError();
 }
 
@@ -46,6 +57,7 @@ inline int tier_go(const TileLaunch& a) {
   t.in0 = (const R*)a.in0; t.in1 = (const R*)a.in1; t.out0 = (R*)a.out0; t.out1 = (R*)a.out1;
   t.N = a.N; t.n = a.n; t.shift = a.shift; t.ntiers = a.ntiers; t.k = round_consts<R>(a.consts);
   t.bc = a.bc;
+  t.bv = round_bcvals<R>(a.bcv);
   const size_t smem = tier_smem_bytes<Prob>(a.n);
   auto kern = swept_tier_kernel<Prob, P, KIND>;
   if (smem > 48 * 1024) {
@@ -105,6 +117,7 @@ inline int char_go(const TileLaunch& a) {
   t.in0 = (const R*)a.in0; t.in1 = (const R*)a.in1; t.out0 = (R*)a.out0; t.out1 = (R*)a.out1;
   t.N = a.N; t.n = a.n; t.shift = a.shift; t.ntiers = a.ntiers; t.k = round_consts<R>(a.consts);
   t.bc = 0;
+  t.bv = round_bcvals<R>(nullptr);
   const size_t smem = char_smem_bytes<Prob>(T, B);
   auto kern = swept_char_kernel<Prob, B, L, KIND>;
   if (smem > 48 * 1024) {

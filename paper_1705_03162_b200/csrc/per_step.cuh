@@ -42,7 +42,7 @@ __device__ __forceinline__ void store_vec(R* __restrict__ p, const R (&v)[P]) {
 template <class Prob, int P>
 __global__ void __launch_bounds__(Prob::MAX_THREADS)
 per_step_kernel(const typename Prob::R* __restrict__ in, const typename Prob::R* __restrict__ base,
-                typename Prob::R* __restrict__ out, int64_t N, int odd, Consts<typename Prob::R> k, int bc) {
+                typename Prob::R* __restrict__ out, int64_t N, int odd, Consts<typename Prob::R> k, int bc, BcVals<typename Prob::R> bv) {
   using R = typename Prob::R;
   constexpr int H = Prob::H, C = Prob::C;
   const int64_t i0 = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) * P;
@@ -60,11 +60,13 @@ per_step_kernel(const typename Prob::R* __restrict__ in, const typename Prob::R*
 #pragma unroll
     for (int j = 0; j < H; ++j) {
       int64_t il = i0 - H + j;
-      if (il < 0) il = bc ? -il : il + N;  // bc: insulated ends, T_{-k} = T_k, T_{N-1+k} = T_{N-1-k} (B.5)
+      const bool fix_l = bc == BC_FIXED && il < 0;       // Dirichlet ghost cells
+      if (il < 0) il = bc ? -il : il + N;                // mirror: T_{-k} = T_k, T_{N-1+k} = T_{N-1-k} (B.5)
       int64_t ir = i0 + P + j;
+      const bool fix_r = bc == BC_FIXED && ir >= N;
       if (ir >= N) ir = bc ? 2 * (N - 1) - ir : ir - N;
-      win[c][j] = __ldg(src + il);
-      win[c][H + P + j] = __ldg(src + ir);
+      win[c][j] = fix_l ? bv.l[c] : __ldg(src + il);
+      win[c][H + P + j] = fix_r ? bv.r[c] : __ldg(src + ir);
     }
   }
   if (Prob::SIGMA == 2 && !odd) {

@@ -60,6 +60,8 @@ struct swept_state {
   int64_t N = 0;
   double dx = 0, dt = 0, alpha = 1, gamma = 1.4;
   double consts[5] = {0, 0, 0, 0, 0};
+  double bcvals[6] = {0, 0, 0, 0, 0, 0};  // Dirichlet end states (Euler tube): left[3], right[3], set by swept_write
+  int kernel_bc() const { return bc == 0 ? 0 : (problem == SWEPT_HEAT ? 1 : 2); }
   cudaStream_t stream = nullptr;
   cudaStream_t capture_stream = nullptr;  // graphs are recorded here (the legacy default stream cannot capture)
   swept_alloc_fn alloc = nullptr;
@@ -97,7 +99,7 @@ int set_device(const swept_state* s) {
 }
 
 int launch_per_step(swept_state* s, const void* in, const void* base, void* out, int odd, int threads, int P) {
-  swept::PerStepLaunch a{in, base, out, s->N, odd, threads, P, s->consts, s->stream, s->bc};
+  swept::PerStepLaunch a{in, base, out, s->N, odd, threads, P, s->consts, s->stream, s->kernel_bc(), s->bcvals};
   int rc;
   switch (s->problem) {
     case SWEPT_HEAT: rc = swept::launch_per_step_heat(s->dtype, a); break;
@@ -113,7 +115,8 @@ int launch_tile(swept_state* s, swept::TileLaunch& a) {
   a.N = s->N;
   a.consts = s->consts;
   a.stream = s->stream;
-  a.bc = s->bc;
+  a.bc = s->kernel_bc();
+  a.bcv = s->bcvals;
   int rc;
   switch (s->problem) {
     case SWEPT_HEAT: rc = swept::launch_tile_heat(s->dtype, a); break;
@@ -558,8 +561,8 @@ swept_state* swept_create(int problem, int64_t N, double dx, double dt, const sw
     return nullptr;
   }
   if (q.bc != SWEPT_BC_PERIODIC && q.bc != SWEPT_BC_PAPER) { fail(SWEPT_EINVAL, "bad bc"); return nullptr; }
-  if (q.bc == SWEPT_BC_PAPER && problem != SWEPT_HEAT) {
-    fail(SWEPT_EUNSUPPORTED, "SWEPT_BC_PAPER is built for the heat problem only (insulated ends, Eq. B.5)");
+  if (q.bc == SWEPT_BC_PAPER && problem == SWEPT_KS) {
+    fail(SWEPT_EUNSUPPORTED, "SWEPT_BC_PAPER: the paper's KS runs are periodic (PAPER.md:356); heat and Euler only");
     return nullptr;
   }
   if ((q.alloc == nullptr) != (q.free == nullptr)) { fail(SWEPT_EINVAL, "alloc and free must be given together"); return nullptr; }
@@ -673,6 +676,12 @@ int swept_write(swept_state* s, const void* host_buf) {
   if (!s || !host_buf) return fail(SWEPT_EINVAL, "null argument");
   if (int rc = set_device(s)) return rc;
   CUDA_TRY(cudaMemcpyAsync(s->slab[s->cur], host_buf, s->slab_bytes, cudaMemcpyHostToDevice, s->stream));
+  if (s->bc && s->problem == SWEPT_EULER) {  // Dirichlet ends = the initial states of the first and last cell
+    for (int c = 0; c < 3; ++c) {
+      s->bcvals[c] = ((const double*)host_buf)[(size_t)c * s->N];
+      s->bcvals[3 + c] = ((const double*)host_buf)[(size_t)c * s->N + s->N - 1];
+    }
+  }
   s->steps_done = 0;
   return 0;
 }
@@ -681,6 +690,13 @@ int swept_write_device(swept_state* s, const void* device_buf) {
   if (!s || !device_buf) return fail(SWEPT_EINVAL, "null argument");
   if (int rc = set_device(s)) return rc;
   CUDA_TRY(cudaMemcpyAsync(s->slab[s->cur], device_buf, s->slab_bytes, cudaMemcpyDeviceToDevice, s->stream));
+  if (s->bc && s->problem == SWEPT_EULER) {  // end states: two small synchronous copies per component
+    for (int c = 0; c < 3; ++c) {
+      const double* d = (const double*)device_buf + (size_t)c * s->N;
+      CUDA_TRY(cudaMemcpy(&s->bcvals[c], d, sizeof(double), cudaMemcpyDeviceToHost));
+      CUDA_TRY(cudaMemcpy(&s->bcvals[3 + c], d + s->N - 1, sizeof(double), cudaMemcpyDeviceToHost));
+    }
+  }
   s->steps_done = 0;
   return 0;
 }

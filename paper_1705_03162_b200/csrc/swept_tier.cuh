@@ -37,7 +37,9 @@ struct TierArgs {
   int n;       // tile width in points
   int shift;   // 0 or n/2
   int ntiers;  // tiers to compute
-  int bc;      // 0 periodic; 1 insulated ends (heat, Eq. (B.5)): T_{-k} = T_k, T_{N-1+k} = T_{N-1-k}
+  int bc;      // BC_WRAP, BC_MIRROR (heat, Eq. (B.5): T_{-k} = T_k, T_{N-1+k} = T_{N-1-k}) or
+               // BC_FIXED (Euler tube: ghost cells hold the end states bv.l / bv.r)
+  BcVals<R> bv;
   Consts<R> k;
 };
 
@@ -73,7 +75,8 @@ __global__ void __launch_bounds__(Prob::MAX_THREADS) swept_tier_kernel(const Tie
   // center"): the tile that wraps holds the last n/2 and the first n/2 points of the domain with the
   // two walls between them.  Its halves are staged 2*PAD slots apart and the gap holds each wall's h ghost values;
   // tiles that end at a wall keep the ghosts in their halo slots.  A ghost is the mirror image of a point the tile
-  // itself updates, so whoever writes a point within h of a wall also writes its image (no extra barrier).
+  // itself updates (mirror), so whoever writes a point within h of a wall also writes its image (no extra barrier);
+  // Dirichlet ghosts are constants written once.
   const bool bcm = a.bc != 0;
   const int GAP = (bcm && len2 > 0) ? 2 * PAD : 0;
   const int jl = !bcm ? -100000 : (len2 > 0 ? len1 : (S == 0 ? 0 : -100000));              // local index of point 0
@@ -108,10 +111,12 @@ __global__ void __launch_bounds__(Prob::MAX_THREADS) swept_tier_kernel(const Tie
       const R* src = (r == 0 ? a.in0 : a.in1) + (int64_t)c * N;
       int64_t g = (j < H) ? (S - H + j) : (S + n + (j - H));
       if (len2 > 0 && j >= H) g = len2 + (j - H);  // the wrapping tile continues at point n/2 (no wall there)
+      const bool fixed = a.bc == BC_FIXED && (g < 0 || g >= N);
+      const R fv = g < 0 ? a.bv.l[c] : a.bv.r[c];
       if (g < 0) g = bcm ? -g : g + N;
       if (g >= N) g = bcm ? 2 * (N - 1) - g : g - N;
       const int s = (j < H) ? (PAD - H + j) : (PAD + n + GAP + (j - H));
-      rows[(r * C + c) * RS + s] = src[g];
+      rows[(r * C + c) * RS + s] = fixed ? fv : src[g];
     }
     if (GAP > 0) {  // ghosts of the two walls inside the wrapping tile: T_{N-1+k} = T_{N-1-k}, T_{-k} = T_k
       for (int i = tid; i < 2 * C * 2 * H; i += blockDim.x) {
@@ -119,7 +124,8 @@ __global__ void __launch_bounds__(Prob::MAX_THREADS) swept_tier_kernel(const Tie
         const R* src = (r == 0 ? a.in0 : a.in1) + (int64_t)c * N;
         const int k = (j < H) ? j + 1 : j - H + 1;
         const int s = (j < H) ? slot_of(jr) + k : slot_of(jl) - k;
-        rows[(r * C + c) * RS + s] = (j < H) ? src[N - 1 - k] : src[k];
+        if (a.bc == BC_FIXED) rows[(r * C + c) * RS + s] = (j < H) ? a.bv.r[c] : a.bv.l[c];
+        else rows[(r * C + c) * RS + s] = (j < H) ? src[N - 1 - k] : src[k];
       }
     }
   }
@@ -152,7 +158,7 @@ __global__ void __launch_bounds__(Prob::MAX_THREADS) swept_tier_kernel(const Tie
         if (j0 + j >= lo && j0 + j < hi) {
 #pragma unroll
           for (int c = 0; c < C; ++c) dst[c * RS + sb + j] = o[c][j];
-          if (bcm) {
+          if (a.bc == BC_MIRROR) {
             const int dl = j0 + j - jl, dr = jr - (j0 + j);
             if (dl > 0 && dl <= H) {
 #pragma unroll

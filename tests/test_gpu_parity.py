@@ -204,6 +204,28 @@ def test_heat_insulated_ends_bc_paper():
         sw.swept_create(sw.KS, 4096, 0.5, 0.005, bc=sw.BC_PAPER)
 
 
+@pytest.mark.parametrize("rk2", [si.RK2_MIDPOINT, si.RK2_HEUN])
+def test_euler_dirichlet_ends_bc_paper(rk2):
+    # the paper's Sod tube: end states held; long enough for the waves to reach and leave the ends
+    for N, steps in ((256, 40), (512, 700), (2048, 300)):
+        w = si.euler_sod(N, steps, rk2=rk2)
+        ref = oracle.run_workload(w)
+        ps, _ = gpu_run(w, steps, sw.PER_STEP)
+        assert np.array_equal(ps, ref), ("per_step", N)
+        ran = 0
+        for n in (32, 128, 512):
+            for P in (1, 2):
+                try:
+                    sx, _ = gpu_run(w, steps, sw.SWEPT, n, sw.FLAVOR_TIER, P)
+                except sw.SweptError as e:   # n > N, or more than 256 threads for the Euler functor
+                    assert "not admissible" in str(e)
+                    continue
+                ran += 1
+                assert np.array_equal(sx, ref), ("swept", N, n, P)
+        assert ran >= 3
+        assert np.array_equal(gpu_run(w, steps, sw.SWEPT)[0], ref)
+
+
 def test_per_step_non_power_of_two_N():
     # the paper's `& lastidx` wrap needs N = 2^k; ours does not
     for N in (1000, 1001, 1002):
