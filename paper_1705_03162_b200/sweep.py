@@ -57,6 +57,8 @@ def main(argv=None):
     ap.add_argument("--dtype", default="f64", choices=["f64", "f32"])
     ap.add_argument("--steps", type=int, default=0, help="timesteps per run (0 = the config's own count)")
     ap.add_argument("--reps", type=int, default=2)
+    ap.add_argument("--bc", default="periodic", choices=["periodic", "paper"],
+                    help="paper = insulated heat ends (B.5) / Dirichlet Euler tube (PAPER.md:377); TIER flavour only")
     ap.add_argument("--csv", default="")
     args = ap.parse_args(argv)
     if not torch.cuda.is_available():
@@ -76,6 +78,8 @@ def main(argv=None):
             out.write(line + "\n")
             out.flush()
 
+    if args.bc == "paper":
+        emit("# boundary conditions: the paper's own (insulated heat ends, Dirichlet Euler tube)")
     emit("problem,dtype,N,nsteps,variant,tile_width,flavor,group,ms,updates_per_s,speedup_vs_per_step,bound,frac_of_bound")
     for pname in args.problems.split(","):
         problem = {"heat": si.HEAT, "ks": si.KS, "euler": si.EULER}[pname]
@@ -85,6 +89,11 @@ def main(argv=None):
             N = 1 << logn
             cfg = {si.HEAT: 2, si.KS: 3, si.EULER: 4}[problem]
             w = si.config(cfg, N=N) if problem != si.EULER else si.config(4, N=N, rk2=si.RK2_HEUN)
+            if args.bc == "paper":
+                if problem == si.KS:
+                    continue
+                w = si.heat_insulated(N, 16, si.BASE_SEED + 6, w.nsteps) if problem == si.HEAT else \
+                    si.euler_sod(N, w.nsteps)
             nsteps = args.steps or w.nsteps
             st = sw.Swept.from_workload(w, dtype=dtype)
             u0_dev = torch.from_numpy(np.ascontiguousarray(w.u0, dtype=dtype)).cuda()

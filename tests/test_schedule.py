@@ -122,12 +122,33 @@ def test_multi_level_remainder_g5(N, n, h, sigma, nsub):
     assert launches < nsub or nsub < 32 // (2 * h)
 
 
+def paper_values():
+    """tests/golden/paper_values.txt: the numbers the paper itself prints, each with its citation."""
+    import os
+    out = {}
+    with open(os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "paper_values.txt")) as f:
+        for line in f:
+            line = line.split("#")[0].strip()
+            if line:
+                k, v = line.split("=")
+                out[k.strip()] = int(v)
+    return out
+
+
 def test_paper_counts():
+    gold = paper_values()
     # PAPER.md:95 — the triangle of a 512-point node holds 65 792 values (incl. the initial row), h = 1
     n, h = 512, 1
     m = n // (2 * h)
     total = n + sum(active_range(UP, t, n, h)[1] - active_range(UP, t, n, h)[0] for t in range(1, m))
-    assert total == 65792
+    assert total == gold["triangle_values_n512"] == 65792
+    assert 2 * n == gold["triangle_two_row_values_n512"]
+    # PAPER.md:268 — a 32-point node needs four times the launches of a 128-point node for the same timesteps (KS)
+    nsub = 2 * 4096
+    launches = {w: sum(1 for p in sw.swept_plan(nsub, w, 2) if p[4] == w) for w in (32, 128)}
+    assert (launches[32] - 1) == gold["ks_launch_ratio_n32_vs_n128"] * (launches[128] - 1)
+    # PAPER.md:83 — two global accesses (one read, one write of the edges) per n sub-timesteps: one launch per n/(2h)
+    assert gold["global_accesses_per_n_substeps"] == 2 and launches[128] - 1 == nsub // (128 // 4)
     # PAPER.md:268 — KS with n = 32: four timesteps per cycle (m = n/(2h) = 8 sub-timesteps)
     plan = sw.swept_plan(2 * 4 * 3, 32, 2)
     assert plan[1][3] == 15 and plan[2][2] - plan[1][2] == 8
