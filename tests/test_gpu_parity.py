@@ -294,6 +294,26 @@ def test_config2_large_N(dtype):
     assert np.array_equal(ps, sx)
 
 
+def test_headline_full_size_in_the_bench_configuration():
+    # BASELINE.json's metric workload at full size (heat FP64, N = 2^20, 10 000 steps) in the launch configuration
+    # bench.py times: the autotuned (n, flavour, group), and the FLOW configuration it reports on B200.  The oracle
+    # runs the full length (a few seconds on the host cores), so every one of the 2^20 outputs is compared
+    w = si.config(2, N=1 << 20)
+    ref = oracle.run_workload(w)
+    s = sw.Swept.from_workload(w)
+    n = s.autotune(sw.SWEPT)
+    _, fl, grp = s.tuned(sw.SWEPT)
+    s.run(w.nsteps, n, sw.SWEPT, fl, grp)
+    got = s.read()
+    s.close()
+    assert np.array_equal(got, ref), (n, fl, grp)
+    assert relerr(got, ref, 1) <= 1e-12
+    got, launches = gpu_run(w, w.nsteps, sw.SWEPT, 512, sw.FLAVOR_FLOW, 3)
+    assert np.array_equal(got, ref) and launches == 3   # one persistent launch + Up/Down of the 16-step tail
+    got, _ = gpu_run(w, w.nsteps, sw.PER_STEP, 0, sw.PS_RESIDENT)
+    assert np.array_equal(got, ref)
+
+
 def test_config3_ks():
     w = si.config(3, N=1 << 14)  # full 20000 steps
     check(w, w.nsteps, [64, 256, 1024], flavors=((sw.FLAVOR_TIER, 2),) + CHAR + FLOW)
