@@ -138,7 +138,8 @@ const void* swept_device_ptr(swept_state* s);
 
 /* swept_autotune — time short runs over admissible tile widths (and flavours) for `variant`
  * (the paper also keeps the best block size per N), restore the field, remember and return
- * the best tile width.  Synchronises. */
+ * the best tile width.  Synchronises.  The result is also kept in a process-wide cache keyed by (device, problem,
+ * dtype, rk2, bc, N): states created later for the same key start with it (tile_width = 0 uses it). */
 int swept_autotune(swept_state* s, int variant, int32_t* best_tile_width);
 
 /* swept_tuned — what swept_autotune remembered for `variant`: tile width, swept flavour and its group

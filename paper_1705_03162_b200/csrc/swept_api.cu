@@ -11,6 +11,7 @@
 #include <cstdio>
 #include <cstring>
 #include <map>
+#include <mutex>
 #include <string>
 #include <tuple>
 #include <vector>
@@ -52,6 +53,16 @@ struct GraphKey {
     return std::tie(threads, P, cur, steps) < std::tie(o.threads, o.P, o.cur, o.steps);
   }
 };
+
+// autotune results of this process, keyed by (device, problem, dtype, rk2, bc, N) — PAPER.md:236 keeps the best
+// launch configuration per problem size; a state created later for the same key starts with it
+struct TunedEntry {
+  int width[2] = {0, 0};
+  int flavor = 0, P = 0;
+};
+using TunedKey = std::tuple<int, int, int, int, int, int64_t>;
+std::mutex g_tuned_mutex;
+std::map<TunedKey, TunedEntry> g_tuned;
 
 }  // namespace
 
@@ -598,6 +609,16 @@ swept_state* swept_create(int problem, int64_t N, double dx, double dt, const sw
     s->consts[2] = lam;
     s->consts[3] = 0.5 * lam;
   }
+  {
+    std::lock_guard<std::mutex> lock(g_tuned_mutex);
+    auto it = g_tuned.find(TunedKey{dev, problem, q.dtype, q.rk2, q.bc, N});
+    if (it != g_tuned.end()) {
+      s->tuned_width[0] = it->second.width[0];
+      s->tuned_width[1] = it->second.width[1];
+      s->tuned_flavor = it->second.flavor;
+      s->tuned_P = it->second.P;
+    }
+  }
   s->slab_bytes = (size_t)kShape[problem].C * (size_t)N * s->elem();
   for (int i = 0; i < 4; ++i) {
     void* ptr = nullptr;
@@ -826,6 +847,12 @@ int swept_autotune(swept_state* s, int variant, int32_t* best_tile_width) {
   if (best_n == 0) return fail(SWEPT_EUNSUPPORTED, "no admissible tile width for N=%lld", (long long)s->N);
   s->tuned_width[variant] = best_n;
   if (variant == SWEPT_SWEPT) { s->tuned_flavor = best_fl; s->tuned_P = best_P; }
+  {
+    std::lock_guard<std::mutex> lock(g_tuned_mutex);
+    TunedEntry& e = g_tuned[TunedKey{s->device, s->problem, s->dtype, s->rk2, s->bc, s->N}];
+    e.width[variant] = best_n;
+    if (variant == SWEPT_SWEPT) { e.flavor = best_fl; e.P = best_P; }
+  }
   if (best_tile_width) *best_tile_width = best_n;
   return 0;
 }

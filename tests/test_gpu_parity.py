@@ -361,5 +361,9 @@ def test_autotune_picks_admissible_width_and_keeps_state():
     assert 32 <= bt <= 1024
     s.run(100, 0, sw.SWEPT)  # uses the tuned width; the field was restored after tuning
     got = s.read()
+    tuned = s.tuned(sw.SWEPT)
     s.close()
     assert np.array_equal(got, oracle.run_workload(w, nsteps=200))
+    s2 = sw.Swept.from_workload(w)   # same (problem, dtype, N): the process-wide cache hands the result over
+    assert s2.tuned(sw.SWEPT) == tuned and tuned[0] == best
+    s2.close()
