@@ -33,6 +33,10 @@ struct TileLaunch {
   cudaStream_t stream;
   int bc = 0;  // kernel boundary mode (TIER flavour only): 0 wrap, 1 mirror, 2 fixed end states
   const double* bcv = nullptr;
+  // hybrid wall handling: TIER launches only the tiles tile_base + b * tile_step, b < tile_count (0 = all tiles);
+  // CHAR leaves the first / last tile of the row unwritten
+  int tile_base = 0, tile_step = 1, tile_count = 0;
+  int skip_first = 0, skip_last = 0;
 };
 
 // FLOW flavour: one whole Up / diamonds / Down cycle of tile width n in a single persistent launch

@@ -58,13 +58,14 @@ inline int tier_go(const TileLaunch& a) {
   t.N = a.N; t.n = a.n; t.shift = a.shift; t.ntiers = a.ntiers; t.k = round_consts<R>(a.consts);
   t.bc = a.bc;
   t.bv = round_bcvals<R>(a.bcv);
+  t.tile_base = a.tile_base; t.tile_step = a.tile_step; t.skip_first = 0; t.skip_last = 0;
   const size_t smem = tier_smem_bytes<Prob>(a.n);
   auto kern = swept_tier_kernel<Prob, P, KIND>;
   if (smem > 48 * 1024) {
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return (int)e;
   }
-  kern<<<(unsigned)(a.N / a.n), a.n / P, smem, a.stream>>>(t);
+  kern<<<(unsigned)(a.tile_count > 0 ? a.tile_count : a.N / a.n), a.n / P, smem, a.stream>>>(t);
   return (int)cudaGetLastError();
 }
 
@@ -118,6 +119,7 @@ inline int char_go(const TileLaunch& a) {
   t.N = a.N; t.n = a.n; t.shift = a.shift; t.ntiers = a.ntiers; t.k = round_consts<R>(a.consts);
   t.bc = 0;
   t.bv = round_bcvals<R>(nullptr);
+  t.tile_base = 0; t.tile_step = 1; t.skip_first = a.skip_first; t.skip_last = a.skip_last;
   const size_t smem = char_smem_bytes<Prob>(T, B);
   auto kern = swept_char_kernel<Prob, B, L, KIND>;
   if (smem > 48 * 1024) {

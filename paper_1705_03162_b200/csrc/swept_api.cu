@@ -95,6 +95,8 @@ struct swept_state {
   int* flow_scratch = nullptr;
   size_t flow_scratch_ints = 0;
   bool flow_pending_check = false;
+  cudaStream_t wall_stream = nullptr;  // hybrid wall handling: the wall tiles run here, beside the CHAR launch
+  cudaEvent_t wall_fork = nullptr, wall_join = nullptr;
   void* resident_scratch = nullptr;  // flags + exchange slots of the resident per-step kernel
   bool resident_pending_check = false;  // a FLOW launch has run since the error word was last read
   size_t elem() const { return dtype == SWEPT_F64 ? 8 : 4; }
@@ -122,10 +124,10 @@ int launch_per_step(swept_state* s, const void* in, const void* base, void* out,
   return 0;
 }
 
-int launch_tile(swept_state* s, swept::TileLaunch& a) {
+int launch_tile(swept_state* s, swept::TileLaunch& a, cudaStream_t stream = nullptr) {
   a.N = s->N;
   a.consts = s->consts;
-  a.stream = s->stream;
+  a.stream = stream ? stream : s->stream;
   a.bc = s->kernel_bc();
   a.bcv = s->bcvals;
   int rc;
@@ -222,7 +224,11 @@ struct TimedScope {
 
 bool tile_ok(const swept_state* s, int flavor, int n, int P) {
   if (n <= 0 || s->N % n != 0) return false;
-  if (s->bc && flavor != SWEPT_FLAVOR_TIER) return false;  // walls are applied by the TIER flavour only
+  // walls are applied by the TIER kernels; the CHAR flavour can run beside them on all other tiles (heat: hybrid)
+  if (s->bc && flavor != SWEPT_FLAVOR_TIER && !(flavor == SWEPT_FLAVOR_CHAR && s->problem == SWEPT_HEAT)) return false;
+  if (s->bc && flavor == SWEPT_FLAVOR_CHAR && !swept::tile_config_ok_heat(s->dtype, SWEPT_FLAVOR_TIER, s->N, n,
+                                                                            n >= 1024 ? 4 : (n >= 512 ? 2 : 1)))
+    return false;
   if (flavor == SWEPT_FLAVOR_FLOW && (s->problem == SWEPT_EULER || P < 0 || P > 16)) return false;
   switch (s->problem) {
     case SWEPT_HEAT: return swept::tile_config_ok_heat(s->dtype, flavor, s->N, n, P);
@@ -531,11 +537,40 @@ int run_swept(swept_state* s, int64_t nsteps, int n, int flavor, int P) {
     }
     a.out0 = s->slab[o0];
     a.out1 = s->slab[o1];
+    const bool hybrid = s->bc && a.flavor == SWEPT_FLAVOR_CHAR && ph.kind != KIND_UP;  // Up reads no halo
+    if (hybrid) {
+      // The tiles that touch a wall (aligned rows: the first and the last tile; shifted rows: the tile split across
+      // the boundary) go to the TIER kernels, which apply the boundary condition, on a second
+      // stream beside the register-resident launch — the paper's Hybrid idea with a stream in
+      // place of the CPU.  Both read the same input rows and write disjoint ranges of the output rows.
+      if (!s->wall_stream) {
+        CUDA_TRY(cudaStreamCreateWithFlags(&s->wall_stream, cudaStreamNonBlocking));
+        CUDA_TRY(cudaEventCreateWithFlags(&s->wall_fork, cudaEventDisableTiming));
+        CUDA_TRY(cudaEventCreateWithFlags(&s->wall_join, cudaEventDisableTiming));
+      }
+      CUDA_TRY(cudaEventRecord(s->wall_fork, s->stream));
+      CUDA_TRY(cudaStreamWaitEvent(s->wall_stream, s->wall_fork, 0));
+      a.skip_first = ph.shift == 0 ? 1 : 0;
+      a.skip_last = 1;
+    }
     {
       TimedScope ts(s, ph.kind, 1);
       if (int rc = launch_tile(s, a)) return rc;
     }
     s->last_launches += 1;
+    if (hybrid) {
+      const int K = (int)(s->N / ph.n);
+      swept::TileLaunch w = a;
+      w.flavor = SWEPT_FLAVOR_TIER;
+      w.P = ph.n >= 1024 ? 4 : (ph.n >= 512 ? 2 : 1);
+      w.skip_first = w.skip_last = 0;
+      if (ph.shift == 0) { w.tile_base = 0; w.tile_step = K - 1; w.tile_count = K > 1 ? 2 : 1; }
+      else { w.tile_base = K - 1; w.tile_step = 0; w.tile_count = 1; }
+      if (int rc = launch_tile(s, w, s->wall_stream)) return rc;
+      s->last_launches += 1;
+      CUDA_TRY(cudaEventRecord(s->wall_join, s->wall_stream));
+      CUDA_TRY(cudaStreamWaitEvent(s->stream, s->wall_join, 0));
+    }
     r0 = o0;
     r1 = o1;
     if (ph.kind == KIND_DOWN) s->cur = o0;  // row0 holds the full time level (T is even)
@@ -654,6 +689,12 @@ void swept_destroy(swept_state* s) {
   for (cudaEvent_t e : s->event_pool) cudaEventDestroy(e);
   if (s->flow_scratch) cudaFree(s->flow_scratch);
   if (s->resident_scratch) cudaFree(s->resident_scratch);
+  if (s->wall_stream) {
+    cudaStreamSynchronize(s->wall_stream);
+    cudaStreamDestroy(s->wall_stream);
+    cudaEventDestroy(s->wall_fork);
+    cudaEventDestroy(s->wall_join);
+  }
   for (int i = 0; i < 4; ++i) {
     if (!s->slab[i]) continue;
     if (s->free_) s->free_(s->alloc_ctx, s->slab[i]);

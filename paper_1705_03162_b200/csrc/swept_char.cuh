@@ -281,8 +281,13 @@ __global__ void __launch_bounds__(128) swept_char_kernel(const TierArgs<typename
 #pragma unroll
       for (int c = 0; c < C; ++c) {
         const R* sm = rows + (r * C + c) * RS + PAD;
-        bulk_s2g(dstg + (int64_t)c * N + S, sm, (uint32_t)(len1 * sizeof(R)));
-        if (len2 > 0) bulk_s2g(dstg + (int64_t)c * N, sm + len1, (uint32_t)(len2 * sizeof(R)));
+        // [lo, hi) of the chunk is written; a wall tile at either end of the row belongs to the TIER launch
+        const int lo = (a.skip_first && blockIdx.x == 0) ? n : 0;
+        const int hi = chunk - ((a.skip_last && blockIdx.x == gridDim.x - 1) ? n : 0);
+        const int e1 = hi < len1 ? hi : len1;  // end of the part before the periodic wrap
+        if (e1 > lo) bulk_s2g(dstg + (int64_t)c * N + S + lo, sm + lo, (uint32_t)((e1 - lo) * sizeof(R)));
+        const int b2 = lo > len1 ? lo : len1;
+        if (hi > b2) bulk_s2g(dstg + (int64_t)c * N + (b2 - len1), sm + b2, (uint32_t)((hi - b2) * sizeof(R)));
       }
     }
     bulk_commit();

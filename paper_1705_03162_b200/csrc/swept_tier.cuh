@@ -40,6 +40,10 @@ struct TierArgs {
   int bc;      // BC_WRAP, BC_MIRROR (heat, Eq. (B.5): T_{-k} = T_k, T_{N-1+k} = T_{N-1-k}) or
                // BC_FIXED (Euler tube: ghost cells hold the end states bv.l / bv.r)
   BcVals<R> bv;
+  // tile selection.  TIER: block b computes tile tile_base + b * tile_step (default 0, 1: every tile).  CHAR: the
+  // first / last tile of the row is left to a TIER launch that applies the walls (hybrid mode)
+  int tile_base, tile_step;
+  int skip_first, skip_last;
   Consts<R> k;
 };
 
@@ -66,7 +70,7 @@ __global__ void __launch_bounds__(Prob::MAX_THREADS) swept_tier_kernel(const Tie
   uint64_t* mbar = reinterpret_cast<uint64_t*>(smem_raw + (size_t)2 * C * RS * sizeof(R));
   const int64_t N = a.N;
   const int tid = threadIdx.x;
-  int64_t S = (int64_t)a.shift + (int64_t)blockIdx.x * n;
+  int64_t S = (int64_t)a.shift + ((int64_t)a.tile_base + (int64_t)blockIdx.x * a.tile_step) * n;
   if (S >= N) S -= N;
   const int len1 = (int)((N - S) < (int64_t)n ? (N - S) : (int64_t)n);  // part before the periodic wrap
   const int len2 = n - len1;

@@ -190,10 +190,24 @@ def test_heat_insulated_ends_bc_paper():
     w = si.heat_insulated(2048, 4, 32, 300)
     assert np.array_equal(gpu_run(w, 300, sw.SWEPT, 128, dtype=np.float32)[0],
                           oracle.run_workload(w, dtype=np.float32))
+    # hybrid: CHAR on every tile that touches no wall, the wall tiles by the TIER kernels on a second stream
+    for N, steps in ((1024, 900), (1 << 15, 700), (1 << 20, 1300)):
+        w2 = si.heat_insulated(N, 6, 33, steps)
+        ref2 = oracle.run_workload(w2)
+        ran = 0
+        for n in (64, 256, 512, 1024):
+            for L in (8, 16, 32):
+                try:
+                    sx, _ = gpu_run(w2, steps, sw.SWEPT, n, sw.FLAVOR_CHAR, L)
+                except sw.SweptError as e:
+                    assert "not admissible" in str(e)
+                    continue
+                ran += 1
+                assert np.array_equal(sx, ref2), ("hybrid", N, n, L)
+        assert ran >= 4
     s = sw.Swept.from_workload(w)
-    for fl in (sw.FLAVOR_CHAR, sw.FLAVOR_FLOW):      # register flavours are periodic only: clean error
-        with pytest.raises(sw.SweptError):
-            s.run(10, 256, sw.SWEPT, fl)
+    with pytest.raises(sw.SweptError):               # the persistent flavours are periodic only: clean error
+        s.run(10, 256, sw.SWEPT, sw.FLAVOR_FLOW)
     with pytest.raises(sw.SweptError):
         s.run(10, 0, sw.PER_STEP, sw.PS_RESIDENT)
     best = s.autotune(sw.SWEPT)
