@@ -23,7 +23,7 @@
 //
 // Shared memory holds the CTA's chunk of both rows (T*B contiguous points, all tiles of the CTA), loaded and
 // stored with TMA 1-D bulk copies, and is updated in place: stream / final writes only touch slots whose
-// input value has already been consumed (see DESIGN.md §5.3 for the hazard argument).
+// input value has already been consumed (see DESIGN.md §5.4 for the hazard argument).
 #pragma once
 #include "common.cuh"
 #include "functors.cuh"
