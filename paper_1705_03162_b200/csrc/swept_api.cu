@@ -386,6 +386,17 @@ void default_tile(const swept_state* s, int* n_io, int* flavor_io, int* P_io) {
   }
   // untuned defaults (measured on B200): heat and KS run fastest with the register-resident
   // CHAR flavour on wide tiles, Euler (about 250 live registers per point) with the TIER flavour
+  // fully default call (no width, no flavour, nothing tuned) on a large periodic heat / KS problem: the persistent
+  // FLOW launch at the width measured best on B200 (N >= 2^19)
+  if (n == 0 && flavor == SWEPT_FLAVOR_AUTO && !s->bc && s->problem != SWEPT_EULER && s->N >= (1 << 19)) {
+    const int cand = s->problem == SWEPT_HEAT ? 512 : 1024;
+    if (tile_ok(s, SWEPT_FLAVOR_FLOW, cand, 0)) {
+      *n_io = cand;
+      *flavor_io = SWEPT_FLAVOR_FLOW;
+      *P_io = 0;
+      return;
+    }
+  }
   const bool want_char = flavor == SWEPT_FLAVOR_CHAR ||
                          (flavor == SWEPT_FLAVOR_AUTO && s->problem != SWEPT_EULER && !s->bc);
   if (n == 0) {

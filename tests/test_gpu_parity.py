@@ -265,6 +265,32 @@ def test_repeated_runs_accumulate_and_launch_counts():
     assert np.array_equal(got, oracle.run_workload(w, nsteps=1800))
 
 
+def test_phase_timing_and_fully_default_run():
+    # swept_set_phase_timing / swept_phase_times: one CUDA-event pair per launch, reported per phase kind
+    w = si.heat_sines(1 << 14, 8, 2, 0)
+    s = sw.Swept.from_workload(w)
+    s.set_phase_timing(True)
+    s.run(128 * 6, 256, sw.SWEPT, sw.FLAVOR_CHAR, 32)      # Up, 5 diamonds (3 split, 2 whole), Down
+    t = s.phase_times()
+    assert [t[k][1] for k in ("UpTriangle", "SplitDiamond", "WholeDiamond", "DownTriangle")] == [1, 3, 2, 1]
+    assert all(t[k][0] > 0 for k in ("UpTriangle", "SplitDiamond", "WholeDiamond", "DownTriangle"))
+    s.run(128 * 6, 256, sw.SWEPT, sw.FLAVOR_FLOW)
+    t = s.phase_times()
+    assert t["FlowCycle"][1] == 1 and t["FlowCycle"][0] > 0 and t["SplitDiamond"][1] == 0
+    s.set_phase_timing(False)
+    s.run(10, 256, sw.SWEPT)
+    assert sum(v[1] for v in s.phase_times().values()) == 0
+    s.close()
+    # swept_run(state, nsteps, 0, SWEPT) with nothing tuned on a large problem: FLOW at the measured-best width
+    for w in (si.heat_sines(1 << 19, 8, 3, 600), si.ks_cos(1 << 19, 3, 300)):
+        s = sw.Swept.from_workload(w)
+        s.run(w.nsteps, 0, sw.SWEPT)
+        got = s.read()
+        s.close()
+        ps, _ = gpu_run(w, w.nsteps, sw.PER_STEP)
+        assert np.array_equal(got, ps)
+
+
 def test_error_codes():
     w = si.heat_sines(4096, 8, 2, 0)
     s = sw.Swept.from_workload(w)
