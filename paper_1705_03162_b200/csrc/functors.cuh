@@ -52,6 +52,7 @@ struct Heat {
   using R = R_;
   static constexpr int H = 1, C = 1, SIGMA = 1;
   static constexpr int MAX_THREADS = 1024;  // per CTA, for __launch_bounds__ (register budget)
+  static constexpr int TIER_MAX_THREADS = 1024;
   __device__ __forceinline__ static R point(R um, R u0, R up, const Consts<R>& k) {
     const R s = um + up;
     const R t = k.a1 * u0;
@@ -73,6 +74,7 @@ struct KS {
   using R = R_;
   static constexpr int H = 2, C = 1, SIGMA = 2;
   static constexpr int MAX_THREADS = 1024;
+  static constexpr int TIER_MAX_THREADS = 1024;
   __device__ __forceinline__ static R rhs(R vm2, R vm1, R v0, R vp1, R vp2, const Consts<R>& k) {
     const R s1 = vp1 + vm1;
     const R s2 = vp2 + vm2;
@@ -112,6 +114,7 @@ struct Euler {
   using R = R_;
   static constexpr int H = 2, C = 3, SIGMA = 2;
   static constexpr int MAX_THREADS = 256;  // ~250 live registers per thread (P:270 'greater low-level memory usage')
+  static constexpr int TIER_MAX_THREADS = 1024;  // the TIER kernel shares pressures and fluxes: 64 registers
 
   __device__ __forceinline__ static R pressure(R rho, R M, R E, const Consts<R>& k) {  // (D.4), X4
     const R u = M / rho;
@@ -151,6 +154,17 @@ struct Euler {
     F[1] = (R)0.5 * fma_(rsp, QL[1] - QR[1], FR1 + FL1);
     F[2] = (R)0.5 * fma_(rsp, QL[2] - QR[2], FR2 + FL2);
   }
+  // one component of one cell: v = stage input, base = u^n, dF = Flux_{j+1/2} - Flux_{j-1/2}
+  __device__ __forceinline__ static R update(R v, R base, R dF, int odd, const Consts<R>& k) {
+    if (HEUN) {
+      const R t = fma_(-k.a2, dF, v);                   // v + dt f(v)
+      return odd ? t : (R)0.5 * (base + t);
+    } else {
+      const R hs = odd ? k.a3 : k.a2;                    // (D.12) with X1 (minus)
+      const R b = odd ? v : base;
+      return fma_(-hs, dF, b);
+    }
+  }
   template <int P>
   __device__ __forceinline__ static void stage(const R (&win)[C][P + 2 * H], const R (&base)[C][P],
                                                R (&out)[C][P], int odd, const Consts<R>& k) {
@@ -172,15 +186,7 @@ struct Euler {
         const int j = i - 1;
 #pragma unroll
         for (int c = 0; c < 3; ++c) {
-          const R dF = F[c] - Fprev[c];
-          if (HEUN) {
-            const R t = fma_(-k.a2, dF, win[c][j + 2]);               // v + dt f(v)
-            out[c][j] = odd ? t : (R)0.5 * (base[c][j] + t);
-          } else {
-            const R hs = odd ? k.a3 : k.a2;                            // (D.12) with X1 (minus)
-            const R b = odd ? win[c][j + 2] : base[c][j];
-            out[c][j] = fma_(-hs, dF, b);
-          }
+          out[c][j] = update(win[c][j + 2], base[c][j], F[c] - Fprev[c], odd, k);
         }
       }
 #pragma unroll

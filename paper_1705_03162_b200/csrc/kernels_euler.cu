@@ -12,7 +12,8 @@ extern template int char_L<Euler<double, 1>, 16>(const TileLaunch&);
 
 int launch_per_step_euler(int dtype, int rk2, const PerStepLaunch& a) {
   if (dtype != 0) return NO_KERNEL;
-  return rk2 == 0 ? per_step_T<Euler<double, 0>, 2>(a) : per_step_T<Euler<double, 1>, 2>(a);
+  if (a.N < 8) return NO_KERNEL;
+  return rk2 == 0 ? per_step_lane_go<Euler<double, 0>>(a) : per_step_lane_go<Euler<double, 1>>(a);
 }
 bool tile_config_ok_euler(int dtype, int flavor, int64_t N, int n, int P) {
   if (dtype != 0) return false;

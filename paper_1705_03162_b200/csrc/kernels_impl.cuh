@@ -39,6 +39,18 @@ inline int per_step_go(const PerStepLaunch& a) {
   return (int)cudaGetLastError();
 }
 
+// Euler: one interface per lane, 28 cells per warp (per_step.cuh)
+template <class Prob>
+inline int per_step_lane_go(const PerStepLaunch& a) {
+  using R = typename Prob::R;
+  const int threads = 256;
+  const int64_t warps = (a.N + 27) / 28;
+  const unsigned grid = (unsigned)((warps * 32 + threads - 1) / threads);
+  per_step_lane_kernel<Prob><<<grid, threads, 0, a.stream>>>((const R*)a.in, (const R*)a.base, (R*)a.out, a.N, a.odd,
+                                                             round_consts<R>(a.consts), a.bc, round_bcvals<R>(a.bcv));
+  return (int)cudaGetLastError();
+}
+
 template <class Prob, int PMAX>
 inline int per_step_T(const PerStepLaunch& a) {
   if (a.N % a.P != 0) return NO_KERNEL;
@@ -86,7 +98,7 @@ inline bool tier_ok(int n, int P, int pmax) {
   if (P != 1 && P != 2 && P != 4) return false;
   if (P > pmax) return false;
   const int threads = n / P;
-  if (threads < 8 || threads > Prob::MAX_THREADS) return false;
+  if (threads < 8 || threads > Prob::TIER_MAX_THREADS) return false;
   return tier_smem_bytes<Prob>(n) <= 227 * 1024;
 }
 

@@ -83,4 +83,52 @@ per_step_kernel(const typename Prob::R* __restrict__ in, const typename Prob::R*
   for (int c = 0; c < C; ++c) store_vec<R, P>(out + (int64_t)c * N + i0, o[c]);
 }
 
+// ---------------------------------------------------------------------------------------------------------
+// Per-step kernel for the finite-volume Euler scheme, one INTERFACE per lane.  The generic kernel above lets every
+// thread rebuild the P+4 pressures and P+1 interface fluxes of its P cells (P = 2: three pressures and 1.5 fluxes
+// per cell, each flux with 8 divisions and 3 square roots).  Here lane l of a warp holds cell j = 28 w + l - 2,
+// computes that cell's pressure and the flux at its right interface j+1/2 once, and receives the neighbours'
+// pressures, the right neighbour's state and the left interface's flux by warp shuffles; lanes 2..29 then update
+// their cell (28 cells per warp: 1.14 pressures and 1.14 fluxes per cell).  Same pressure(), flux() and update
+// expressions as Euler::stage, so the result is bit-identical.
+template <class Prob>
+__global__ void __launch_bounds__(256)
+per_step_lane_kernel(const typename Prob::R* __restrict__ in, const typename Prob::R* __restrict__ base,
+                     typename Prob::R* __restrict__ out, int64_t N, int odd, Consts<typename Prob::R> k, int bc,
+                     BcVals<typename Prob::R> bv) {
+  using R = typename Prob::R;
+  static_assert(Prob::C == 3 && Prob::H == 2, "interface-per-lane kernel is written for the Euler scheme");
+  constexpr int USE = 28;  // cells updated per warp
+  const int lane = threadIdx.x & 31;
+  const int64_t w = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+  if (w * USE >= N) return;  // whole warp
+  const int64_t j = w * USE + lane - 2;
+  // state of cell j: periodic wrap, or the fixed end states of the tube in the ghost cells
+  int64_t g = j;
+  const bool ghost = bc == BC_FIXED && (j < 0 || j >= N);
+  if (g < 0) g += N;
+  while (g >= N) g -= N;  // the tail warp may reach a few cells past N + 1: any valid cell will do, nothing is stored
+  R V[3];
+#pragma unroll
+  for (int c = 0; c < 3; ++c) V[c] = ghost ? (j < 0 ? bv.l[c] : bv.r[c]) : __ldg(in + (int64_t)c * N + g);
+  const R pr = Prob::pressure(V[0], V[1], V[2], k);
+  const R pm1 = __shfl_up_sync(0xffffffffu, pr, 1);
+  const R pp1 = __shfl_down_sync(0xffffffffu, pr, 1);
+  const R pp2 = __shfl_down_sync(0xffffffffu, pr, 2);
+  R Vr[3];
+#pragma unroll
+  for (int c = 0; c < 3; ++c) Vr[c] = __shfl_down_sync(0xffffffffu, V[c], 1);
+  R F[3], Fl[3];
+  Prob::flux(V, Vr, pr - pm1, pp1 - pr, pp2 - pp1, F, k);  // interface j + 1/2 (meaningless in lanes 0, 30, 31)
+#pragma unroll
+  for (int c = 0; c < 3; ++c) Fl[c] = __shfl_up_sync(0xffffffffu, F[c], 1);  // interface j - 1/2
+  if (lane >= 2 && lane < 2 + USE && j < N) {
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+      const R b0 = (!odd) ? __ldg(base + (int64_t)c * N + j) : V[c];
+      out[(int64_t)c * N + j] = Prob::update(V[c], b0, F[c] - Fl[c], odd, k);
+    }
+  }
+}
+
 }  // namespace swept

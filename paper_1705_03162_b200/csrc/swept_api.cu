@@ -368,7 +368,10 @@ int64_t make_plan(int64_t nsub, const std::vector<int>& widths, int h, std::vect
 constexpr int MIN_LEVEL_WIDTH = 32;  // narrowest tile of the remainder cycles
 
 int tier_default_P(const swept_state* s, int n) {
-  const int pmax = 4, tmax = s->problem == SWEPT_EULER ? 256 : 1024;
+  // Euler's TIER tiers spread their pressure / flux work over all threads of the CTA: one thread per point
+  // (measured: 256 threads per tile are best, more only add barrier cost)
+  if (s->problem == SWEPT_EULER) return n <= 256 ? 1 : (n <= 2048 ? 2 : 4);
+  const int pmax = 4, tmax = 1024;
   int P = std::min(pmax, std::max(1, n / 256));
   while (P < pmax && n / P > tmax) P *= 2;
   if (P == 3) P = 2;

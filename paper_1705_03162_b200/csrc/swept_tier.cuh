@@ -60,7 +60,7 @@ __device__ __forceinline__ void tier_range(int t, int n, int h, int m, int& lo, 
 }
 
 template <class Prob, int P, int KIND>
-__global__ void __launch_bounds__(Prob::MAX_THREADS) swept_tier_kernel(const TierArgs<typename Prob::R> a) {
+__global__ void __launch_bounds__(Prob::TIER_MAX_THREADS) swept_tier_kernel(const TierArgs<typename Prob::R> a) {
   using R = typename Prob::R;
   constexpr int H = Prob::H, C = Prob::C, PAD = Pad16<R>::value;
   extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -68,6 +68,8 @@ __global__ void __launch_bounds__(Prob::MAX_THREADS) swept_tier_kernel(const Tie
   const int RS = n + 4 * PAD;  // padded row stride: body starts 16 bytes in; room for the wall gap (see below)
   R* rows = reinterpret_cast<R*>(smem_raw);
   uint64_t* mbar = reinterpret_cast<uint64_t*>(smem_raw + (size_t)2 * C * RS * sizeof(R));
+  R* xtr = reinterpret_cast<R*>(smem_raw + (size_t)2 * C * RS * sizeof(R) + 16);  // Euler: pressures, fluxes
+  (void)xtr;
   const int64_t N = a.N;
   const int tid = threadIdx.x;
   int64_t S = (int64_t)a.shift + ((int64_t)a.tile_base + (int64_t)blockIdx.x * a.tile_step) * n;
@@ -145,7 +147,39 @@ __global__ void __launch_bounds__(Prob::MAX_THREADS) swept_tier_kernel(const Tie
     R* dst = rows + par * C * RS;
     int lo, hi;
     tier_range<KIND>(t, n, H, m, lo, hi);
-    if (j0 < hi && j0 + P > lo) {
+    if constexpr (Prob::C == 3) {
+      // Euler: every pressure and every interface flux of the tier is computed ONCE and shared through shared
+      // memory (Prob::stage would rebuild P+4 pressures and P+1 fluxes per thread: 8 divisions and 3 square roots
+      // per flux).  Three steps per tier, all threads of the CTA share the slots of the active range evenly:
+      //   A  pressure (D.4) of the slots [lo-2, hi+2);  B  flux (D.6)-(D.11) at the right interface of the slots
+      //   [lo-1, hi);  C  update (D.12) of the points [lo, hi).  Same pressure()/flux()/update() as Prob::stage.
+      R* prs = xtr;
+      R* flx = xtr + RS;
+      const int s_lo = slot_of(lo), s_hi = slot_of(hi - 1) + 1;  // slot range of the active points (gap included)
+      for (int q = s_lo - 2 + tid; q < s_hi + 2; q += blockDim.x)
+        prs[q] = Prob::pressure(src[q], src[RS + q], src[2 * RS + q], a.k);
+      __syncthreads();
+      for (int q = s_lo - 1 + tid; q < s_hi; q += blockDim.x) {
+        const R vl[3] = {src[q], src[RS + q], src[2 * RS + q]};
+        const R vr[3] = {src[q + 1], src[RS + q + 1], src[2 * RS + q + 1]};
+        R F[3];
+        Prob::flux(vl, vr, prs[q] - prs[q - 1], prs[q + 1] - prs[q], prs[q + 2] - prs[q + 1], F, a.k);
+        flx[q] = F[0];
+        flx[RS + q] = F[1];
+        flx[2 * RS + q] = F[2];
+      }
+      __syncthreads();
+#pragma unroll
+      for (int j = 0; j < P; ++j)
+        if (j0 + j >= lo && j0 + j < hi) {
+#pragma unroll
+          for (int c = 0; c < C; ++c) {
+            const R v = src[c * RS + sb + j];
+            const R b = !par ? dst[c * RS + sb + j] : v;
+            dst[c * RS + sb + j] = Prob::update(v, b, flx[c * RS + sb + j] - flx[c * RS + sb + j - 1], par, a.k);
+          }
+        }
+    } else if (j0 < hi && j0 + P > lo) {
       R win[C][P + 2 * H], bs[C][P], o[C][P];
 #pragma unroll
       for (int c = 0; c < C; ++c)
@@ -200,7 +234,8 @@ __global__ void __launch_bounds__(Prob::MAX_THREADS) swept_tier_kernel(const Tie
 template <class Prob>
 inline size_t tier_smem_bytes(int n) {
   using R = typename Prob::R;
-  return (size_t)2 * Prob::C * (n + 4 * Pad16<R>::value) * sizeof(R) + 16;
+  const size_t row = ((size_t)n + 4 * Pad16<R>::value) * sizeof(R);
+  return (size_t)2 * Prob::C * row + 16 + (Prob::C == 3 ? 4 * row : 0);  // Euler: + one pressure and three flux rows
 }
 
 }  // namespace swept
