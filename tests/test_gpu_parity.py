@@ -249,6 +249,14 @@ def test_per_step_non_power_of_two_N():
         assert np.array_equal(got, ref)
     w = si.ks_cos(1001, 9, 30)
     assert np.array_equal(gpu_run(w, 30, sw.PER_STEP)[0], oracle.run_workload(w))
+    # Euler's interface-per-lane kernel: 28 cells per warp, ragged last warp, wrap inside a warp
+    for N in (30, 57, 1000, 1023):
+        w = si.euler_double_sod(N, 25)
+        w.u0 = si.random_smooth(si.EULER, N, 77)
+        w.dt = 0.1 * w.dx
+        assert np.array_equal(gpu_run(w, 25, sw.PER_STEP)[0], oracle.run_workload(w)), N
+    w = si.euler_sod(999, 40)
+    assert np.array_equal(gpu_run(w, 40, sw.PER_STEP)[0], oracle.run_workload(w))
 
 
 def test_repeated_runs_accumulate_and_launch_counts():
