@@ -158,7 +158,9 @@ inline bool char_ok(int64_t N, int n, int L) {
   if (L != 8 && L != 16 && L != 32) return false;
   if (n % L) return false;
   const int B = n / L;
-  if (B != 8 && B != 16 && B != 32) return false;
+  // B = 4 (3-point stencil only: the chain length B/2h must stay even for the 5-point RK2 schemes) serves the
+  // narrow tiles of the remainder cycles: n = 32 with L = 8
+  if (B != 8 && B != 16 && B != 32 && !(B == 4 && Prob::H == 1)) return false;
   if (B > BMAX || B % (2 * Prob::H)) return false;
   const int T = char_threads(N, B);
   return T >= L && N % n == 0;
@@ -178,6 +180,7 @@ template <class Prob, int BMAX>
 int char_T(const TileLaunch& a) {
   if (!char_ok<Prob, BMAX>(a.N, a.n, a.P)) return NO_KERNEL;
   switch (a.n / a.P) {
+    case 4: if (Prob::H == 1) return char_L<Prob, (Prob::H == 1 ? 4 : 8)>(a); break;
     case 8: return char_L<Prob, 8>(a);
     case 16: if (BMAX >= 16) return char_L<Prob, (BMAX >= 16 ? 16 : 8)>(a); break;
     case 32: if (BMAX >= 32) return char_L<Prob, (BMAX >= 32 ? 32 : 8)>(a); break;

@@ -458,7 +458,7 @@ bool level_config(const swept_state* s, int n_top, int flavor_top, int P_top, in
   }
   if (flavor_top == SWEPT_FLAVOR_CHAR) {
     const int B_top = n_top / P_top;
-    for (int B : {B_top, 16, 8, 32}) {
+    for (int B : {B_top, 16, 8, 32, 4}) {
       if (n % B) continue;
       if (tile_ok(s, SWEPT_FLAVOR_CHAR, n, n / B)) {
         *flavor = SWEPT_FLAVOR_CHAR;
