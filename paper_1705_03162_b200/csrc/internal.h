@@ -73,6 +73,7 @@ constexpr int RESIDENT_MAX_CTAS = 4096;
 // combination has no kernel.
 int launch_per_step_heat(int dtype, const PerStepLaunch& a);
 int launch_per_step_ks(int dtype, int rk2, const PerStepLaunch& a);
+int launch_per_step_ks_fused(int dtype, int rk2, const PerStepLaunch& a);  // both stages of a timestep in one launch
 int launch_per_step_euler(int dtype, int rk2, const PerStepLaunch& a);
 int launch_tile_heat(int dtype, const TileLaunch& a);
 int launch_tile_ks(int dtype, int rk2, const TileLaunch& a);

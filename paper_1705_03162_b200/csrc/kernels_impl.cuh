@@ -39,6 +39,19 @@ inline int per_step_go(const PerStepLaunch& a) {
   return (int)cudaGetLastError();
 }
 
+// scalar RK2 schemes: both stages of a timestep in one launch (per_step.cuh)
+template <class Prob, int P>
+inline int per_step_fused_go(const PerStepLaunch& a) {
+  using R = typename Prob::R;
+  if (a.N % P || a.bc) return NO_KERNEL;
+  const int64_t nthreads = a.N / P;
+  const int threads = a.threads < Prob::MAX_THREADS ? a.threads : Prob::MAX_THREADS;
+  const unsigned grid = (unsigned)((nthreads + threads - 1) / threads);
+  per_step_fused_kernel<Prob, P><<<grid, threads, 0, a.stream>>>((const R*)a.in, (R*)a.out, a.N,
+                                                                   round_consts<R>(a.consts));
+  return (int)cudaGetLastError();
+}
+
 // Euler: one interface per lane, 28 cells per warp (per_step.cuh)
 template <class Prob>
 inline int per_step_lane_go(const PerStepLaunch& a) {

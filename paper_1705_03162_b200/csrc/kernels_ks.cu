@@ -5,6 +5,13 @@ int launch_per_step_ks(int dtype, int rk2, const PerStepLaunch& a) {
   if (dtype != 0) return NO_KERNEL;
   return rk2 == 0 ? per_step_T<KS<double, 0>, 4>(a) : per_step_T<KS<double, 1>, 4>(a);
 }
+// one launch per timestep: in = u^n, out = u^{n+1} (a.base and a.odd unused); P = 4 or 2 or 1 by divisibility
+int launch_per_step_ks_fused(int dtype, int rk2, const PerStepLaunch& a) {
+  if (dtype != 0) return NO_KERNEL;
+  if (a.P == 4) return rk2 == 0 ? per_step_fused_go<KS<double, 0>, 4>(a) : per_step_fused_go<KS<double, 1>, 4>(a);
+  if (a.P == 2) return rk2 == 0 ? per_step_fused_go<KS<double, 0>, 2>(a) : per_step_fused_go<KS<double, 1>, 2>(a);
+  return NO_KERNEL;
+}
 bool tile_config_ok_ks(int dtype, int flavor, int64_t N, int n, int P) {
   if (dtype != 0) return false;
   if (flavor == SWEPT_FLAVOR_TIER) return tier_ok<KS<double, 0>>(n, P, 4);

@@ -84,6 +84,47 @@ per_step_kernel(const typename Prob::R* __restrict__ in, const typename Prob::R*
 }
 
 // ---------------------------------------------------------------------------------------------------------
+// Per-step kernel for a two-stage scalar scheme (KS), one launch per TIMESTEP (north_star allows "one launch per
+// timestep or RK stage"): a thread reads the window of its P points widened by 2h on either side, evaluates the
+// predictor stage on its P points and their h neighbours on either side (recomputed, not communicated), then
+// the final stage on its P points.  Same Prob::stage trees as the two-launch form, so the same bits; half the
+// launches and no predictor array in global memory (16 B instead of 40 B per point and timestep).
+template <class Prob, int P>
+__global__ void __launch_bounds__(Prob::MAX_THREADS)
+per_step_fused_kernel(const typename Prob::R* __restrict__ in, typename Prob::R* __restrict__ out, int64_t N,
+                      Consts<typename Prob::R> k) {
+  using R = typename Prob::R;
+  constexpr int H = Prob::H;
+  static_assert(Prob::C == 1 && Prob::SIGMA == 2, "fused two-stage kernel: scalar RK2 schemes");
+  const int64_t i0 = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) * P;
+  if (i0 >= N) return;
+  constexpr int Q = P + 2 * H;  // points whose predictor value this thread needs
+  alignas(16) R win[1][Q + 2 * H];
+  alignas(16) R body[P];
+  load_vec<R, P>(in + i0, body);
+#pragma unroll
+  for (int j = 0; j < P; ++j) win[0][2 * H + j] = body[j];
+#pragma unroll
+  for (int j = 0; j < 2 * H; ++j) {
+    int64_t il = i0 - 2 * H + j;
+    if (il < 0) il += N;
+    int64_t ir = i0 + P + j;
+    if (ir >= N) ir -= N;
+    win[0][j] = __ldg(in + il);
+    win[0][2 * H + P + j] = __ldg(in + ir);
+  }
+  R ctr[1][Q], pred[1][Q];
+#pragma unroll
+  for (int j = 0; j < Q; ++j) ctr[0][j] = win[0][H + j];
+  Prob::template stage<Q>(win, ctr, pred, 1, k);  // predictor u* at i0-h .. i0+P+h-1 (odd tier)
+  R bs[1][P], o[1][P];
+#pragma unroll
+  for (int j = 0; j < P; ++j) bs[0][j] = body[j];
+  Prob::template stage<P>(pred, bs, o, 0, k);      // final stage: window = u*, base = u^n
+  store_vec<R, P>(out + i0, o[0]);
+}
+
+// ---------------------------------------------------------------------------------------------------------
 // Per-step kernel for the finite-volume Euler scheme, one INTERFACE per lane.  The generic kernel above lets every
 // thread rebuild the P+4 pressures and P+1 interface fluxes of its P cells (P = 2: three pressures and 1.5 fluxes
 // per cell, each flux with 8 divisions and 3 square roots).  Here lane l of a warp holds cell j = 28 w + l - 2,

@@ -254,6 +254,13 @@ int enqueue_steps(swept_state* s, int64_t steps, int threads, int P, int* cur_io
   for (int64_t i = 0; i < steps; ++i) {
     if (sigma == 1) {
       if (int rc = launch_per_step(s, s->slab[cur], s->slab[cur], s->slab[nxt], 0, threads, P)) return rc;
+    } else if (s->problem == SWEPT_KS && P >= 2) {
+      // both RK2 stages in one launch (north_star: "one launch per timestep or RK stage")
+      swept::PerStepLaunch a{s->slab[cur], s->slab[cur], s->slab[nxt], s->N, 0, threads, P, s->consts, s->stream, 0,
+                             nullptr};
+      const int rc = swept::launch_per_step_ks_fused(s->dtype, s->rk2, a);
+      if (rc == NO_KERNEL) return fail(SWEPT_EUNSUPPORTED, "no fused per-step kernel for P=%d", P);
+      if (rc != 0) return fail(SWEPT_ECUDA, "per-step launch: %s", cudaGetErrorString((cudaError_t)rc));
     } else {
       if (int rc = launch_per_step(s, s->slab[cur], s->slab[cur], s->slab[pred], 1, threads, P)) return rc;
       if (int rc = launch_per_step(s, s->slab[pred], s->slab[cur], s->slab[nxt], 0, threads, P)) return rc;
@@ -268,6 +275,7 @@ int run_per_step(swept_state* s, int64_t steps, int threads) {
   if (steps <= 0) return 0;
   const int sigma = kShape[s->problem].sigma;
   const int P = per_step_P(s);
+  const int lps = (s->problem == SWEPT_KS && P >= 2) ? 1 : sigma;  // launches per timestep (KS: fused stages)
   if (threads == 0) threads = 256;
   if (threads < 32 || threads > 1024 || (threads & (threads - 1)))
     return fail(SWEPT_EINVAL, "per-step tile_width (threads per block) must be a power of two in 32..1024");
@@ -300,13 +308,13 @@ int run_per_step(swept_state* s, int64_t steps, int threads) {
     }
     CUDA_TRY(cudaGraphLaunch(it->second, s->stream));
     left -= CH;  // CH even: s->cur unchanged
-    s->last_launches += CH * sigma;
+    s->last_launches += CH * lps;
   }
   if (left > 0) {
     int cur = s->cur;
     if (int rc = enqueue_steps(s, left, threads, P, &cur)) return rc;
     s->cur = cur;
-    s->last_launches += left * sigma;
+    s->last_launches += left * lps;
   }
   return 0;
 }

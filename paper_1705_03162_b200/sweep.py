@@ -28,7 +28,7 @@ import paper_1705_03162_b200 as sw  # noqa: E402
 FLAVOR_NAME = {sw.FLAVOR_TIER: "tier", sw.FLAVOR_CHAR: "char", sw.FLAVOR_FLOW: "flow"}
 # FP64-pipe instructions per point and timestep of the canonical expression trees
 FP64_INSTR = {sw.HEAT: 3, sw.KS: 22}
-BYTES_PER_STEP = {sw.HEAT: 16, sw.KS: 40, sw.EULER: 120}  # per-step algorithmic traffic, FP64
+BYTES_PER_STEP = {sw.HEAT: 16, sw.KS: 16, sw.EULER: 120}  # per-step algorithmic traffic, FP64
 
 
 def _time(torch, st, u0_dev, nsteps, n, variant, flavor, group, reps):
