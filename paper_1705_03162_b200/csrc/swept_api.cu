@@ -226,8 +226,7 @@ bool tile_ok(const swept_state* s, int flavor, int n, int P) {
   if (n <= 0 || s->N % n != 0) return false;
   // walls are applied by the TIER kernels; the CHAR flavour can run beside them on all other tiles (heat: hybrid)
   if (s->bc && flavor != SWEPT_FLAVOR_TIER && !(flavor == SWEPT_FLAVOR_CHAR && s->problem == SWEPT_HEAT)) return false;
-  if (s->bc && flavor == SWEPT_FLAVOR_CHAR && !swept::tile_config_ok_heat(s->dtype, SWEPT_FLAVOR_TIER, s->N, n,
-                                                                            n >= 1024 ? 4 : (n >= 512 ? 2 : 1)))
+  if (s->bc && flavor == SWEPT_FLAVOR_CHAR && !swept::tile_config_ok_heat(s->dtype, SWEPT_FLAVOR_TIER, s->N, n, 1))
     return false;
   if (flavor == SWEPT_FLAVOR_FLOW && (s->problem == SWEPT_EULER || P < 0 || P > 16)) return false;
   switch (s->problem) {
@@ -566,7 +565,11 @@ int run_swept(swept_state* s, int64_t nsteps, int n, int flavor, int P) {
       // stream beside the register-resident launch — the paper's Hybrid idea with a stream in
       // place of the CPU.  Both read the same input rows and write disjoint ranges of the output rows.
       if (!s->wall_stream) {
-        CUDA_TRY(cudaStreamCreateWithFlags(&s->wall_stream, cudaStreamNonBlocking));
+        // highest priority: the wall tile is one long latency chain and must not wait for a slot behind the
+        // register-resident launch, which fills the machine
+        int lo_prio = 0, hi_prio = 0;
+        CUDA_TRY(cudaDeviceGetStreamPriorityRange(&lo_prio, &hi_prio));
+        CUDA_TRY(cudaStreamCreateWithPriority(&s->wall_stream, cudaStreamNonBlocking, hi_prio));
         CUDA_TRY(cudaEventCreateWithFlags(&s->wall_fork, cudaEventDisableTiming));
         CUDA_TRY(cudaEventCreateWithFlags(&s->wall_join, cudaEventDisableTiming));
       }
@@ -574,25 +577,24 @@ int run_swept(swept_state* s, int64_t nsteps, int n, int flavor, int P) {
       CUDA_TRY(cudaStreamWaitEvent(s->wall_stream, s->wall_fork, 0));
       a.skip_first = ph.shift == 0 ? 1 : 0;
       a.skip_last = 1;
-    }
-    {
-      TimedScope ts(s, ph.kind, 1);
-      if (int rc = launch_tile(s, a)) return rc;
-    }
-    s->last_launches += 1;
-    if (hybrid) {
+      // wall tiles first, so that they are resident before the big launch takes every slot
       const int K = (int)(s->N / ph.n);
       swept::TileLaunch w = a;
       w.flavor = SWEPT_FLAVOR_TIER;
-      w.P = ph.n >= 1024 ? 4 : (ph.n >= 512 ? 2 : 1);
+      w.P = 1;  // one thread per point: the shortest tier latency (measured), and the wall tile is a latency chain
       w.skip_first = w.skip_last = 0;
       if (ph.shift == 0) { w.tile_base = 0; w.tile_step = K - 1; w.tile_count = K > 1 ? 2 : 1; }
       else { w.tile_base = K - 1; w.tile_step = 0; w.tile_count = 1; }
       if (int rc = launch_tile(s, w, s->wall_stream)) return rc;
       s->last_launches += 1;
       CUDA_TRY(cudaEventRecord(s->wall_join, s->wall_stream));
-      CUDA_TRY(cudaStreamWaitEvent(s->stream, s->wall_join, 0));
     }
+    {
+      TimedScope ts(s, ph.kind, 1);
+      if (int rc = launch_tile(s, a)) return rc;
+    }
+    s->last_launches += 1;
+    if (hybrid) CUDA_TRY(cudaStreamWaitEvent(s->stream, s->wall_join, 0));
     r0 = o0;
     r1 = o1;
     if (ph.kind == KIND_DOWN) s->cur = o0;  // row0 holds the full time level (T is even)
