@@ -112,6 +112,9 @@ def test_wide_tiles():
     check(w, 3000, [2048, 4096], flavors=((sw.FLAVOR_TIER, 4),))
     w = si.ks_cos(8192, 5, 700)
     check(w, 700, [2048, 4096], flavors=((sw.FLAVOR_TIER, 4),))
+    # Euler: the TIER kernel with shared pressures / fluxes, up to 1024 threads per tile
+    w = si.euler_double_sod(8192, 600)
+    check(w, 600, [1024, 2048], flavors=((sw.FLAVOR_TIER, 1), (sw.FLAVOR_TIER, 2), (sw.FLAVOR_TIER, 4)))
 
 
 @pytest.mark.parametrize("warps", [0, 1, 3])  # resident CTAs per SM (0 = default policy)
