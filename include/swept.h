@@ -46,10 +46,10 @@ enum { SWEPT_RK2_MIDPOINT = 0, SWEPT_RK2_HEUN = 1 };        /* KS/Euler integrat
 /* boundary conditions: periodic (all BASELINE.json configs) or the paper's own: insulated ends for heat,
  * Eq. (B.5), T_{-1} = T_1 and T_N = T_{N-2} for points 0..N-1; Dirichlet ends for the Euler
  * tube: cells -2, -1 and N, N+1 hold the states that swept_write found in the first and last
- * cell.  SWEPT_BC_PAPER is built for per-step (launch per sub-timestep), the swept TIER flavour, where the
+ * cell.  SWEPT_BC_PAPER is built for per-step (both flavours), the swept TIER flavour, where the
  * tile split across the boundary applies the condition at its centre, and for heat the CHAR
  * flavour in hybrid mode (wall tiles by the TIER kernels on a second stream); KS (periodic in
- * the paper), FLOW and SWEPT_PS_RESIDENT: SWEPT_EUNSUPPORTED. */
+ * the paper) and the FLOW flavour: SWEPT_EUNSUPPORTED. */
 enum { SWEPT_BC_PERIODIC = 0, SWEPT_BC_PAPER = 1 };
 enum { SWEPT_NKINDS = 6 };                                   /* phase kinds reported by swept_phase_times */
 enum { SWEPT_OK = 0, SWEPT_EINVAL = -1, SWEPT_EUNSUPPORTED = -2, SWEPT_ECUDA = -3, SWEPT_ENOMEM = -4 };

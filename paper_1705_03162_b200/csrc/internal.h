@@ -60,6 +60,8 @@ struct ResidentLaunch {
   void* xch;       // device scratch, resident_scratch_bytes() bytes, 16-byte aligned; first the flags
   const double* consts;
   cudaStream_t stream;
+  int bc = 0;      // kernel boundary mode (0 wrap, 1 mirror, 2 fixed end states)
+  const double* bcv = nullptr;
 };
 // scratch needed for at most `max_ctas` CTAs (flags + error word, then the exchange slots of the widest problem)
 // layout: one 128-byte line per CTA flag, one line for the error word, then 2 x max_ctas x 2 exchange lines

@@ -225,6 +225,8 @@ inline int resident_try(const ResidentLaunch& a, int threads, int pass) {
   r.in = (const R*)a.in; r.out = (R*)a.out; r.N = a.N; r.nsteps = a.nsteps;
   r.flags = (int*)a.xch;
   r.err = r.flags + RESIDENT_MAX_CTAS * 32;
+  r.bc = a.bc;
+  r.bv = round_bcvals<R>(a.bcv);
   r.xch = (R*)((char*)a.xch + resident_flag_bytes(RESIDENT_MAX_CTAS));
   r.k = round_consts<R>(a.consts);
   void* args[] = {&r};

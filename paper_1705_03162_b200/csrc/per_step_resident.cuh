@@ -29,6 +29,8 @@ struct ResidentArgs {
   R* xch;          // [2 parities][G CTAs][2 sides] slots of RS_LINE bytes, each holding [C][H] edge values
   int* flags;      // sub-steps published by CTA i at flags[i * RS_LINE / 4]; zero on entry
   int* err;        // error word: set if a neighbour wait timed out
+  int bc;          // BC_WRAP, BC_MIRROR (insulated heat ends) or BC_FIXED (Euler tube): applied by the two end threads
+  BcVals<R> bv;
   Consts<R> k;
 };
 
@@ -108,7 +110,10 @@ __global__ void __launch_bounds__(Prob::MAX_THREADS < 512 ? Prob::MAX_THREADS : 
 #pragma unroll
           for (int j = 0; j < P; ++j) win[c][H + j] = src[c][j];
         // left halo = last H points of the thread before, right halo = first H points of the thread after
-        const bool gl_left = tid == 0 && G > 1, gl_right = tid == t_last && G > 1;
+        // the two ends of the domain under a non-periodic boundary condition: no neighbour, the halo is the mirror
+        // image of the thread's own points (B.5) or the fixed end state
+        const bool wall_l = a.bc != BC_WRAP && g == 0, wall_r = a.bc != BC_WRAP && g == nthr - 1;
+        const bool gl_left = tid == 0 && G > 1 && !wall_l, gl_right = tid == t_last && G > 1 && !wall_r;
         if (gl_left || gl_right) {
           const int who = gl_left ? left_cta : right_cta;
           unsigned polls = 0;
@@ -128,6 +133,18 @@ __global__ void __launch_bounds__(Prob::MAX_THREADS < 512 ? Prob::MAX_THREADS : 
             win[c][e] = gl_left ? __ldcg(xslot(par, left_cta, 1, c, e)) : eslot(par, 1, c, e, tl);
             win[c][H + P + e] = gl_right ? __ldcg(xslot(par, right_cta, 0, c, e)) : eslot(par, 0, c, e, tr);
           }
+        if (wall_l) {
+#pragma unroll
+          for (int c = 0; c < C; ++c)
+#pragma unroll
+            for (int e = 0; e < H; ++e) win[c][e] = a.bc == BC_FIXED ? a.bv.l[c] : src[c][H - e];
+        }
+        if (wall_r) {
+#pragma unroll
+          for (int c = 0; c < C; ++c)
+#pragma unroll
+            for (int e = 0; e < H; ++e) win[c][H + P + e] = a.bc == BC_FIXED ? a.bv.r[c] : src[c][P - 2 - e];
+        }
         if (gl_left && gl_right) {  // one active thread in this CTA: it needs both neighbours
           unsigned polls = 0;
           while (rs_ld_acquire(a.flags + right_cta * (RS_LINE / 4)) < sub + 1 && ++polls < (1u << 22)) {}

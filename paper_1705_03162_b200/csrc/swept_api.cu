@@ -321,7 +321,6 @@ int run_per_step(swept_state* s, int64_t steps, int threads) {
 // ---- resident per-step: every sub-timestep in one persistent launch (per_step_resident.cuh) -----------
 int run_resident(swept_state* s, int64_t steps) {
   if (steps <= 0) return 0;
-  if (s->bc) return fail(SWEPT_EUNSUPPORTED, "the resident per-step flavour is periodic only");
   if (!s->resident_scratch) {
     CUDA_TRY(cudaMalloc(&s->resident_scratch, swept::resident_scratch_bytes(swept::RESIDENT_MAX_CTAS)));
     CUDA_TRY(cudaMemsetAsync(s->resident_scratch, 0, swept::resident_flag_bytes(swept::RESIDENT_MAX_CTAS), s->stream));
@@ -329,7 +328,8 @@ int run_resident(swept_state* s, int64_t steps) {
   // flags restart from zero every launch; the error word behind them is sticky until swept_read looks at it
   CUDA_TRY(cudaMemsetAsync(s->resident_scratch, 0, (size_t)swept::RESIDENT_MAX_CTAS * 128, s->stream));
   const int nxt = (s->cur + 1) & 3;
-  swept::ResidentLaunch a{s->slab[s->cur], s->slab[nxt], s->N, steps, s->resident_scratch, s->consts, s->stream};
+  swept::ResidentLaunch a{s->slab[s->cur], s->slab[nxt], s->N, steps, s->resident_scratch, s->consts, s->stream,
+                          s->kernel_bc(), s->bcvals};
   int rc;
   switch (s->problem) {
     case SWEPT_HEAT: rc = swept::launch_resident_heat(s->dtype, a); break;

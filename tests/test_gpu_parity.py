@@ -190,6 +190,8 @@ def test_heat_insulated_ends_bc_paper():
                 assert np.array_equal(sx, ref), ("swept", N, n, P)
         sx, _ = gpu_run(w, steps, sw.SWEPT)          # library default: must pick an admissible (TIER) configuration
         assert np.array_equal(sx, ref)
+        rs, _ = gpu_run(w, steps, sw.PER_STEP, 0, sw.PS_RESIDENT)   # launch-free per-step, walls at the two end threads
+        assert np.array_equal(rs, ref), ("resident", N)
     w = si.heat_insulated(2048, 4, 32, 300)
     assert np.array_equal(gpu_run(w, 300, sw.SWEPT, 128, dtype=np.float32)[0],
                           oracle.run_workload(w, dtype=np.float32))
@@ -211,8 +213,6 @@ def test_heat_insulated_ends_bc_paper():
     s = sw.Swept.from_workload(w)
     with pytest.raises(sw.SweptError):               # the persistent flavours are periodic only: clean error
         s.run(10, 256, sw.SWEPT, sw.FLAVOR_FLOW)
-    with pytest.raises(sw.SweptError):
-        s.run(10, 0, sw.PER_STEP, sw.PS_RESIDENT)
     best = s.autotune(sw.SWEPT)
     s.run(300, 0, sw.SWEPT)
     assert np.array_equal(s.read(), oracle.run_workload(w)) and best >= 32
@@ -241,6 +241,7 @@ def test_euler_dirichlet_ends_bc_paper(rk2):
                 assert np.array_equal(sx, ref), ("swept", N, n, P)
         assert ran >= 3
         assert np.array_equal(gpu_run(w, steps, sw.SWEPT)[0], ref)
+        assert np.array_equal(gpu_run(w, steps, sw.PER_STEP, 0, sw.PS_RESIDENT)[0], ref), ("resident", N)
 
 
 def test_per_step_non_power_of_two_N():
