@@ -97,20 +97,23 @@ swept_state* swept_create(int problem, int64_t N, double dx, double dt, const sw
  * memory makes the call synchronous).  Resets the step counter. */
 int swept_write(swept_state* s, const void* host_buf);
 
-/* swept_write_device — same, from DEVICE memory (device-to-device copy on the stream). */
+/* swept_write_device — same, from DEVICE memory (device-to-device copy on the stream).  With SWEPT_BC_PAPER on
+ * the Euler problem the end states are read back with small synchronous copies. */
 int swept_write_device(swept_state* s, const void* device_buf);
 
 /* swept_run — advance by nsteps full timesteps (PAPER.md:236 counts timesteps; KS/Euler timesteps have two
  * sub-timesteps).
  *   variant SWEPT_PER_STEP: tile_width = threads per block of the per-step kernel (32..1024, power of two;
- *                           0 = library default).
+ *                           0 = library default).  One launch per sub-timestep (heat, Euler) or per timestep
+ *                           with both RK2 stages fused (KS), replayed from a CUDA graph in chunks.
  *   variant SWEPT_SWEPT   : tile_width = n = spatial points per tile ("node"), a power of two,
  *                           32 <= n <= 4096 (the paper sweeps 32..1024), n >= 16 h for the
  *                           5-point problems, N % n == 0; 0 = autotuned / default value.
  *                           The run is Up, D diamonds, Down, covering the largest T = (D+1) n/(2h)
- *                           sub-timesteps that fit, and the remainder is finished with per-step stages
- *                           (readout granularity; reading G5).  If N has no admissible tile
- *                           the call fails with SWEPT_EUNSUPPORTED.
+ *                           sub-timesteps that fit; what is left runs further Up..Down cycles of width n/2,
+ *                           n/4, ... >= 32 and finally per-step stages (readout granularity, PAPER.md:83;
+ *                           reading G5).  If N has no admissible tile the call fails with
+ *                           SWEPT_EUNSUPPORTED.
  * Asynchronous on the state's stream; launch errors surface at the next synchronising call. */
 int swept_run(swept_state* s, int64_t nsteps, int32_t tile_width, int variant);
 
