@@ -89,7 +89,11 @@ typedef struct {
 /* swept_create — set up one problem: N periodic points, spacing dx, fixed timestep dt.
  * Scheme constants are computed once, in double, on the host (Fo = alpha dt/dx^2; etc.) and
  * rounded once to REAL.  p may be NULL (FP64, midpoint, alpha = 1, gamma = 1.4, current device).
- * Requires N >= 32 (and N >= 8 for per-step only use), dx > 0, dt > 0.  Returns NULL on error. */
+ * Requires 8 <= N <= 2^31, dx > 0, dt > 0 (the swept variant additionally needs N to hold at least one tile:
+ * N >= 32, see swept_run).  All device memory the state will ever use — four field slabs and the scratch of the
+ * persistent flavours — is allocated here, through p->alloc when given; creation may synchronise p->stream.
+ * p->stream = NULL means the CUDA legacy default stream (the Python binding passes torch's current stream and
+ * re-sets it with swept_set_stream before every call).  Returns NULL on error. */
 swept_state* swept_create(int problem, int64_t N, double dx, double dt, const swept_params* p);
 
 /* swept_write — copy initial data from HOST memory (C*N REALs, layout above) to the device, asynchronously
@@ -98,7 +102,8 @@ swept_state* swept_create(int problem, int64_t N, double dx, double dt, const sw
 int swept_write(swept_state* s, const void* host_buf);
 
 /* swept_write_device — same, from DEVICE memory (device-to-device copy on the stream).  With SWEPT_BC_PAPER on
- * the Euler problem the end states are read back with small synchronous copies. */
+ * the Euler problem the six end-state scalars are read back on the state's stream and the call synchronises it.
+ * (Both write calls: new Dirichlet end states discard the cached per-step CUDA graphs, which hold them.) */
 int swept_write_device(swept_state* s, const void* device_buf);
 
 /* swept_run — advance by nsteps full timesteps (PAPER.md:236 counts timesteps; KS/Euler timesteps have two
@@ -114,7 +119,10 @@ int swept_write_device(swept_state* s, const void* device_buf);
  *                           n/4, ... >= 32 and finally per-step stages (readout granularity, PAPER.md:83;
  *                           reading G5).  If N has no admissible tile the call fails with
  *                           SWEPT_EUNSUPPORTED.
- * Asynchronous on the state's stream; launch errors surface at the next synchronising call. */
+ * Asynchronous on the state's stream: the call enqueues kernels (and, the first time a 256-step per-step chunk is
+ * needed, records a CUDA graph on a private stream); it neither allocates device memory nor synchronises, so it
+ * may itself be captured into a CUDA graph.  Launch errors surface at the next synchronising call
+ * (swept_read, swept_sync, swept_phase_times, swept_autotune). */
 int swept_run(swept_state* s, int64_t nsteps, int32_t tile_width, int variant);
 
 /* per-step flavours */
@@ -135,6 +143,12 @@ int swept_run_flavor(swept_state* s, int64_t nsteps, int32_t tile_width, int var
  * swept_write).  Errors of the asynchronous launches since the last synchronising call surface here
  * (SWEPT_ECUDA), including a FLOW launch whose dependency wait timed out. */
 int swept_read(swept_state* s, void* host_buf);
+
+/* swept_sync — synchronise the state's stream and report what the asynchronous launches since the last
+ * synchronising call left behind: SWEPT_ECUDA if a persistent launch (FLOW, PS_RESIDENT) gave up waiting for a
+ * dependency — its tiles are then not stored and the field is invalid — else 0.  Callers that consume
+ * swept_device_ptr directly (no swept_read) use this to learn about such a failure. */
+int swept_sync(swept_state* s);
 
 /* swept_device_ptr — DEVICE pointer to the current full time level (C*N REALs), valid until the next
  * swept_run/swept_write on this state; stream-ordered (no synchronisation). */
@@ -164,7 +178,7 @@ int64_t swept_last_launches(const swept_state* s);
  * each kernel kind can be measured live, inside a timed region, without a profiler.  Off by default. */
 int swept_set_phase_timing(swept_state* s, int on);
 
-/* swept_phase_times — synchronise the stream and return, per phase kind (index 0 Up, 1 SplitDiamond,
+/* swept_phase_times — synchronise the stream (reporting failures like swept_sync) and return, per phase kind (index 0 Up, 1 SplitDiamond,
  * 2 WholeDiamond, 3 Down, 4 per-step remainder, 5 whole FLOW cycle), the summed device time in milliseconds
  * and the number of kernel launches recorded since timing was switched on or since the previous call; then
  * reset the record.  ms and launches are caller-owned HOST arrays of SWEPT_NKINDS (6) entries. */

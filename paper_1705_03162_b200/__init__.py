@@ -68,6 +68,7 @@ def load():
     lib.swept_run.argtypes = [c_void_p, c_int64, c_int32, c_int]
     lib.swept_run_flavor.argtypes = [c_void_p, c_int64, c_int32, c_int, c_int]
     lib.swept_read.argtypes = [c_void_p, c_void_p]
+    lib.swept_sync.argtypes = [c_void_p]
     lib.swept_device_ptr.restype = c_void_p
     lib.swept_device_ptr.argtypes = [c_void_p]
     lib.swept_autotune.argtypes = [c_void_p, c_int, POINTER(c_int32)]
@@ -164,6 +165,10 @@ def swept_read(state: int, host_buf: np.ndarray) -> None:
     _check(load().swept_read(state, host_buf.ctypes.data_as(c_void_p)))
 
 
+def swept_sync(state: int) -> None:
+    _check(load().swept_sync(state))
+
+
 def swept_autotune(state: int, variant: int) -> int:
     best = c_int32(0)
     _check(load().swept_autotune(state, variant, byref(best)))
@@ -256,6 +261,10 @@ class Swept:
         swept_set_stream(self._h, _current_stream())
         swept_read(self._h, out)
         return out
+
+    def sync(self) -> None:
+        swept_set_stream(self._h, _current_stream())
+        swept_sync(self._h)
 
     def autotune(self, variant: int = SWEPT) -> int:
         swept_set_stream(self._h, _current_stream())

@@ -45,8 +45,8 @@ struct FlowLaunch {
   void* buf[2][2];   // [buffer][row]; row r of the cycle writes buffer r & 1
   int64_t N;
   int n, rows;       // tile width; rows = D + 2
-  int* flags;        // rows * N/n ints, zeroed by the caller (stream-ordered)
-  unsigned* ticket;  // zeroed by the caller
+  int* flags;        // 2 * N/n words, zero (the kernel leaves them zero again; swept_flow.cuh)
+  unsigned* ticket;  // 4 words: task counter, sticky error word, leave counter, unused; counters zero
   int ctas_per_sm;   // resident CTAs (of 4 warps) per SM; 0 = default policy
   const double* consts;
   cudaStream_t stream;

@@ -91,7 +91,9 @@ struct swept_state {
   bool timing = false;
   std::vector<Timed> timed;
   std::vector<cudaEvent_t> event_pool;
-  // FLOW flavour scratch: ticket counter + one flag per tile of a cycle
+  // FLOW flavour scratch (allocated and zeroed by swept_create): word 0 = ticket counter, word 1 = sticky error
+  // word, word 2 = leave counter, words 4.. = 2 * N/256 flags (swept_flow.cuh).  Every launch leaves the counters
+  // and flags zero again, so nothing is cleared between launches.
   int* flow_scratch = nullptr;
   size_t flow_scratch_ints = 0;
   bool flow_pending_check = false;
@@ -142,25 +144,31 @@ int launch_tile(swept_state* s, swept::TileLaunch& a, cudaStream_t stream = null
   return 0;
 }
 
+// device memory through the caller's allocator hooks (swept_params.alloc / free), else cudaMalloc / cudaFree
+void* dev_alloc(swept_state* s, size_t bytes) {
+  void* ptr = nullptr;
+  if (s->alloc) return s->alloc(s->alloc_ctx, bytes);
+  if (cudaMalloc(&ptr, bytes) != cudaSuccess) {
+    cudaGetLastError();
+    return nullptr;
+  }
+  return ptr;
+}
+void dev_free(swept_state* s, void* ptr) {
+  if (!ptr) return;
+  if (s->free_) s->free_(s->alloc_ctx, ptr);
+  else cudaFree(ptr);
+}
+
+constexpr int FLOW_MIN_WIDTH = 256;  // narrowest tile of the FLOW flavour: sizes the flag array
+
 int launch_flow(swept_state* s, swept::FlowLaunch& a) {
   a.N = s->N;
   a.consts = s->consts;
   a.stream = s->stream;
-  const size_t need = (size_t)a.rows * (size_t)(s->N / a.n) + 4;
-  if (need > s->flow_scratch_ints) {
-    if (s->flow_scratch) {
-      CUDA_TRY(cudaStreamSynchronize(s->stream));
-      CUDA_TRY(cudaFree(s->flow_scratch));
-      s->flow_scratch = nullptr;
-      s->flow_scratch_ints = 0;
-    }
-    CUDA_TRY(cudaMalloc((void**)&s->flow_scratch, need * sizeof(int)));
-    s->flow_scratch_ints = need;
-    CUDA_TRY(cudaMemsetAsync(s->flow_scratch, 0, 4 * sizeof(int), s->stream));
-  }
-  // word 0 = ticket, word 1 = sticky error word (cleared when read), words 4.. = one flag per tile
-  CUDA_TRY(cudaMemsetAsync(s->flow_scratch, 0, sizeof(int), s->stream));
-  CUDA_TRY(cudaMemsetAsync(s->flow_scratch + 4, 0, (need - 4) * sizeof(int), s->stream));
+  const size_t need = 4 + 2 * (size_t)(s->N / a.n);
+  if (!s->flow_scratch || need > s->flow_scratch_ints)
+    return fail(SWEPT_EUNSUPPORTED, "no FLOW kernel for this problem / n=%d", a.n);
   a.ticket = (unsigned*)s->flow_scratch;
   a.flags = s->flow_scratch + 4;
   int rc;
@@ -189,8 +197,11 @@ int check_flow_error(swept_state* s) {
   s->flow_pending_check = false;
   int err = 0;
   CUDA_TRY(cudaMemcpy(&err, s->flow_scratch + 1, sizeof(int), cudaMemcpyDeviceToHost));
-  if (err) CUDA_TRY(cudaMemset(s->flow_scratch + 1, 0, sizeof(int)));
-  if (err) return fail(SWEPT_ECUDA, "FLOW kernel: a tile waited too long for its parents (grid not co-resident?)");
+  if (err) {
+    CUDA_TRY(cudaMemset(s->flow_scratch + 1, 0, sizeof(int)));
+    return fail(SWEPT_ECUDA, "FLOW kernel: a tile waited too long for its parents (grid not co-resident?); "
+                             "the field is invalid, write it again");
+  }
   return 0;
 }
 
@@ -228,7 +239,7 @@ bool tile_ok(const swept_state* s, int flavor, int n, int P) {
   if (s->bc && flavor != SWEPT_FLAVOR_TIER && !(flavor == SWEPT_FLAVOR_CHAR && s->problem == SWEPT_HEAT)) return false;
   if (s->bc && flavor == SWEPT_FLAVOR_CHAR && !swept::tile_config_ok_heat(s->dtype, SWEPT_FLAVOR_TIER, s->N, n, 1))
     return false;
-  if (flavor == SWEPT_FLAVOR_FLOW && (s->problem == SWEPT_EULER || P < 0 || P > 16)) return false;
+  if (flavor == SWEPT_FLAVOR_FLOW && (s->problem == SWEPT_EULER || P < 0 || P > 16 || !s->flow_scratch)) return false;
   switch (s->problem) {
     case SWEPT_HEAT: return swept::tile_config_ok_heat(s->dtype, flavor, s->N, n, P);
     case SWEPT_KS: return swept::tile_config_ok_ks(s->dtype, flavor, s->N, n, P);
@@ -321,10 +332,7 @@ int run_per_step(swept_state* s, int64_t steps, int threads) {
 // ---- resident per-step: every sub-timestep in one persistent launch (per_step_resident.cuh) -----------
 int run_resident(swept_state* s, int64_t steps) {
   if (steps <= 0) return 0;
-  if (!s->resident_scratch) {
-    CUDA_TRY(cudaMalloc(&s->resident_scratch, swept::resident_scratch_bytes(swept::RESIDENT_MAX_CTAS)));
-    CUDA_TRY(cudaMemsetAsync(s->resident_scratch, 0, swept::resident_flag_bytes(swept::RESIDENT_MAX_CTAS), s->stream));
-  }
+  if (!s->resident_scratch) return fail(SWEPT_EUNSUPPORTED, "no resident scratch (state creation failed to allocate it)");
   // flags restart from zero every launch; the error word behind them is sticky until swept_read looks at it
   CUDA_TRY(cudaMemsetAsync(s->resident_scratch, 0, (size_t)swept::RESIDENT_MAX_CTAS * 128, s->stream));
   const int nxt = (s->cur + 1) & 3;
@@ -564,15 +572,7 @@ int run_swept(swept_state* s, int64_t nsteps, int n, int flavor, int P) {
       // the boundary) go to the TIER kernels, which apply the boundary condition, on a second
       // stream beside the register-resident launch — the paper's Hybrid idea with a stream in
       // place of the CPU.  Both read the same input rows and write disjoint ranges of the output rows.
-      if (!s->wall_stream) {
-        // highest priority: the wall tile is one long latency chain and must not wait for a slot behind the
-        // register-resident launch, which fills the machine
-        int lo_prio = 0, hi_prio = 0;
-        CUDA_TRY(cudaDeviceGetStreamPriorityRange(&lo_prio, &hi_prio));
-        CUDA_TRY(cudaStreamCreateWithPriority(&s->wall_stream, cudaStreamNonBlocking, hi_prio));
-        CUDA_TRY(cudaEventCreateWithFlags(&s->wall_fork, cudaEventDisableTiming));
-        CUDA_TRY(cudaEventCreateWithFlags(&s->wall_join, cudaEventDisableTiming));
-      }
+      if (!s->wall_stream) return fail(SWEPT_ECUDA, "no wall stream (swept_create makes it for SWEPT_BC_PAPER heat)");
       CUDA_TRY(cudaEventRecord(s->wall_fork, s->stream));
       CUDA_TRY(cudaStreamWaitEvent(s->wall_stream, s->wall_fork, 0));
       a.skip_first = ph.shift == 0 ? 1 : 0;
@@ -680,25 +680,47 @@ swept_state* swept_create(int problem, int64_t N, double dx, double dt, const sw
   }
   s->slab_bytes = (size_t)kShape[problem].C * (size_t)N * s->elem();
   for (int i = 0; i < 4; ++i) {
-    void* ptr = nullptr;
-    if (s->alloc) {
-      ptr = s->alloc(s->alloc_ctx, s->slab_bytes);
-    } else if (cudaMalloc(&ptr, s->slab_bytes) != cudaSuccess) {
-      ptr = nullptr;
-      cudaGetLastError();
-    }
+    void* ptr = dev_alloc(s, s->slab_bytes);
     if (!ptr) {
       fail(SWEPT_ENOMEM, "device allocation of %zu bytes failed", s->slab_bytes);
       swept_destroy(s);
       return nullptr;
     }
+    s->slab[i] = ptr;
     if (((uintptr_t)ptr & 15) != 0) {
-      s->slab[i] = ptr;
       fail(SWEPT_EINVAL, "allocator returned a pointer that is not 16-byte aligned");
       swept_destroy(s);
       return nullptr;
     }
-    s->slab[i] = ptr;
+  }
+  // Scratch of the persistent flavours, sized here for the worst admissible plan so that swept_run never
+  // allocates or synchronises: FLOW (periodic heat / KS, N a multiple of its narrowest tile) needs a ticket word,
+  // a leave counter, an error word and 2 N/256 flags; PS_RESIDENT one flag line and two exchange lines per CTA.
+  cudaError_t e = cudaSuccess;
+  if (problem != SWEPT_EULER && q.bc == SWEPT_BC_PERIODIC && N % FLOW_MIN_WIDTH == 0) {
+    s->flow_scratch_ints = 4 + 2 * (size_t)(N / FLOW_MIN_WIDTH);
+    s->flow_scratch = (int*)dev_alloc(s, s->flow_scratch_ints * sizeof(int));
+    if (s->flow_scratch) e = cudaMemsetAsync(s->flow_scratch, 0, s->flow_scratch_ints * sizeof(int), s->stream);
+  }
+  s->resident_scratch = dev_alloc(s, swept::resident_scratch_bytes(swept::RESIDENT_MAX_CTAS));
+  if (s->resident_scratch && e == cudaSuccess)
+    e = cudaMemsetAsync(s->resident_scratch, 0, swept::resident_flag_bytes(swept::RESIDENT_MAX_CTAS), s->stream);
+  if (e == cudaSuccess && q.bc == SWEPT_BC_PAPER && problem == SWEPT_HEAT) {
+    // hybrid wall handling: the wall tiles run on a second, highest-priority stream — the wall
+    // tile is one long latency chain and must not wait for a slot behind the register-resident launch
+    int lo_prio = 0, hi_prio = 0;
+    e = cudaDeviceGetStreamPriorityRange(&lo_prio, &hi_prio);
+    if (e == cudaSuccess) e = cudaStreamCreateWithPriority(&s->wall_stream, cudaStreamNonBlocking, hi_prio);
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&s->wall_fork, cudaEventDisableTiming);
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&s->wall_join, cudaEventDisableTiming);
+  }
+  // the clears above must not race with a later swept_set_stream: finish them here (creation may synchronise)
+  if (e == cudaSuccess) e = cudaStreamSynchronize(s->stream);
+  if (e != cudaSuccess || !s->resident_scratch || (s->flow_scratch_ints && !s->flow_scratch)) {
+    if (e != cudaSuccess) fail(SWEPT_ECUDA, "swept_create: %s", cudaGetErrorString(e));
+    else fail(SWEPT_ENOMEM, "device allocation of the scratch buffers failed");
+    swept_destroy(s);
+    return nullptr;
   }
   return s;
 }
@@ -711,19 +733,15 @@ void swept_destroy(swept_state* s) {
   if (s->capture_stream) cudaStreamDestroy(s->capture_stream);
   for (auto& t : s->timed) { cudaEventDestroy(t.e0); cudaEventDestroy(t.e1); }
   for (cudaEvent_t e : s->event_pool) cudaEventDestroy(e);
-  if (s->flow_scratch) cudaFree(s->flow_scratch);
-  if (s->resident_scratch) cudaFree(s->resident_scratch);
+  dev_free(s, s->flow_scratch);
+  dev_free(s, s->resident_scratch);
   if (s->wall_stream) {
     cudaStreamSynchronize(s->wall_stream);
     cudaStreamDestroy(s->wall_stream);
-    cudaEventDestroy(s->wall_fork);
-    cudaEventDestroy(s->wall_join);
   }
-  for (int i = 0; i < 4; ++i) {
-    if (!s->slab[i]) continue;
-    if (s->free_) s->free_(s->alloc_ctx, s->slab[i]);
-    else cudaFree(s->slab[i]);
-  }
+  if (s->wall_fork) cudaEventDestroy(s->wall_fork);
+  if (s->wall_join) cudaEventDestroy(s->wall_join);
+  for (int i = 0; i < 4; ++i) dev_free(s, s->slab[i]);
   delete s;
 }
 
@@ -755,19 +773,41 @@ int swept_phase_times(swept_state* s, double* ms, int64_t* launches) {
   }
   s->timed.clear();
   cudaGetLastError();
+  return check_flow_error(s);
+}
+
+int swept_sync(swept_state* s) {
+  if (!s) return fail(SWEPT_EINVAL, "null state");
+  if (int rc = set_device(s)) return rc;
+  CUDA_TRY(cudaStreamSynchronize(s->stream));
+  return check_flow_error(s);
+}
+
+// Dirichlet end states of the Euler tube = the initial states of the first and last cell.  The
+// captured per-step graphs hold them as kernel arguments: new values invalidate the cache.
+static int set_end_states(swept_state* s, const double (&v)[6]) {
+  if (std::memcmp(s->bcvals, v, sizeof v) == 0) return 0;
+  std::memcpy(s->bcvals, v, sizeof v);
+  if (!s->graphs.empty()) {
+    CUDA_TRY(cudaStreamSynchronize(s->stream));  // a replay may still be in flight
+    for (auto& kv : s->graphs) cudaGraphExecDestroy(kv.second);
+    s->graphs.clear();
+  }
   return 0;
 }
 
 int swept_write(swept_state* s, const void* host_buf) {
   if (!s || !host_buf) return fail(SWEPT_EINVAL, "null argument");
   if (int rc = set_device(s)) return rc;
-  CUDA_TRY(cudaMemcpyAsync(s->slab[s->cur], host_buf, s->slab_bytes, cudaMemcpyHostToDevice, s->stream));
-  if (s->bc && s->problem == SWEPT_EULER) {  // Dirichlet ends = the initial states of the first and last cell
+  if (s->bc && s->problem == SWEPT_EULER) {
+    double v[6];
     for (int c = 0; c < 3; ++c) {
-      s->bcvals[c] = ((const double*)host_buf)[(size_t)c * s->N];
-      s->bcvals[3 + c] = ((const double*)host_buf)[(size_t)c * s->N + s->N - 1];
+      v[c] = ((const double*)host_buf)[(size_t)c * s->N];
+      v[3 + c] = ((const double*)host_buf)[(size_t)c * s->N + s->N - 1];
     }
+    if (int rc = set_end_states(s, v)) return rc;
   }
+  CUDA_TRY(cudaMemcpyAsync(s->slab[s->cur], host_buf, s->slab_bytes, cudaMemcpyHostToDevice, s->stream));
   s->steps_done = 0;
   return 0;
 }
@@ -775,14 +815,18 @@ int swept_write(swept_state* s, const void* host_buf) {
 int swept_write_device(swept_state* s, const void* device_buf) {
   if (!s || !device_buf) return fail(SWEPT_EINVAL, "null argument");
   if (int rc = set_device(s)) return rc;
-  CUDA_TRY(cudaMemcpyAsync(s->slab[s->cur], device_buf, s->slab_bytes, cudaMemcpyDeviceToDevice, s->stream));
-  if (s->bc && s->problem == SWEPT_EULER) {  // end states: two small synchronous copies per component
+  if (s->bc && s->problem == SWEPT_EULER) {
+    // end states: six scalars read back on the state's stream (ordered after whatever produced device_buf there)
+    double v[6];
     for (int c = 0; c < 3; ++c) {
       const double* d = (const double*)device_buf + (size_t)c * s->N;
-      CUDA_TRY(cudaMemcpy(&s->bcvals[c], d, sizeof(double), cudaMemcpyDeviceToHost));
-      CUDA_TRY(cudaMemcpy(&s->bcvals[3 + c], d + s->N - 1, sizeof(double), cudaMemcpyDeviceToHost));
+      CUDA_TRY(cudaMemcpyAsync(&v[c], d, sizeof(double), cudaMemcpyDeviceToHost, s->stream));
+      CUDA_TRY(cudaMemcpyAsync(&v[3 + c], d + s->N - 1, sizeof(double), cudaMemcpyDeviceToHost, s->stream));
     }
+    CUDA_TRY(cudaStreamSynchronize(s->stream));
+    if (int rc = set_end_states(s, v)) return rc;
   }
+  CUDA_TRY(cudaMemcpyAsync(s->slab[s->cur], device_buf, s->slab_bytes, cudaMemcpyDeviceToDevice, s->stream));
   s->steps_done = 0;
   return 0;
 }
@@ -858,13 +902,18 @@ int swept_autotune(swept_state* s, int variant, int32_t* best_tile_width) {
   if (int rc = set_device(s)) return rc;
   const ProblemShape sh = kShape[s->problem];
   // keep the field: the trial runs scribble over all four slabs
-  void* backup = nullptr;
-  CUDA_TRY(cudaMalloc(&backup, s->slab_bytes));
-  cudaMemcpyAsync(backup, s->slab[s->cur], s->slab_bytes, cudaMemcpyDeviceToDevice, s->stream);
+  void* backup = dev_alloc(s, s->slab_bytes);
+  if (!backup) return fail(SWEPT_ENOMEM, "autotune: device allocation of %zu bytes failed", s->slab_bytes);
   const int64_t saved_steps = s->steps_done;
-  cudaEvent_t e0, e1;
-  cudaEventCreate(&e0);
-  cudaEventCreate(&e1);
+  cudaEvent_t e0 = nullptr, e1 = nullptr;
+  int rc_final = 0;
+  // every CUDA call below is checked; the first failure ends the search, and the clean-up still runs
+  auto ok = [&](cudaError_t e, const char* what) {
+    if (e != cudaSuccess && !rc_final) rc_final = fail(SWEPT_ECUDA, "autotune: %s: %s", what, cudaGetErrorString(e));
+    return e == cudaSuccess;
+  };
+  ok(cudaMemcpyAsync(backup, s->slab[s->cur], s->slab_bytes, cudaMemcpyDeviceToDevice, s->stream), "backup copy");
+  ok(cudaEventCreate(&e0), "event") && ok(cudaEventCreate(&e1), "event");
   double best = 1e300;
   int best_n = 0, best_fl = 0, best_P = 0;
   struct Cand { int n, fl, P; };
@@ -880,33 +929,37 @@ int swept_autotune(swept_state* s, int variant, int32_t* best_tile_width) {
       for (int ctas : {1, 2, 3, 4, 6})  // resident CTAs per SM (clamped to the occupancy limit at launch)
         if (tile_ok(s, SWEPT_FLAVOR_FLOW, n, ctas)) cands.push_back({n, SWEPT_FLAVOR_FLOW, ctas});
   }
-  int rc_final = 0;
   for (const Cand& c : cands) {
+    if (rc_final) break;
     // enough steps for Up + 14 diamonds + Down at this width, so that the Up/Down rows and the start-up of a
     // persistent FLOW launch weigh as little as in a long run (and a few graph chunks for per-step)
     int64_t steps;
     if (variant == SWEPT_PER_STEP) steps = 512;
     else steps = std::max<int64_t>(16 * (c.n / (2 * sh.h)) / sh.sigma, 64);
     double t_best = 1e300;
-    for (int rep = 0; rep < 3; ++rep) {  // rep 0 warms up (graph capture, attribute setting)
-      cudaMemcpyAsync(s->slab[s->cur], backup, s->slab_bytes, cudaMemcpyDeviceToDevice, s->stream);
-      cudaEventRecord(e0, s->stream);
+    for (int rep = 0; rep < 3 && !rc_final; ++rep) {  // rep 0 warms up (graph capture, attribute setting)
+      if (!ok(cudaMemcpyAsync(s->slab[s->cur], backup, s->slab_bytes, cudaMemcpyDeviceToDevice, s->stream), "restore") ||
+          !ok(cudaEventRecord(e0, s->stream), "event record"))
+        break;
       int rc = variant == SWEPT_PER_STEP ? run_per_step(s, steps, c.n) : run_swept(s, steps, c.n, c.fl, c.P);
-      cudaEventRecord(e1, s->stream);
       if (rc) { rc_final = rc; break; }
-      if (cudaEventSynchronize(e1) != cudaSuccess) { rc_final = fail(SWEPT_ECUDA, "autotune trial failed: %s", cudaGetErrorString(cudaGetLastError())); break; }
+      if (!ok(cudaEventRecord(e1, s->stream), "event record") || !ok(cudaEventSynchronize(e1), "trial run")) break;
+      if (int rc2 = check_flow_error(s)) { rc_final = rc2; break; }
       float ms = 0;
-      cudaEventElapsedTime(&ms, e0, e1);
+      if (!ok(cudaEventElapsedTime(&ms, e0, e1), "event time")) break;
       if (rep > 0) t_best = std::min(t_best, (double)ms / (double)steps);
     }
-    if (rc_final) break;
-    if (t_best < best) { best = t_best; best_n = c.n; best_fl = c.fl; best_P = c.P; }
+    if (!rc_final && t_best < best) { best = t_best; best_n = c.n; best_fl = c.fl; best_P = c.P; }
   }
-  cudaMemcpyAsync(s->slab[s->cur], backup, s->slab_bytes, cudaMemcpyDeviceToDevice, s->stream);
-  cudaStreamSynchronize(s->stream);
-  cudaFree(backup);
-  cudaEventDestroy(e0);
-  cudaEventDestroy(e1);
+  // restore the field whatever happened (keep the first error)
+  {
+    cudaError_t e = cudaMemcpyAsync(s->slab[s->cur], backup, s->slab_bytes, cudaMemcpyDeviceToDevice, s->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(s->stream);
+    ok(e, "restoring the field");
+  }
+  dev_free(s, backup);
+  if (e0) cudaEventDestroy(e0);
+  if (e1) cudaEventDestroy(e1);
   s->steps_done = saved_steps;
   if (rc_final) return rc_final;
   if (best_n == 0) return fail(SWEPT_EUNSUPPORTED, "no admissible tile width for N=%lld", (long long)s->N);

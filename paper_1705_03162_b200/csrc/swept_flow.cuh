@@ -39,8 +39,13 @@ struct FlowArgs {
   int64_t N;
   int K;          // tiles per row = N / n
   int rows;       // D + 2
-  int* flags;     // rows * K, zero on entry; flags[r * K + k] = 1 once tile (r, k) is in global memory
-  unsigned* ticket;  // zero on entry; ticket[1] is an error word (set if a dependency wait timed out)
+  int* flags;     // 2 * K words, zero on entry: flags[(r & 1) * K + k] = r + 1 once tile (r, k) is in global memory.
+                  // Reusing the slot two rows later is safe: tile (r+2, k) cannot finish before both children of
+                  // tile (r, k) — the only readers of its flag — have finished.
+  unsigned* ticket;  // ticket[0] = task counter, ticket[2] = warps that have left; both zero on entry.  The last
+                     // warp to leave clears them and the flags again, so a launch needs no host-side reset and a
+                     // captured launch can be replayed.  ticket[1] = sticky error word (a dependency wait timed
+                     // out), read and cleared by the host.
   Consts<R> k;
 };
 
@@ -107,18 +112,25 @@ __global__ void __launch_bounds__(128) swept_flow_kernel(const FlowArgs<typename
       // parents: the tiles of row r-1 overlapping [S, S+n)
       const int p0 = (r & 1) ? k : (k == 0 ? a.K - 1 : k - 1);
       const int p1 = (r & 1) ? (k + 1 == a.K ? 0 : k + 1) : k;
-      const int* f = a.flags + (size_t)(r - 1) * a.K;
+      const int* f = a.flags + (size_t)((r - 1) & 1) * a.K;
+      const int want = r;  // row r-1 publishes (r-1) + 1
       unsigned ns = 32, polls = 0;
-      while (ld_relaxed_gpu(f + p0) == 0 || ld_relaxed_gpu(f + p1) == 0) {
+      bool dead = false;
+      while (ld_relaxed_gpu(f + p0) < want || ld_relaxed_gpu(f + p1) < want) {
         __nanosleep(ns);
         if (ns < FLOW_MAX_SLEEP) ns *= 2;
         // cannot happen while the grid is co-resident; bounded so that a scheduling surprise yields an error
-        // code (swept_read reports it) instead of a hung device: 2^22 polls x >= 2 us
-        if (++polls > (1u << 22)) {
+        // code (the next synchronising call reports it) instead of a hung device: 2^22 polls x >= 0.25 us.
+        // A warp that gives up raises the sticky error word; every other waiting warp sees it and leaves too,
+        // and nobody stores a tile computed from unready inputs.
+        ++polls;
+        if (polls > (1u << 22) || ((polls & 255u) == 0 && ld_relaxed_gpu((const int*)a.ticket + 1) != 0)) {
           if (lane == 0) atomicExch(a.ticket + 1, 1u);
+          dead = true;
           break;
         }
       }
+      if (dead) break;
       fence_acq_rel_gpu();
     }
     // ---- stage the tile: both rows over [S-h, S+n+h) (Up: row 0 of the initial level, no halo)
@@ -161,9 +173,21 @@ __global__ void __launch_bounds__(128) swept_flow_kernel(const FlowArgs<typename
     __syncwarp();
     if (lane == 0) {
       __threadfence();
-      st_release_gpu(a.flags + t, 1);
+      st_release_gpu(a.flags + (size_t)(r & 1) * a.K + k, r + 1);
     }
     __syncwarp();  // the slice is reused by the next task of this warp
+  }
+  // Leave the scratch as it was found.  A warp arrives here after its last task is in global memory; the warp that
+  // arrives last therefore knows that every task of the launch is done.
+  unsigned gone = 0;
+  if (lane == 0) gone = atomicAdd(a.ticket + 2, 1u);
+  gone = __shfl_sync(0xffffffffu, gone, 0);
+  if (gone == gridDim.x * (blockDim.x >> 5) - 1) {
+    for (int i = lane; i < 2 * a.K; i += 32) a.flags[i] = 0;
+    if (lane == 0) {
+      a.ticket[2] = 0;
+      a.ticket[0] = 0;
+    }
   }
 }
 

@@ -36,11 +36,62 @@ def gpu_run(w, nsteps, variant, tile_width=0, flavor=sw.FLAVOR_AUTO, group=0, dt
 
 
 CHAR = tuple((sw.FLAVOR_CHAR, L) for L in (8, 16, 32))
-FLOW = ((sw.FLAVOR_FLOW, 0),)   # heat / KS, n in {256, 512, 1024}; "not admissible" elsewhere
+FLOW = ((sw.FLAVOR_FLOW, 0),)   # heat / KS, n in {256, 512, 1024}
 TIER12 = ((sw.FLAVOR_TIER, 1), (sw.FLAVOR_TIER, 2))
 
 
-def check(w, nsteps, tile_widths, dtype=np.float64, flavors=((sw.FLAVOR_TIER, 0),) + CHAR + FLOW, exact=True):
+def admissible(w, n, flavor, group, dtype=np.float64):
+    """Which (tile width, flavour, group) the library must accept for workload `w` — the rules of include/swept.h and
+    DESIGN.md §5, restated here independently of the library, so that a regression which makes a flavour
+    inadmissible (or silently admits one it has no kernel for) fails the tests instead of being skipped."""
+    N, problem, bc = w.N, w.problem, getattr(w, "bc", 0)
+    h, _, C = si.PROBLEM_SHAPE[problem]
+    size = np.dtype(dtype).itemsize
+    if n < 32 or n & (n - 1) or N % n:
+        return False
+    if flavor == sw.FLAVOR_TIER:  # one CTA per tile, P points per thread, rows (+ Euler pressures/fluxes) in shared memory
+        P = group
+        if P == 0:
+            P = (1 if n <= 256 else 2 if n <= 2048 else 4) if problem == si.EULER else \
+                {32: 1, 64: 1, 128: 1, 256: 1, 512: 2, 1024: 4, 2048: 4, 4096: 4}.get(n, 0)
+        row = (n + 4 * (16 // size)) * size
+        smem = 2 * C * row + 16 + (4 * row if problem == si.EULER else 0)
+        return n <= 4096 and P in (1, 2, 4) and 8 <= n // P <= 1024 and smem <= 227 * 1024
+    if flavor == sw.FLAVOR_CHAR:  # L lanes per tile, B = n/L lines per lane in registers, 32 or 64 threads per CTA
+        if bc and not (problem == si.HEAT and n <= 1024):  # walls: hybrid with TIER wall tiles, heat only
+            return False
+        Ls = (group,) if group else (32, 16, 8)
+        for L in Ls:
+            if L not in (8, 16, 32) or n % L:
+                continue
+            B = n // L
+            if B not in ((4, 8, 16, 32) if h == 1 else (8, 16, 32)) or B > (16 if problem == si.EULER else 32):
+                continue
+            T = 64 if N % (64 * B) == 0 else 32 if N % (32 * B) == 0 else 0
+            if T >= L:
+                return True
+        return False
+    if flavor == sw.FLAVOR_FLOW:  # persistent launch: periodic heat / KS, 32 lanes per tile, B = n/32 in {8, 16, 32}
+        return problem != si.EULER and not bc and n in (256, 512, 1024) and N % 256 == 0 and group <= 16
+    raise ValueError(flavor)
+
+
+def run_or_refusal(w, nsteps, n, fl, grp, dtype=np.float64):
+    """The swept result, or None when the library refuses the configuration — and it must refuse exactly the
+    inadmissible ones (no silent skip: the expected set is `admissible`)."""
+    want = admissible(w, n, fl, grp, dtype)
+    try:
+        sx, _ = gpu_run(w, nsteps, sw.SWEPT, n, fl, grp, dtype=dtype)
+    except sw.SweptError as e:
+        assert not want, f"library refused an admissible configuration (n={n}, flavor={fl}, group={grp}): {e}"
+        assert "not admissible" in str(e) or "no FLOW kernel" in str(e), str(e)
+        return None
+    assert want, f"library ran a configuration this table calls inadmissible (n={n}, flavor={fl}, group={grp})"
+    return sx
+
+
+def check(w, nsteps, tile_widths, dtype=np.float64, flavors=((sw.FLAVOR_TIER, 0),) + CHAR + FLOW, exact=True,
+          min_ran=None):
     C = w.components
     ref = oracle.run_workload(w, nsteps=nsteps, dtype=dtype)
     ps, _ = gpu_run(w, nsteps, sw.PER_STEP, dtype=dtype)
@@ -49,19 +100,19 @@ def check(w, nsteps, tile_widths, dtype=np.float64, flavors=((sw.FLAVOR_TIER, 0)
     assert relerr(ps, ref, C) <= tol, f"per_step vs oracle: {relerr(ps, ref, C)}"
     if exact:
         assert np.array_equal(ps, ref), "same expression trees: expected 0 ulp"
-    ran = 0
+    ran = []
     for n in tile_widths:
         for fl, grp in flavors:
-            try:
-                sx, _ = gpu_run(w, nsteps, sw.SWEPT, n, fl, grp, dtype=dtype)
-            except sw.SweptError as e:
-                if "not admissible" in str(e) or "no FLOW kernel" in str(e):  # e.g. CHAR needs n/L in {8,16,32}
-                    continue
-                raise
-            ran += 1
+            sx = run_or_refusal(w, nsteps, n, fl, grp, dtype)
+            if sx is None:
+                continue
+            ran.append((n, fl, grp))
             assert np.array_equal(sx, ps), f"swept(n={n}, flavor={fl}, group={grp}) != per_step bitwise"
             assert relerr(sx, ref, C) <= tol
-    assert ran >= min(1, len(tile_widths)), "no swept configuration was admissible"
+    expected = [(n, fl, grp) for n in tile_widths for fl, grp in flavors if admissible(w, n, fl, grp, dtype)]
+    assert ran == expected
+    if min_ran is not None:  # the caller's own count of what this case is meant to exercise
+        assert len(ran) >= min_ran, (len(ran), min_ran)
     return ran
 
 
@@ -182,12 +233,9 @@ def test_heat_insulated_ends_bc_paper():
             if N % n:
                 continue
             for P in (1, 2, 4):
-                try:
-                    sx, _ = gpu_run(w, steps, sw.SWEPT, n, sw.FLAVOR_TIER, P)
-                except sw.SweptError as e:
-                    assert "not admissible" in str(e)
-                    continue
-                assert np.array_equal(sx, ref), ("swept", N, n, P)
+                sx = run_or_refusal(w, steps, n, sw.FLAVOR_TIER, P)
+                if sx is not None:
+                    assert np.array_equal(sx, ref), ("swept", N, n, P)
         sx, _ = gpu_run(w, steps, sw.SWEPT)          # library default: must pick an admissible (TIER) configuration
         assert np.array_equal(sx, ref)
         rs, _ = gpu_run(w, steps, sw.PER_STEP, 0, sw.PS_RESIDENT)   # launch-free per-step, walls at the two end threads
@@ -202,14 +250,12 @@ def test_heat_insulated_ends_bc_paper():
         ran = 0
         for n in (64, 256, 512, 1024):
             for L in (8, 16, 32):
-                try:
-                    sx, _ = gpu_run(w2, steps, sw.SWEPT, n, sw.FLAVOR_CHAR, L)
-                except sw.SweptError as e:
-                    assert "not admissible" in str(e)
+                sx = run_or_refusal(w2, steps, n, sw.FLAVOR_CHAR, L)
+                if sx is None:
                     continue
                 ran += 1
                 assert np.array_equal(sx, ref2), ("hybrid", N, n, L)
-        assert ran >= 4
+        assert ran == sum(admissible(w2, n, sw.FLAVOR_CHAR, L) for n in (64, 256, 512, 1024) for L in (8, 16, 32)) >= 8
     s = sw.Swept.from_workload(w)
     with pytest.raises(sw.SweptError):               # the persistent flavours are periodic only: clean error
         s.run(10, 256, sw.SWEPT, sw.FLAVOR_FLOW)
@@ -232,16 +278,84 @@ def test_euler_dirichlet_ends_bc_paper(rk2):
         ran = 0
         for n in (32, 128, 512):
             for P in (1, 2):
-                try:
-                    sx, _ = gpu_run(w, steps, sw.SWEPT, n, sw.FLAVOR_TIER, P)
-                except sw.SweptError as e:   # n > N, or more than 256 threads for the Euler functor
-                    assert "not admissible" in str(e)
+                sx = run_or_refusal(w, steps, n, sw.FLAVOR_TIER, P)   # refused only where n > N
+                if sx is None:
                     continue
                 ran += 1
                 assert np.array_equal(sx, ref), ("swept", N, n, P)
-        assert ran >= 3
+        assert ran == 2 * sum(1 for n in (32, 128, 512) if n <= N) >= 4
         assert np.array_equal(gpu_run(w, steps, sw.SWEPT)[0], ref)
         assert np.array_equal(gpu_run(w, steps, sw.PER_STEP, 0, sw.PS_RESIDENT)[0], ref), ("resident", N)
+
+
+def test_euler_dirichlet_rewrite_discards_cached_graphs():
+    # The per-step CUDA graphs hold the Dirichlet end states as kernel arguments: writing a field with other end
+    # states must not replay graphs captured for the old ones.  300 steps = one 256-step graph + 44 launches
+    wA = si.euler_sod(2048, 300)
+    wB = si.euler_sod(2048, 300)
+    N = wB.N
+    u = wB.u0.reshape(3, N).copy()
+    u[0, : N // 2] *= 1.5          # other left state (density, energy) ...
+    u[2, : N // 2] *= 1.25
+    u[0, N // 2:] *= 0.8           # ... and other right state
+    wB.u0 = u.reshape(-1)
+    s = sw.Swept.from_workload(wA)
+    s.run(300, 0, sw.PER_STEP)
+    assert np.array_equal(s.read(), oracle.run_workload(wA))
+    s.write(wB.u0)
+    s.run(300, 0, sw.PER_STEP)
+    assert np.array_equal(s.read(), oracle.run_workload(wB))
+    s.write(wA.u0)                 # and back, through the device-to-device entry point
+    import torch
+    dev = torch.from_numpy(wA.u0).cuda()
+    sw.load().swept_write_device(s._h, dev.data_ptr())
+    s.run(300, 0, sw.PER_STEP)
+    s.run(300, 128, sw.SWEPT)
+    assert np.array_equal(s.read(), oracle.run_workload(wA, nsteps=600))
+    s.close()
+
+
+def test_swept_run_neither_allocates_nor_synchronises():
+    # "swept_run never synchronises", device memory comes from the allocator hooks at creation.
+    # Proof by capture: under a GLOBAL-mode stream capture any cudaMalloc / cudaFree / synchronisation made by the
+    # capturing thread is an error that invalidates the capture.  Each variant is recorded into a CUDA graph,
+    # replayed and checked against the oracle; a last case replays twice (the persistent launch must leave its
+    # scratch as it found it).
+    import torch
+    w = si.heat_sines(1 << 14, 8, 2, 0)
+    wk = si.ks_cos(1 << 13, 4, 0)
+    wb = si.heat_insulated(1 << 13, 4, 5, 0)
+    cases = [(w, sw.SWEPT, 256, sw.FLAVOR_FLOW, 0, 128 * 6 + 20), (w, sw.SWEPT, 256, sw.FLAVOR_CHAR, 32, 128 * 3 + 5),
+             (w, sw.SWEPT, 64, sw.FLAVOR_TIER, 1, 200), (w, sw.SWEPT, 0, sw.FLAVOR_AUTO, 0, 500),
+             (wk, sw.SWEPT, 256, sw.FLAVOR_FLOW, 0, 150), (wk, sw.PER_STEP, 0, sw.PS_LAUNCH, 0, 70),
+             (wb, sw.SWEPT, 256, sw.FLAVOR_CHAR, 32, 300),          # hybrid: wall tiles on the second stream
+             (w, sw.PER_STEP, 0, sw.PS_LAUNCH, 0, 100), (w, sw.PER_STEP, 0, sw.PS_RESIDENT, 0, 60)]
+    for wl, variant, n, fl, grp, steps in cases:
+        s = sw.Swept.from_workload(wl)
+        torch.cuda.synchronize()
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g, capture_error_mode="global"):
+            s.run(steps, n, variant, fl, grp)
+        assert s.last_launches >= 1
+        g.replay()
+        got = s.read()
+        assert np.array_equal(got, oracle.run_workload(wl, nsteps=steps)), (wl.name, variant, n, fl)
+        s.close()
+    # replay-safety of the FLOW scratch proper: capture write + run together, replay twice
+    s = sw.Swept.from_workload(w)
+    dev = torch.from_numpy(w.u0).cuda()
+    torch.cuda.synchronize()
+    g = torch.cuda.CUDAGraph()
+    lib = sw.load()
+    with torch.cuda.graph(g, capture_error_mode="global"):
+        sw.swept_set_stream(s._h, int(torch.cuda.current_stream().cuda_stream))
+        assert lib.swept_write_device(s._h, dev.data_ptr()) == 0
+        s.run(128 * 4, 256, sw.SWEPT, sw.FLAVOR_FLOW)
+    ref = oracle.run_workload(w, nsteps=512)
+    for _ in range(2):
+        g.replay()
+        assert np.array_equal(s.read(), ref)
+    s.close()
 
 
 def test_per_step_non_power_of_two_N():
@@ -395,12 +509,9 @@ def test_config5_sampled_grid():
                 assert np.array_equal(ps, oracle.run_workload(w, nsteps=steps))
             for n in (32, 128, 512, 1024):
                 for fl, grp in ((sw.FLAVOR_TIER, 0), (sw.FLAVOR_CHAR, 16), (sw.FLAVOR_CHAR, 32), (sw.FLAVOR_FLOW, 0)):
-                    try:
-                        sx, _ = gpu_run(w, steps, sw.SWEPT, n, fl, grp)
-                    except sw.SweptError as e:
-                        assert "not admissible" in str(e) or "no FLOW kernel" in str(e)
-                        continue
-                    assert np.array_equal(ps, sx), (problem, N, n, fl, grp)
+                    sx = run_or_refusal(w, steps, n, fl, grp)
+                    if sx is not None:
+                        assert np.array_equal(ps, sx), (problem, N, n, fl, grp)
 
 
 def test_autotune_picks_admissible_width_and_keeps_state():

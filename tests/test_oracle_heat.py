@@ -102,6 +102,80 @@ def test_p6_rational_brute_force():
     assert np.max(np.abs(got - np.array([float(x) for x in u]))) < 8 * np.finfo(float).eps
 
 
+# ---- FP32 instantiation (the checker of north_star's 1e-5 gate, reading X15): pinned to the BIT, not to "close to FP64"
+def round_to_binary32(fr):
+    """Nearest-even rounding of an exact rational to IEEE binary32 (normal range), by integer arithmetic."""
+    fr = Fraction(fr)
+    if fr == 0:
+        return np.float32(0.0)
+    sign, a = (-1 if fr < 0 else 1), abs(fr)
+    e = a.numerator.bit_length() - a.denominator.bit_length()
+    if Fraction(2) ** e > a:
+        e -= 1
+    assert Fraction(2) ** e <= a < Fraction(2) ** (e + 1) and -126 <= e <= 127
+    q = a / Fraction(2) ** (e - 23)          # in [2^23, 2^24)
+    n = q.numerator // q.denominator
+    rem = q - n
+    if rem > Fraction(1, 2) or (rem == Fraction(1, 2) and n % 2 == 1):
+        n += 1
+    return np.float32(sign * float(Fraction(n) * Fraction(2) ** (e - 23)))   # exact in double, exact in float
+
+
+@pytest.mark.parametrize("N", [5, 8, 16])
+@pytest.mark.parametrize("s", [1, 2, 7, 11])
+def test_p2_delta_binomial_bit_exact_fp32(N, s):
+    # C(2s, s+j) < 2^24 for s <= 11 (and every partial sum of a step is such a dyadic), so binary32 is exact too
+    pos = 2
+    u0 = np.zeros(N, dtype=np.float32)
+    u0[pos] = 1.0
+    dx = 1.0 / N
+    u = oracle.run(oracle.HEAT, u0, N, s, dx, 0.25 * dx * dx, dtype=np.float32)
+    exp = np.zeros(N)
+    for j in range(-s, s + 1):
+        exp[(pos + j) % N] += comb(2 * s, s + j) / 4.0 ** s
+    assert u.dtype == np.float32 and np.array_equal(u.astype(np.float64), exp)
+
+
+def test_p3_nyquist_and_constant_exact_fp32():
+    N = 32
+    dx = 1.0 / N
+    ny = ((-1.0) ** np.arange(N)).astype(np.float32)
+    assert np.array_equal(oracle.run(oracle.HEAT, ny, N, 1, dx, 0.25 * dx * dx, dtype=np.float32), np.zeros(N, np.float32))
+    const = np.full(N, 0.3, dtype=np.float32)
+    assert np.array_equal(oracle.run(oracle.HEAT, const, N, 100, dx, 0.25 * dx * dx, dtype=np.float32), const)
+
+
+def test_p6_fp32_rational_and_bit_level_emulation():
+    # Eq. (B.4) with r != 2^-k on 11 points, three steps, float data:
+    # (a) against the exact rational value of B.4 applied to the float inputs with the once-rounded constants:
+    #     within a few binary32 ulps — a wrong sign, term, index or a constant built from rounded pieces fails;
+    # (b) bit for bit against B.4 evaluated with correctly rounded binary32 operations built from integer
+    #     arithmetic (sum, product, ONE rounding for the fused multiply-add, SURVEY.md §8(c) F-heat): a double
+    #     intermediate, a missing fusion or a twice-rounded constant in the float instantiation fails.
+    rng = np.random.default_rng(12)
+    N, steps = 11, 3
+    u0 = rng.uniform(-1, 1, N).astype(np.float32)
+    alpha, dx = 0.7, 0.1
+    dt = 0.3 * dx * dx / alpha
+    Fo_d = alpha * dt / (dx * dx)                       # double, as the F-rules say; rounded ONCE to float
+    Fo, c0 = Fraction(float(np.float32(Fo_d))), Fraction(float(np.float32(1.0 - 2.0 * Fo_d)))
+    exact = [Fraction(float(x)) for x in u0]
+    emu = [Fraction(float(x)) for x in u0]
+    for _ in range(steps):
+        exact = [Fo * (exact[(i + 1) % N] + exact[(i - 1) % N]) + c0 * exact[i] for i in range(N)]
+        nxt = []
+        for i in range(N):
+            ssum = Fraction(float(round_to_binary32(emu[(i - 1) % N] + emu[(i + 1) % N])))
+            t = Fraction(float(round_to_binary32(c0 * emu[i])))
+            nxt.append(Fraction(float(round_to_binary32(Fo * ssum + t))))
+        emu = nxt
+    got = oracle.run(oracle.HEAT, u0, N, steps, dx, dt, alpha=alpha, dtype=np.float32)
+    assert got.dtype == np.float32
+    ulp = np.finfo(np.float32).eps
+    assert np.max(np.abs(got.astype(np.float64) - np.array([float(x) for x in exact]))) < 6 * ulp
+    assert np.array_equal(got.astype(np.float64), np.array([float(x) for x in emu]))
+
+
 def test_fp32_instantiation_tracks_fp64():
     w = si.heat_sines(256, 16, 3, 200)
     u64 = oracle.run_workload(w)
