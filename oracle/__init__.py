@@ -23,7 +23,7 @@ _LIB = os.path.join(_HERE, "libswept_oracle.so")
 _lock = threading.Lock()
 _lib = None
 
-HEAT, KS, EULER = 0, 1, 2
+HEAT, KS, EULER, KS3 = 0, 1, 2, 3   # KS3: Eq. (C.2) with three sub-timesteps per timestep (SSP-RK3, row f3)
 RK2_MIDPOINT, RK2_HEUN = 0, 1
 
 
@@ -55,6 +55,7 @@ def _load():
         lib.oracle_euler_bc_f64.argtypes = [vp, i64, i64, dbl, dbl, dbl, ci]
         lib.oracle_ks_f64.argtypes = [vp, i64, i64, dbl, dbl, ci]
         lib.oracle_ks_f32.argtypes = [vp, i64, i64, dbl, dbl, ci]
+        lib.oracle_ks3_f64.argtypes = [vp, i64, i64, dbl, dbl]
         lib.oracle_euler_f64.argtypes = [vp, i64, i64, dbl, dbl, dbl, ci]
         lib.oracle_euler_f32.argtypes = [vp, i64, i64, dbl, dbl, dbl, ci]
         lib.oracle_set_num_threads.argtypes = [ci]
@@ -89,6 +90,12 @@ def run(problem: int, u0: np.ndarray, N: int, nsteps: int, dx: float, dt: float,
         raise ValueError(f"expected {C * N} values, got {u.size}")
     sfx = "f64" if dtype == np.float64 else "f32"
     ptr = u.ctypes.data_as(ctypes.c_void_p)
+    if problem == KS3:
+        if bc or dtype != np.float64:
+            raise ValueError("KS3 is periodic and FP64 only")
+        if lib.oracle_ks3_f64(ptr, N, nsteps, dx, dt) != 0:
+            raise ValueError("oracle rejected the arguments")
+        return u
     if bc and (problem == KS or (problem == EULER and dtype != np.float64)):
         raise ValueError("non-periodic ends exist for heat (B.5) and FP64 Euler (PAPER.md:377) only")
     if problem == HEAT:

@@ -15,6 +15,8 @@
 //           Eqs. (C.3)-(C.4) PAPER.md:348-354 (App. C)                 — 5-point, 2 stages / step
 //   Euler : 2nd-order finite volume, Eqs. (D.3)-(D.12) PAPER.md:366-416,
 //           RK2 "with the same procedure" as (C.3)-(C.4), PAPER.md:418 — 5-point, 2 stages / step
+//   KS3   : Eq. (C.2) advanced by the three-stage Shu-Osher SSP-RK3 (row f3: "more than two
+//           sub-timesteps per timestep")                  — 5-point, 3 stages / step
 //
 // Readings of garbled / silent / ambiguous passages (all listed in DESIGN.md §3):
 //   X1  (D.12) update is Q - dt/dx (F_{i+1/2} - F_{i-1/2}) (conservation law D.1).
@@ -140,6 +142,53 @@ void ks_run(R* u, int64_t N, int64_t nsteps, double dx, double dt, int rk2) {
                 const R t = std::fma(-k.dt, ks_rhs(p, i, N, k), p[i]);
                 b[i] = (R)0.5 * (a[i] + t);
             }
+        }
+        R* tmp = a; a = b; b = tmp;
+    }
+    if (a != u) std::memcpy(u, a, sizeof(R) * (size_t)N);
+}
+
+// ---------------------------------------------------------------- KS with THREE sub-timesteps per timestep
+// SURVEY.md §8(f) row f3.  The paper stops at two sub-timesteps per timestep and says the decomposition "must be
+// adjusted ... when there are more than two sub-timesteps per timestep" and "adjusted further" beyond four
+// (PAPER.md:103-115 on sub-timesteps that all use the minimum stencil).  The scheme taken for that
+// row: the same spatial discretisation (C.2) advanced by the three-stage strong-stability-preserving Runge-Kutta
+// method of Shu and Osher (a textbook scheme, not in the paper), every stage on the same 5-point stencil:
+//     u1      = u^n + dt f(u^n)
+//     u2      = 3/4 u^n + 1/4 (u1 + dt f(u1))
+//     u^{n+1} = 1/3 u^n + 2/3 (u2 + dt f(u2))
+// Stage s reads the previous stage on the stencil and u^n at its own point (s-1 sub-timesteps back): with three
+// sub-timesteps the paper's two-row working array would have overwritten it (the conflict of PAPER.md Fig. 3).
+// Canonical trees:  e = fma(-dt, rhs(v), v) with rhs of F-KS;  stage 1: e;  stage 2: fma(1/4, e, (3/4) u^n);
+// stage 3: fma(c23, e, c13 u^n) with c13 = REAL(1.0/3.0), c23 = REAL(2.0/3.0) (rounded once, like every constant).
+// Pins: tests/test_oracle_ks3.py (growth polynomial 1 + z + z^2/2 + z^3/6, third-order convergence in dt,
+// conservation of the mean, PDE consistency, exact-rational hand expansion).
+template <class R>
+void ks3_run(R* u, int64_t N, int64_t nsteps, double dx, double dt) {
+    KSConst<R> k;
+    k.cx = (R)(1.0 / (4.0 * dx));
+    k.cxx = (R)(1.0 / (dx * dx));
+    k.cxxxx = (R)(1.0 / ((dx * dx) * (dx * dx)));
+    k.dt = (R)dt;
+    k.half_dt = (R)(0.5 * dt);
+    const R c14 = (R)0.25, c34 = (R)0.75, c13 = (R)(1.0 / 3.0), c23 = (R)(2.0 / 3.0);
+    std::vector<R> s1((size_t)N), s2((size_t)N), un((size_t)N);
+    R* a = u;
+    R* b = un.data();
+    R* p = s1.data();
+    R* q = s2.data();
+    for (int64_t s = 0; s < nsteps; ++s) {
+#pragma omp parallel for schedule(static) if (N >= OMP_MIN_N)
+        for (int64_t i = 0; i < N; ++i) p[i] = std::fma(-k.dt, ks_rhs(a, i, N, k), a[i]);
+#pragma omp parallel for schedule(static) if (N >= OMP_MIN_N)
+        for (int64_t i = 0; i < N; ++i) {
+            const R e = std::fma(-k.dt, ks_rhs(p, i, N, k), p[i]);
+            q[i] = std::fma(c14, e, c34 * a[i]);
+        }
+#pragma omp parallel for schedule(static) if (N >= OMP_MIN_N)
+        for (int64_t i = 0; i < N; ++i) {
+            const R e = std::fma(-k.dt, ks_rhs(q, i, N, k), q[i]);
+            b[i] = std::fma(c23, e, c13 * a[i]);
         }
         R* tmp = a; a = b; b = tmp;
     }
@@ -336,6 +385,12 @@ int oracle_ks_f64(double* u, int64_t N, int64_t nsteps, double dx, double dt, in
 int oracle_ks_f32(float* u, int64_t N, int64_t nsteps, double dx, double dt, int rk2) {
     if (!u || N < 5 || nsteps < 0) return -1;
     ks_run<float>(u, N, nsteps, dx, dt, rk2);
+    return 0;
+}
+// KS, three sub-timesteps per timestep (SSP-RK3)
+int oracle_ks3_f64(double* u, int64_t N, int64_t nsteps, double dx, double dt) {
+    if (!u || N < 5 || nsteps < 0) return -1;
+    ks3_run<double>(u, N, nsteps, dx, dt);
     return 0;
 }
 int oracle_euler_f64(double* q, int64_t N, int64_t nsteps, double dx, double dt, double gamma,

@@ -21,11 +21,12 @@ import numpy as np
 
 BASE_SEED = 170503162
 
-HEAT, KS, EULER = 0, 1, 2
+HEAT, KS, EULER, KS3 = 0, 1, 2, 3
 RK2_MIDPOINT, RK2_HEUN = 0, 1
-PROBLEM_NAMES = {HEAT: "heat", KS: "ks", EULER: "euler"}
+PROBLEM_NAMES = {HEAT: "heat", KS: "ks", EULER: "euler", KS3: "ks3"}
 #: stencil half-width h, sub-timesteps per timestep sigma, components C
-PROBLEM_SHAPE = {HEAT: (1, 1, 1), KS: (2, 2, 1), EULER: (2, 2, 3)}
+#: (KS3 = the KS discretisation advanced with three sub-timesteps per timestep)
+PROBLEM_SHAPE = {HEAT: (1, 1, 1), KS: (2, 2, 1), EULER: (2, 2, 3), KS3: (2, 3, 1)}
 
 
 @dataclass
@@ -94,6 +95,15 @@ def ks_cos(N: int, seed: int, nsteps: int, dx: float = 0.5, dt: float = 0.005,
     x = np.arange(N, dtype=np.float64) * dx
     u0 = np.cos(x / 16.0) * (1.0 + np.sin(x / 16.0)) + noise * rng.standard_normal(N)
     return Workload(KS, N, dx, dt, nsteps, u0, rk2=RK2_MIDPOINT, name=name or f"ks_N{N}")
+
+
+def ks3_cos(N: int, seed: int, nsteps: int, dx: float = 0.5, dt: float = 0.005, noise: float = 1e-3,
+            name: str = "") -> Workload:
+    """Row f3 (a scheme with three sub-timesteps per timestep): config 3's KS field and steps, advanced with the
+    three-stage SSP Runge-Kutta method instead of the midpoint rule."""
+    w = ks_cos(N, seed, nsteps, dx, dt, noise, name or f"ks3_N{N}")
+    w.problem = KS3
+    return w
 
 
 def euler_double_sod(N: int, nsteps: int, rk2: int = RK2_HEUN, gamma: float = 1.4,
