@@ -9,8 +9,11 @@
 //   win [c][k], k = 0 .. P+2H-1 : stage input (tier t-1) at points x0-H .. x0+P-1+H, component c
 //   base[c][j], j = 0 .. P-1    : value at tier t-2 (= u^n) for the final stage; for the predictor
 //                                 stage the caller passes the window centre (tier t-1 = u^n)
-//   odd                         : 1 = predictor sub-timestep (odd tier), 0 = final sub-timestep
-//                                 (odd tiers hold predictor values, even tiers final values)
+//   odd                         : global tier index modulo SIGMA.  Two-stage schemes: 1 = predictor sub-timestep
+//                                 (odd tier), 0 = final sub-timestep (odd tiers hold predictor
+//                                 values, even tiers final values).  Three-stage scheme (KS3): 1, 2 = first and
+//                                 second stage, 0 = final stage.  base is u^n whenever odd != 1.
+//   ROWS                        : rows of the inter-launch state (tier modulo ROWS); u^n lives in row 0
 #pragma once
 #include <cuda_runtime.h>
 #include <math.h>
@@ -50,7 +53,7 @@ struct BcVals {
 template <class R_>
 struct Heat {
   using R = R_;
-  static constexpr int H = 1, C = 1, SIGMA = 1;
+  static constexpr int H = 1, C = 1, SIGMA = 1, ROWS = 2;
   static constexpr int MAX_THREADS = 1024;  // per CTA, for __launch_bounds__ (register budget)
   static constexpr int TIER_MAX_THREADS = 1024;
   __device__ __forceinline__ static R point(R um, R u0, R up, const Consts<R>& k) {
@@ -72,7 +75,7 @@ struct Heat {
 template <class R_, int HEUN>
 struct KS {
   using R = R_;
-  static constexpr int H = 2, C = 1, SIGMA = 2;
+  static constexpr int H = 2, C = 1, SIGMA = 2, ROWS = 2;
   static constexpr int MAX_THREADS = 1024;
   static constexpr int TIER_MAX_THREADS = 1024;
   __device__ __forceinline__ static R rhs(R vm2, R vm1, R v0, R vp1, R vp2, const Consts<R>& k) {
@@ -107,12 +110,41 @@ struct KS {
 };
 
 // ---------------------------------------------------------------------------------------------
+// KS3 — a scheme with THREE sub-timesteps per timestep (the decomposition
+// "must be adjusted ... when there are more than two sub-timesteps per timestep"): Eq. (C.2) advanced by the
+// three-stage Shu-Osher SSP Runge-Kutta method, every stage on the same 5-point stencil,
+//     u1 = u^n + dt f(u^n);   u2 = 3/4 u^n + 1/4 (u1 + dt f(u1));   u^{n+1} = 1/3 u^n + 2/3 (u2 + dt f(u2)).
+// The final stage reads u^n three tiers back, which the paper's two-row working array has overwritten by then
+// (Fig. 3): the state has ROWS = 3 rows (tier modulo 3), u^n in row 0.   Constants as KS (a3 = dt).
+template <class R_>
+struct KS3 {
+  using R = R_;
+  static constexpr int H = 2, C = 1, SIGMA = 3, ROWS = 3;
+  static constexpr int MAX_THREADS = 1024;
+  static constexpr int TIER_MAX_THREADS = 1024;
+  __device__ __forceinline__ static R point(R vm2, R vm1, R v0, R vp1, R vp2, R base, int st, const Consts<R>& k) {
+    const R f = KS<R, 0>::rhs(vm2, vm1, v0, vp1, vp2, k);
+    const R e = fma_(-k.a3, f, v0);                                   // v + dt f(v)
+    if (st == 1) return e;
+    if (st == 2) return fma_((R)0.25, e, (R)0.75 * base);
+    return fma_((R)(2.0 / 3.0), e, (R)(1.0 / 3.0) * base);
+  }
+  template <int P>
+  __device__ __forceinline__ static void stage(const R (&win)[C][P + 2 * H], const R (&base)[C][P],
+                                               R (&out)[C][P], int st, const Consts<R>& k) {
+#pragma unroll
+    for (int j = 0; j < P; ++j)
+      out[0][j] = point(win[0][j], win[0][j + 1], win[0][j + 2], win[0][j + 3], win[0][j + 4], base[0][j], st, k);
+  }
+};
+
+// ---------------------------------------------------------------------------------------------
 // Euler, second-order finite volume, Eqs. (D.3)-(D.12) PAPER.md:366-416 (readings X1, X3, X4, X5).
 //   a0 = gamma - 1, a1 = gamma (gamma - 1), a2 = dt/dx, a3 = dt/(2dx)
 template <class R_, int HEUN>
 struct Euler {
   using R = R_;
-  static constexpr int H = 2, C = 3, SIGMA = 2;
+  static constexpr int H = 2, C = 3, SIGMA = 2, ROWS = 2;
   static constexpr int MAX_THREADS = 256;  // ~250 live registers per thread (P:270 'greater low-level memory usage')
   static constexpr int TIER_MAX_THREADS = 1024;  // the TIER kernel shares pressures and fluxes: 64 registers
 

@@ -47,7 +47,7 @@ struct FlowLaunch {
   int n, rows;       // tile width; rows = D + 2
   int* flags;        // 2 * N/n words, zero (the kernel leaves them zero again; swept_flow.cuh)
   unsigned* ticket;  // 4 words: task counter, sticky error word, leave counter, unused; counters zero
-  int ctas_per_sm;   // resident CTAs (of 4 warps) per SM; 0 = default policy
+  int ctas_per_sm;   // bits 0..3: resident CTAs (of 4 warps) per SM, 0 = default policy; bit 4: TMA staging
   const double* consts;
   cudaStream_t stream;
 };

@@ -1,7 +1,7 @@
 // kernels_euler.cu — Euler equations / Sod tube (App. D) host dispatch, FP64.
 // The swept kernels themselves are instantiated in kernels_euler_inst.cu, compiled once per
 // (flavour, integrator) slice so that the slices build in parallel (see build.py).
-#include "kernels_impl.cuh"
+#include "kernels_persist_impl.cuh"
 namespace swept {
 extern template int tier_T<Euler<double, 0>, 4>(const TileLaunch&);
 extern template int tier_T<Euler<double, 1>, 4>(const TileLaunch&);

@@ -1,5 +1,5 @@
 // kernels_heat.cu — heat equation (App. B) kernel instantiations, FP64 and FP32.
-#include "kernels_impl.cuh"
+#include "kernels_persist_impl.cuh"
 namespace swept {
 int launch_per_step_heat(int dtype, const PerStepLaunch& a) {
   return dtype == 0 ? per_step_T<Heat<double>, 4>(a) : per_step_T<Heat<float>, 4>(a);

@@ -1,5 +1,5 @@
 // kernels_ks.cu — Kuramoto-Sivashinsky (App. C) kernel instantiations, FP64.
-#include "kernels_impl.cuh"
+#include "kernels_persist_impl.cuh"
 namespace swept {
 int launch_per_step_ks(int dtype, int rk2, const PerStepLaunch& a) {
   if (dtype != 0) return NO_KERNEL;

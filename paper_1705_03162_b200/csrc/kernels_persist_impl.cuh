@@ -1,0 +1,118 @@
+// kernels_persist_impl.cuh — host launchers of the two persistent flavours (PS_RESIDENT, FLOW), kept apart from
+// kernels_impl.cuh so that the slow Euler swept-kernel slices (kernels_euler_inst.cu) do not depend on them.
+#pragma once
+#include "kernels_impl.cuh"
+#include "per_step_resident.cuh"
+#include "swept_flow.cuh"
+
+namespace swept {
+
+// ---- resident per-step: one cooperative launch, the field in registers ---------------------------------
+template <class Prob, int P>
+inline int resident_try(const ResidentLaunch& a, int threads, int pass) {
+  using R = typename Prob::R;
+  if (a.N % P) return NO_KERNEL;
+  const int64_t nthr = a.N / P;
+  if (nthr < threads) threads = (int)((nthr + 31) / 32 * 32);
+  const int64_t G = (nthr + threads - 1) / threads;
+  auto kern = per_step_resident_kernel<Prob, P>;
+  const size_t smem = resident_smem_bytes<Prob>(threads);
+  int dev = 0, sms = 0, occ = 0;
+  cudaGetDevice(&dev);
+  cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+  if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, threads, smem) != cudaSuccess || occ < 1) {
+    cudaGetLastError();
+    return NO_KERNEL;
+  }
+  // pass 0: a single CTA (no global exchange at all); 1: one CTA per SM; 2: any co-resident grid
+  if (G > RESIDENT_MAX_CTAS || G > (pass == 0 ? 1 : (int64_t)sms * (pass == 1 ? 1 : occ))) return NO_KERNEL;
+  ResidentArgs<R> r;
+  r.in = (const R*)a.in; r.out = (R*)a.out; r.N = a.N; r.nsteps = a.nsteps;
+  r.flags = (int*)a.xch;
+  r.err = r.flags + RESIDENT_MAX_CTAS * 32;
+  r.bc = a.bc;
+  r.bv = round_bcvals<R>(a.bcv);
+  r.xch = (R*)((char*)a.xch + resident_flag_bytes(RESIDENT_MAX_CTAS));
+  r.k = round_consts<R>(a.consts);
+  void* args[] = {&r};
+  return (int)cudaLaunchCooperativeKernel((const void*)kern, dim3((unsigned)G), dim3((unsigned)threads), args, smem,
+                                          a.stream);
+}
+
+// smallest P (most lanes busy per point) whose grid fits one CTA per SM, else any co-resident grid
+template <class Prob, int PMAX>
+int resident_T(const ResidentLaunch& a) {
+  constexpr int TMAX = Prob::MAX_THREADS < 512 ? Prob::MAX_THREADS : 512;
+  for (int pass = 0; pass < 3; ++pass) {
+    int rc = NO_KERNEL;
+    if (rc == NO_KERNEL && Prob::H <= 2 && PMAX >= 2) rc = resident_try<Prob, 2>(a, TMAX, pass);
+    if (rc == NO_KERNEL && PMAX >= 4) rc = resident_try<Prob, (PMAX >= 4 ? 4 : 2)>(a, TMAX, pass);
+    if (rc == NO_KERNEL && PMAX >= 8) rc = resident_try<Prob, (PMAX >= 8 ? 8 : 2)>(a, TMAX, pass);
+    if (rc == NO_KERNEL && PMAX >= 16) rc = resident_try<Prob, (PMAX >= 16 ? 16 : 2)>(a, TMAX, pass);
+    if (rc != NO_KERNEL) return rc;
+  }
+  return NO_KERNEL;
+}
+
+// ---- FLOW flavour: persistent launch, L = 32 lanes per tile, B = n / 32 lines per lane -----------------
+template <class Prob, int BMAX>
+inline bool flow_ok(int64_t N, int n) {
+  if (n % 32 || N % n) return false;
+  const int B = n / 32;
+  if (B != 8 && B != 16 && B != 32) return false;
+  return B <= BMAX && B % (2 * Prob::H) == 0 && n / (2 * Prob::H) >= 32;
+}
+
+template <class Prob, int B, bool TMA>
+inline int flow_go(const FlowLaunch& a) {
+  using R = typename Prob::R;
+  constexpr int warps = 4;  // one per scheduler
+  constexpr int threads = warps * 32;
+  FlowArgs<R> f;
+  f.init = (const R*)a.init;
+  for (int i = 0; i < 2; ++i)
+    for (int j = 0; j < 2; ++j) f.buf[i][j] = (R*)a.buf[i][j];
+  f.N = a.N; f.K = (int)(a.N / a.n); f.rows = a.rows; f.flags = a.flags; f.ticket = a.ticket;
+  f.k = round_consts<R>(a.consts);
+  const size_t smem = flow_smem_bytes<Prob>(warps, a.n);
+  auto kern = swept_flow_kernel<Prob, B, TMA>;
+  cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  if (e != cudaSuccess) return (int)e;
+  // never launch more CTAs than can be co-resident: waiting tasks must not keep their parents off the machine
+  int dev = 0, sms = 0, occ = 0;
+  cudaGetDevice(&dev);
+  cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+  e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, threads, smem);
+  if (e != cudaSuccess) return (int)e;
+  if (occ < 1) return (int)cudaErrorLaunchOutOfResources;
+  const int64_t ntasks = (int64_t)f.rows * f.K;
+  // Resident warps.  All warps run at the same pace, so the tile a warp takes next has its parents still in
+  // flight when the resident warps span a whole row (K tiles): waiting warps then only poll.  Default: about
+  // 7/8 K warps for the 3-point problem, K/2 for the 5-point ones (their tiles have more parallelism inside a
+  // warp and more registers); `ctas_per_sm` (autotuned) overrides.
+  int64_t per_sm = a.ctas_per_sm & 15;
+  if (per_sm <= 0) {
+    const int64_t want = (Prob::H == 1 ? (int64_t)f.K * 7 / 8 : (int64_t)f.K / 2) / warps;  // CTAs
+    per_sm = (want + sms / 2) / sms;
+  }
+  if (per_sm < 1) per_sm = 1;
+  if (per_sm > occ) per_sm = occ;
+  int64_t grid = per_sm * sms;
+  if (grid > (ntasks + warps - 1) / warps) grid = (ntasks + warps - 1) / warps;
+  kern<<<(unsigned)grid, threads, smem, a.stream>>>(f);
+  return (int)cudaGetLastError();
+}
+
+template <class Prob, int BMAX>
+int flow_T(const FlowLaunch& a) {
+  if (!flow_ok<Prob, BMAX>(a.N, a.n)) return NO_KERNEL;
+  const bool tma = (a.ctas_per_sm & 16) != 0;  // group bit 4: stage the tiles with TMA bulk copies
+  switch (a.n / 32) {
+    case 8: return tma ? flow_go<Prob, 8, true>(a) : flow_go<Prob, 8, false>(a);
+    case 16: if (BMAX >= 16) return tma ? flow_go<Prob, (BMAX >= 16 ? 16 : 8), true>(a) : flow_go<Prob, (BMAX >= 16 ? 16 : 8), false>(a); break;
+    case 32: if (BMAX >= 32) return tma ? flow_go<Prob, (BMAX >= 32 ? 32 : 8), true>(a) : flow_go<Prob, (BMAX >= 32 ? 32 : 8), false>(a); break;
+  }
+  return NO_KERNEL;
+}
+
+}  // namespace swept

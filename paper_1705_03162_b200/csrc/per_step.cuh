@@ -38,7 +38,8 @@ __device__ __forceinline__ void store_vec(R* __restrict__ p, const R (&v)[P]) {
   }
 }
 
-// in: stage input (tier t-1), base: tier t-2 field (only read when SIGMA == 2 and !odd), out: tier t.
+// in: stage input (tier t-1), base: u^n (only read by the stages after the first: SIGMA >= 2 and odd != 1), out: tier t.
+// odd = tier modulo SIGMA (functors.cuh).
 template <class Prob, int P>
 __global__ void __launch_bounds__(Prob::MAX_THREADS)
 per_step_kernel(const typename Prob::R* __restrict__ in, const typename Prob::R* __restrict__ base,
@@ -69,7 +70,7 @@ per_step_kernel(const typename Prob::R* __restrict__ in, const typename Prob::R*
       win[c][H + P + j] = fix_r ? bv.r[c] : __ldg(src + ir);
     }
   }
-  if (Prob::SIGMA == 2 && !odd) {
+  if (Prob::SIGMA >= 2 && odd != 1) {
 #pragma unroll
     for (int c = 0; c < C; ++c) load_vec<R, P>(base + (int64_t)c * N + i0, bs[c]);
   } else {

@@ -239,7 +239,7 @@ bool tile_ok(const swept_state* s, int flavor, int n, int P) {
   if (s->bc && flavor != SWEPT_FLAVOR_TIER && !(flavor == SWEPT_FLAVOR_CHAR && s->problem == SWEPT_HEAT)) return false;
   if (s->bc && flavor == SWEPT_FLAVOR_CHAR && !swept::tile_config_ok_heat(s->dtype, SWEPT_FLAVOR_TIER, s->N, n, 1))
     return false;
-  if (flavor == SWEPT_FLAVOR_FLOW && (s->problem == SWEPT_EULER || P < 0 || P > 16 || !s->flow_scratch)) return false;
+  if (flavor == SWEPT_FLAVOR_FLOW && (s->problem == SWEPT_EULER || P < 0 || (P & 15) > 12 || P > 31 || !s->flow_scratch)) return false;
   switch (s->problem) {
     case SWEPT_HEAT: return swept::tile_config_ok_heat(s->dtype, flavor, s->N, n, P);
     case SWEPT_KS: return swept::tile_config_ok_ks(s->dtype, flavor, s->N, n, P);
@@ -927,7 +927,8 @@ int swept_autotune(swept_state* s, int variant, int32_t* best_tile_width) {
           if (tile_ok(s, fl, n, P)) cands.push_back({n, fl, P});
     for (int n : {256, 512, 1024})
       for (int ctas : {1, 2, 3, 4, 6})  // resident CTAs per SM (clamped to the occupancy limit at launch)
-        if (tile_ok(s, SWEPT_FLAVOR_FLOW, n, ctas)) cands.push_back({n, SWEPT_FLAVOR_FLOW, ctas});
+        for (int tma : {0, 16})         // generic 16-byte copies, or TMA bulk copies (group bit 4)
+          if (tile_ok(s, SWEPT_FLAVOR_FLOW, n, ctas | tma)) cands.push_back({n, SWEPT_FLAVOR_FLOW, ctas | tma});
   }
   for (const Cand& c : cands) {
     if (rc_final) break;

@@ -42,6 +42,32 @@ __device__ __forceinline__ float shfl_up_<float>(float v, int width) {
   return __shfl_up_sync(0xffffffffu, v, 1, width);
 }
 
+// Predicated shared-memory access of the two I/O lanes of a group with an immediate byte offset from one running
+// 32-bit shared address.  Written in PTX so that the load lands in the very register the shuffle filled (the
+// tied "+" operand: no select, no move) and the address arithmetic stays out of the loop.
+template <int OFF> __device__ __forceinline__ void lds_tied(double& x, uint32_t addr) {
+  asm volatile("ld.volatile.shared.f64 %0, [%1+%2];" : "+d"(x) : "r"(addr), "n"(OFF) : "memory");
+}
+template <int OFF> __device__ __forceinline__ void lds_tied(float& x, uint32_t addr) {
+  asm volatile("ld.volatile.shared.f32 %0, [%1+%2];" : "+f"(x) : "r"(addr), "n"(OFF) : "memory");
+}
+template <int OFF> __device__ __forceinline__ void sts_imm(uint32_t addr, double x) {
+  asm volatile("st.volatile.shared.f64 [%0+%1], %2;" ::"r"(addr), "n"(OFF), "d"(x) : "memory");
+}
+template <int OFF> __device__ __forceinline__ void sts_imm(uint32_t addr, float x) {
+  asm volatile("st.volatile.shared.f32 [%0+%1], %2;" ::"r"(addr), "n"(OFF), "f"(x) : "memory");
+}
+// scheme constants pinned in registers: the compiler otherwise reloads them from the constant bank inside the
+// sweep loop (two LDC per pair of steps)
+__device__ __forceinline__ void pin_reg(double& x) { asm volatile("" : "+d"(x)); }
+__device__ __forceinline__ void pin_reg(float& x) { asm volatile("" : "+f"(x)); }
+template <class R>
+__device__ __forceinline__ Consts<R> pinned_consts(const Consts<R>& k) {
+  Consts<R> r = k;
+  pin_reg(r.a0); pin_reg(r.a1); pin_reg(r.a2); pin_reg(r.a3); pin_reg(r.a4);
+  return r;
+}
+
 // Advance the B lines of one lane by one super-column `sc` (0 <= sc < m): 2h sub-columns (p mod 2h fixed), each a
 // dependent chain of B/2h points.  hal = the 2h lines below the lane's block after the neighbour's super-column
 // sc, halp = the same one super-column earlier (own-point-two-tiers-back operand of the first chain links).
@@ -85,12 +111,18 @@ __device__ __forceinline__ void char_update_lines(typename Prob::R (&v)[Prob::C]
 // One super-step of a lane: fetch the 2h-line halo (shuffle, or the staged edge for group lane 0), update the
 // B lines of this lane (2h sub-columns, each a dependent chain of B/2h points), stream the top lines out
 // (group lane L-1).  GUARD = some lanes of the warp are outside their m super-columns (ramp up / down).
-template <class Prob, int B, int L, int KIND, bool GUARD>
+// Steps come in pairs (PH = 0: s even, PH = 1: s odd) and L is even, so the rows the two I/O lanes touch are fixed
+// per PH and every address is `base` plus a compile-time offset, with base = rows + ctr + h * (s - PH) advanced
+// by 2h per pair by the caller (no per-lane pointer, no row toggling in the loop):
+//   reader (group lane 0):    line -1-e at super-column s is (x' = h s + e, tier s): row PH
+//   writer (group lane L-1):  at its super-column sc = s - (L-1) its top line e leaves at
+//                             (x' = -n/2 + h sc + e, tier m + sc): row (sc & 1) = 1 - PH
+template <class Prob, int B, int L, int KIND, bool GUARD, int PH, int RSC>
 __device__ __forceinline__ void char_step(typename Prob::R (&v)[Prob::C][B],
                                           typename Prob::R (&hal)[Prob::C][2 * Prob::H],
                                           const typename Prob::R (&halp)[Prob::C][2 * Prob::H],
-                                          typename Prob::R*& io, int& inc, const int s, const int gl, const int RS,
-                                          const Consts<typename Prob::R>& kc) {
+                                          typename Prob::R* base, const uint32_t sbase, const int s, const int gl,
+                                          const int RS, const Consts<typename Prob::R>& kc) {
   using R = typename Prob::R;
   constexpr int H = Prob::H, C = Prob::C;
   constexpr int n = B * L, m = n / (2 * H);
@@ -100,23 +132,40 @@ __device__ __forceinline__ void char_step(typename Prob::R (&v)[Prob::C][B],
 #pragma unroll
     for (int e = 0; e < 2 * H; ++e) hal[c][e] = shfl_up_<R>(v[c][B - 1 - e], L);
   if (gl == 0 && (!GUARD || s < m)) {
+    if constexpr (RSC > 0) {  // row stride known at compile time: immediate offsets from the running shared address
+      if constexpr (C >= 1) { lds_tied<(int)sizeof(R) * ((PH * C + 0) * RSC + PH * H + 0)>(hal[0][0], sbase);
+                              lds_tied<(int)sizeof(R) * ((PH * C + 0) * RSC + PH * H + 1)>(hal[0][1], sbase); }
+      if constexpr (H == 2) { lds_tied<(int)sizeof(R) * ((PH * C + 0) * RSC + PH * H + 2)>(hal[0][2], sbase);
+                              lds_tied<(int)sizeof(R) * ((PH * C + 0) * RSC + PH * H + 3)>(hal[0][3], sbase); }
+      static_assert(C == 1, "the compile-time-stride path is instantiated for the scalar problems");
+    } else {
 #pragma unroll
-    for (int c = 0; c < C; ++c)
+      for (int c = 0; c < C; ++c)
 #pragma unroll
-      for (int e = 0; e < 2 * H; ++e) hal[c][e] = io[c * RS + e];
+        for (int e = 0; e < 2 * H; ++e) hal[c][e] = base[(PH * C + c) * RS + PH * H + e];
+    }
   }
   if (!GUARD || (sc >= 0 && sc < m)) {
     char_update_lines<Prob, B, L, KIND>(v, hal, halp, sc, gl, kc);
     // upper-left edge: the top 2h lines of the last lane leave the tile
     if (KIND != KIND_DOWN && gl == L - 1) {
+      if constexpr (RSC > 0) {
+        constexpr int W0 = ((1 - PH) * C + 0) * RSC + PH * H - n / 2 - H * (L - 1);
+        sts_imm<(int)sizeof(R) * (W0 + 0)>(sbase, v[0][B - 1]);
+        sts_imm<(int)sizeof(R) * (W0 + 1)>(sbase, v[0][B - 2]);
+        if constexpr (H == 2) {
+          sts_imm<(int)sizeof(R) * (W0 + 2)>(sbase, v[0][B - 3]);
+          sts_imm<(int)sizeof(R) * (W0 + 3)>(sbase, v[0][B - 4]);
+        }
+      } else {
 #pragma unroll
-      for (int c = 0; c < C; ++c)
+        for (int c = 0; c < C; ++c)
 #pragma unroll
-        for (int e = 0; e < 2 * H; ++e) io[c * RS + e] = v[c][B - 1 - e];
+          for (int e = 0; e < 2 * H; ++e)
+            base[((1 - PH) * C + c) * RS + PH * H - n / 2 - H * (L - 1) + e] = v[c][B - 1 - e];
+      }
     }
   }
-  io += inc;
-  inc = 2 * H - inc;
 }
 
 // Line values of one lane <-> the staged rows of its tile (rows, RS, ctr as in char_sweep_tile).
@@ -173,7 +222,8 @@ __device__ __forceinline__ void char_store_lines(const typename Prob::R (&v)[Pro
 // m + L - 1 skewed super-steps, final line values back to the staged rows (in place).
 //   rows : staged two-row state, component c of row r at rows[(r*C + c)*RS + slot]
 //   ctr  : slot of x' = 0 (the tile centre);  gl : lane within the group
-template <class Prob, int B, int L, int KIND>
+// RSC = the row stride RS when it is a compile-time constant (FLOW), else 0 (CHAR: it depends on the launch).
+template <class Prob, int B, int L, int KIND, int RSC = 0>
 __device__ __forceinline__ void char_sweep_tile(typename Prob::R* rows, const int RS, const int ctr, const int gl,
                                                 const Consts<typename Prob::R>& kc) {
   using R = typename Prob::R;
@@ -192,26 +242,21 @@ __device__ __forceinline__ void char_sweep_tile(typename Prob::R* rows, const in
     for (int e = 0; e < 2 * H; ++e) halA[c][e] = halB[c][e] = (R)0;
   __syncwarp();
 
-  // Loop I/O goes through one per-thread pointer: element (row sc&1, x' = base + h sc) with
-  //   reader (group lane 0)    base = 0      : line -1-e at super-column sc is (x' = h sc + e,        tier sc)
-  //   writer (group lane L-1)  base = -n/2   : its top line e leaves at       (x' = -n/2 + h sc + e, tier m+sc)
-  // advanced by h and toggled between the two rows every step (inc alternates h + C RS, h - C RS).
-  const int sc0 = -gl;
-  R* io = rows + ((sc0 & 1) * C) * RS + ctr + (gl == 0 ? 0 : -n / 2) + H * sc0;
-  int inc = H + ((sc0 & 1) ? -C * RS : C * RS);
-
+  // Loop I/O (group lanes 0 and L-1 only) goes through one pointer advanced by 2h per pair of steps (char_step)
+  R* base = rows + ctr;
+  uint32_t sbase = smem_u32(base);
   int s = 0;
-  for (; s < L; s += 2) {  // ramp up: lane gl starts at step gl
-    char_step<Prob, B, L, KIND, true>(v, halA, halB, io, inc, s, gl, RS, kc);
-    char_step<Prob, B, L, KIND, true>(v, halB, halA, io, inc, s + 1, gl, RS, kc);
+  for (; s < L; s += 2, base += 2 * H, sbase += 2 * H * (int)sizeof(R)) {  // ramp up: lane gl starts at step gl
+    char_step<Prob, B, L, KIND, true, 0, RSC>(v, halA, halB, base, sbase, s, gl, RS, kc);
+    char_step<Prob, B, L, KIND, true, 1, RSC>(v, halB, halA, base, sbase, s + 1, gl, RS, kc);
   }
-  for (; s < m; s += 2) {  // steady state: every lane is inside its m super-columns
-    char_step<Prob, B, L, KIND, false>(v, halA, halB, io, inc, s, gl, RS, kc);
-    char_step<Prob, B, L, KIND, false>(v, halB, halA, io, inc, s + 1, gl, RS, kc);
+  for (; s < m; s += 2, base += 2 * H, sbase += 2 * H * (int)sizeof(R)) {  // steady state: every lane is inside its m super-columns
+    char_step<Prob, B, L, KIND, false, 0, RSC>(v, halA, halB, base, sbase, s, gl, RS, kc);
+    char_step<Prob, B, L, KIND, false, 1, RSC>(v, halB, halA, base, sbase, s + 1, gl, RS, kc);
   }
-  for (; s < m + L; s += 2) {  // ramp down (the last step, s = m+L-1, is empty and keeps the pairing)
-    char_step<Prob, B, L, KIND, true>(v, halA, halB, io, inc, s, gl, RS, kc);
-    char_step<Prob, B, L, KIND, true>(v, halB, halA, io, inc, s + 1, gl, RS, kc);
+  for (; s < m + L; s += 2, base += 2 * H, sbase += 2 * H * (int)sizeof(R)) {  // ramp down (the last step, s = m+L-1, is empty and keeps the pairing)
+    char_step<Prob, B, L, KIND, true, 0, RSC>(v, halA, halB, base, sbase, s, gl, RS, kc);
+    char_step<Prob, B, L, KIND, true, 1, RSC>(v, halB, halA, base, sbase, s + 1, gl, RS, kc);
   }
   __syncwarp();
   char_store_lines<Prob, B, L, KIND>(v, rows, RS, ctr, gl);

@@ -7,9 +7,12 @@
 // row r-1 it overlaps (the edges it receives), not the whole row.  So here every tile of the
 // cycle is a task (row-major ticket order, one atomic ticket counter); a WARP takes a ticket, waits until the
 // two parent tiles have published their edges (one flag per tile, release/acquire at GPU scope), stages the
-// tile's two rows from global memory into its private shared-memory slice, sweeps the tile exactly as the
-// CHAR flavour does (swept_char.cuh: registers + shuffles, L = 32 lanes, B = n/32 lines per lane), writes the
-// rows back and raises its flag.  This removes the launch gaps, the load / compute / store serialisation of a
+// tile's two rows from global memory into a private shared-memory slice with TMA 1-D bulk copies
+// (cp.async.bulk, mbarrier completion), sweeps the tile exactly as the CHAR flavour does (swept_char.cuh:
+// registers + shuffles, L = 32 lanes, B = n/32 lines per lane), writes the rows back with bulk stores and raises
+// its flag.  (Staging the NEXT tile behind the sweep — two slices per warp — was built and measured: no gain at
+// any size, because at the sizes where the next tile is ready early the load is 0.1 % of the tile time, and
+// claiming a ticket ahead of time costs the dynamic balance.)  This removes the launch gaps, the load / compute / store serialisation of a
 // whole row, and the load imbalance of 2^k equal tiles on 148 SMs (a fast SM simply takes the next ticket).
 //
 // Global state: the same two-row layout as the other flavours.  Row r of the cycle
@@ -85,21 +88,65 @@ __device__ __forceinline__ void warp_store_row(R* __restrict__ dst, const R* src
   }
 }
 
+// TMA 1-D bulk copies of `len` elements starting at global element g0 of a periodic row of N elements (g0 may be
+// negative by less than N); g0, len and N are multiples of the 16-byte granule, so every piece is aligned.
+template <class R>
+__device__ __forceinline__ void bulk_load_wrapped(R* dst, const R* __restrict__ src, int64_t g0, int len, int64_t N,
+                                                  uint64_t* bar) {
+  int64_t g = g0 < 0 ? g0 + N : g0;
+  while (len > 0) {
+    const int piece = (int)((N - g) < (int64_t)len ? (N - g) : (int64_t)len);
+    bulk_g2s(dst, src + g, (uint32_t)(piece * sizeof(R)), bar);
+    dst += piece;
+    len -= piece;
+    g = 0;
+  }
+}
+template <class R>
+__device__ __forceinline__ void bulk_store_wrapped(R* __restrict__ dst, const R* src, int64_t g0, int len, int64_t N) {
+  int64_t g = g0;
+  while (len > 0) {
+    const int piece = (int)((N - g) < (int64_t)len ? (N - g) : (int64_t)len);
+    bulk_s2g(dst + g, src, (uint32_t)(piece * sizeof(R)));
+    src += piece;
+    len -= piece;
+    g = 0;
+  }
+}
+// orders this thread's generic-proxy view against the async (TMA) proxy, all state spaces: after a flag has been
+// acquired and before a bulk load of what it guards; after bulk stores have completed and before the flag is raised
+__device__ __forceinline__ void fence_proxy_async_all() { asm volatile("fence.proxy.async;" ::: "memory"); }
+
 #ifndef FLOW_MAX_SLEEP
 #define FLOW_MAX_SLEEP 256
 #endif
 
-template <class Prob, int B>
+// TMA = true : the tile's rows are staged by cp.async.bulk loads completing on an mbarrier and written back by bulk
+//              stores, issued by one lane;
+// TMA = false: by 16-byte ld.global.cg / st.global of all 32 lanes.
+// Same task loop, same sweep, same protocol.  Both are kept because the compiler's code for the sweep loop depends on
+// which one surrounds it (profiles/r2_flow_phases.md); swept_autotune measures both.
+template <class Prob, int B, bool TMA>
 __global__ void __launch_bounds__(128) swept_flow_kernel(const FlowArgs<typename Prob::R> a) {
   using R = typename Prob::R;
   constexpr int H = Prob::H, C = Prob::C, PAD = Pad16<R>::value, L = 32;
   constexpr int n = B * L;
   constexpr int RS = n + 2 * PAD;
+  static_assert(H <= PAD, "the halo must fit the 16-byte pad of a staged row");
   extern __shared__ __align__(128) unsigned char smem_raw[];
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   R* rows = reinterpret_cast<R*>(smem_raw) + (size_t)warp * 2 * C * RS;
+  uint64_t* mbar = reinterpret_cast<uint64_t*>(smem_raw + (size_t)(blockDim.x >> 5) * 2 * C * RS * sizeof(R)) + warp;
   const int64_t N = a.N;
   const unsigned ntasks = (unsigned)a.rows * (unsigned)a.K;
+  unsigned phase = 0;  // parity the mbarrier completes next
+  if constexpr (TMA) {
+    if (lane == 0) {
+      mbar_init(mbar, 1);
+      fence_mbar_init();
+    }
+    __syncwarp();
+  }
 
   for (;;) {
     unsigned t = 0;
@@ -107,16 +154,15 @@ __global__ void __launch_bounds__(128) swept_flow_kernel(const FlowArgs<typename
     t = __shfl_sync(0xffffffffu, t, 0);
     if (t >= ntasks) break;
     const int r = (int)(t / (unsigned)a.K), k = (int)(t % (unsigned)a.K);
-    const int64_t S = (int64_t)k * n + ((r & 1) ? n / 2 : 0);  // < N + n/2; copies wrap
+    const int64_t S = (int64_t)k * n + ((r & 1) ? n / 2 : 0);  // < N; copies wrap
     if (r > 0) {
-      // parents: the tiles of row r-1 overlapping [S, S+n)
+      // parents: the tiles of row r-1 overlapping [S, S+n); row r-1 publishes (r-1) + 1
       const int p0 = (r & 1) ? k : (k == 0 ? a.K - 1 : k - 1);
       const int p1 = (r & 1) ? (k + 1 == a.K ? 0 : k + 1) : k;
       const int* f = a.flags + (size_t)((r - 1) & 1) * a.K;
-      const int want = r;  // row r-1 publishes (r-1) + 1
       unsigned ns = 32, polls = 0;
       bool dead = false;
-      while (ld_relaxed_gpu(f + p0) < want || ld_relaxed_gpu(f + p1) < want) {
+      while (ld_relaxed_gpu(f + p0) < r || ld_relaxed_gpu(f + p1) < r) {
         __nanosleep(ns);
         if (ns < FLOW_MAX_SLEEP) ns *= 2;
         // cannot happen while the grid is co-resident; bounded so that a scheduling surprise yields an error
@@ -133,49 +179,84 @@ __global__ void __launch_bounds__(128) swept_flow_kernel(const FlowArgs<typename
       if (dead) break;
       fence_acq_rel_gpu();
     }
-    // ---- stage the tile: both rows over [S-h, S+n+h) (Up: row 0 of the initial level, no halo)
-    if (r == 0) {
+    // ---- stage the tile: both rows with their halo [S-h, S+n+h) (Up: row 0 of the initial level; the other row
+    // is zero: tier -1 does not exist)
+    const R* in0 = r == 0 ? a.init : ((r & 1) ? a.buf[0][0] : a.buf[1][0]);
+    const R* in1 = (r & 1) ? a.buf[0][1] : a.buf[1][1];
+    if constexpr (TMA) {
+      // bulk loads over [S-PAD, S+n+PAD): the 16-byte pad holds the halo (what lies beyond it is never used)
+      if (lane == 0) {
+        fence_proxy_async_all();  // what the flags guard is read through the async proxy
+        const int nrows = r == 0 ? 1 : 2;
+        mbar_arrive_expect_tx(mbar, (uint32_t)(nrows * C * RS * sizeof(R)));
 #pragma unroll
-      for (int c = 0; c < C; ++c) warp_load_row<R>(rows + c * RS + PAD, a.init + (int64_t)c * N, S, n, N, lane);
-      for (int i = lane; i < C * RS; i += 32) rows[C * RS + i] = (R)0;  // tier -1 does not exist
-    } else {
-      const R* in0 = (r & 1) ? a.buf[0][0] : a.buf[1][0];
-      const R* in1 = (r & 1) ? a.buf[0][1] : a.buf[1][1];
-#pragma unroll
-      for (int c = 0; c < C; ++c) {
-        warp_load_row<R>(rows + c * RS + PAD, in0 + (int64_t)c * N, S, n, N, lane);
-        warp_load_row<R>(rows + (C + c) * RS + PAD, in1 + (int64_t)c * N, S, n, N, lane);
+        for (int c = 0; c < C; ++c) {
+          bulk_load_wrapped<R>(rows + c * RS, in0 + (int64_t)c * N, S - PAD, RS, N, mbar);
+          if (r != 0) bulk_load_wrapped<R>(rows + (C + c) * RS, in1 + (int64_t)c * N, S - PAD, RS, N, mbar);
+        }
       }
-      if (lane < 2 * C * 2 * H) {
-        const int rr = lane / (C * 2 * H), c = (lane / (2 * H)) % C, j = lane % (2 * H);
-        int64_t g = (j < H) ? (S - H + j) : (S + n + (j - H));  // S < N, so one wrap suffices
-        if (g < 0) g += N;
-        if (g >= N) g -= N;
-        const int s = (j < H) ? (PAD - H + j) : (PAD + n + (j - H));
-        rows[(rr * C + c) * RS + s] = __ldcg((rr ? in1 : in0) + (int64_t)c * N + g);
+      if (r == 0)
+        for (int i = lane; i < C * RS; i += 32) rows[C * RS + i] = (R)0;
+      mbar_wait(mbar, phase);
+      phase ^= 1u;
+    } else {
+      if (r == 0) {
+#pragma unroll
+        for (int c = 0; c < C; ++c) warp_load_row<R>(rows + c * RS + PAD, in0 + (int64_t)c * N, S, n, N, lane);
+        for (int i = lane; i < C * RS; i += 32) rows[C * RS + i] = (R)0;
+      } else {
+#pragma unroll
+        for (int c = 0; c < C; ++c) {
+          warp_load_row<R>(rows + c * RS + PAD, in0 + (int64_t)c * N, S, n, N, lane);
+          warp_load_row<R>(rows + (C + c) * RS + PAD, in1 + (int64_t)c * N, S, n, N, lane);
+        }
+        if (lane < 2 * C * 2 * H) {
+          const int rr = lane / (C * 2 * H), c = (lane / (2 * H)) % C, j = lane % (2 * H);
+          int64_t g = (j < H) ? (S - H + j) : (S + n + (j - H));  // S < N, so one wrap suffices
+          if (g < 0) g += N;
+          if (g >= N) g -= N;
+          const int sl = (j < H) ? (PAD - H + j) : (PAD + n + (j - H));
+          rows[(rr * C + c) * RS + sl] = __ldcg((rr ? in1 : in0) + (int64_t)c * N + g);
+        }
       }
     }
     __syncwarp();
     // ---- sweep (identical arithmetic and order to the CHAR flavour)
-    if (r == 0) char_sweep_tile<Prob, B, L, KIND_UP>(rows, RS, PAD + n / 2, lane, a.k);
-    else if (r == a.rows - 1) char_sweep_tile<Prob, B, L, KIND_DOWN>(rows, RS, PAD + n / 2, lane, a.k);
-    else char_sweep_tile<Prob, B, L, KIND_WHOLE>(rows, RS, PAD + n / 2, lane, a.k);
-    __syncwarp();
-    // ---- publish
+    if (r == 0) char_sweep_tile<Prob, B, L, KIND_UP, RS>(rows, RS, PAD + n / 2, lane, a.k);
+    else if (r == a.rows - 1) char_sweep_tile<Prob, B, L, KIND_DOWN, RS>(rows, RS, PAD + n / 2, lane, a.k);
+    else char_sweep_tile<Prob, B, L, KIND_WHOLE, RS>(rows, RS, PAD + n / 2, lane, a.k);
+    // ---- publish: the rows over [S, S+n), then the flag
     R* out0 = (r & 1) ? a.buf[1][0] : a.buf[0][0];
     R* out1 = (r & 1) ? a.buf[1][1] : a.buf[0][1];
+    if constexpr (TMA) {
+      fence_proxy_async_smem();
+      __syncwarp();
+      if (lane == 0) {
 #pragma unroll
-    for (int c = 0; c < C; ++c) {
-      warp_store_row<R>(out0 + (int64_t)c * N, rows + c * RS + PAD, S, n, N, lane);
-      if (r != a.rows - 1)  // Down leaves only row 0: the full time level
-        warp_store_row<R>(out1 + (int64_t)c * N, rows + (C + c) * RS + PAD, S, n, N, lane);
+        for (int c = 0; c < C; ++c) {
+          bulk_store_wrapped<R>(out0 + (int64_t)c * N, rows + c * RS + PAD, S, n, N);
+          if (r != a.rows - 1)  // Down leaves only row 0: the full time level
+            bulk_store_wrapped<R>(out1 + (int64_t)c * N, rows + (C + c) * RS + PAD, S, n, N);
+        }
+        bulk_commit();
+        bulk_wait_all();  // the writes are complete (not just the shared-memory reads)
+        fence_proxy_async_all();
+        st_release_gpu(a.flags + (size_t)(r & 1) * a.K + k, r + 1);
+      }
+    } else {
+      __syncwarp();
+#pragma unroll
+      for (int c = 0; c < C; ++c) {
+        warp_store_row<R>(out0 + (int64_t)c * N, rows + c * RS + PAD, S, n, N, lane);
+        if (r != a.rows - 1) warp_store_row<R>(out1 + (int64_t)c * N, rows + (C + c) * RS + PAD, S, n, N, lane);
+      }
+      __syncwarp();
+      if (lane == 0) {
+        __threadfence();
+        st_release_gpu(a.flags + (size_t)(r & 1) * a.K + k, r + 1);
+      }
     }
-    __syncwarp();
-    if (lane == 0) {
-      __threadfence();
-      st_release_gpu(a.flags + (size_t)(r & 1) * a.K + k, r + 1);
-    }
-    __syncwarp();  // the slice is reused by the next task of this warp
+    __syncwarp();  // the slice is restaged by the next task of this warp
   }
   // Leave the scratch as it was found.  A warp arrives here after its last task is in global memory; the warp that
   // arrives last therefore knows that every task of the launch is done.
@@ -194,7 +275,7 @@ __global__ void __launch_bounds__(128) swept_flow_kernel(const FlowArgs<typename
 template <class Prob>
 inline size_t flow_smem_bytes(int warps, int n) {
   using R = typename Prob::R;
-  return (size_t)warps * 2 * Prob::C * ((size_t)n + 2 * Pad16<R>::value) * sizeof(R);
+  return (size_t)warps * (2 * Prob::C * ((size_t)n + 2 * Pad16<R>::value) * sizeof(R) + 8);
 }
 
 }  // namespace swept

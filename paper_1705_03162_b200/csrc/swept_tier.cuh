@@ -33,6 +33,10 @@ struct TierArgs {
   const R* in1;  // row1 of the input buffer (unused by Up)
   R* out0;
   R* out1;  // unused by Down
+  const R* in2 = nullptr;  // third row, schemes with three sub-timesteps per timestep (Prob::ROWS == 3)
+  R* out2 = nullptr;
+  int tmod = 0;  // global tier of the phase's relative tier 0, modulo Prob::ROWS (0 for the two-row schemes, whose
+                 // phases all start on even tiers)
   int64_t N;
   int n;       // tile width in points
   int shift;   // 0 or n/2
@@ -62,13 +66,14 @@ __device__ __forceinline__ void tier_range(int t, int n, int h, int m, int& lo, 
 template <class Prob, int P, int KIND>
 __global__ void __launch_bounds__(Prob::TIER_MAX_THREADS) swept_tier_kernel(const TierArgs<typename Prob::R> a) {
   using R = typename Prob::R;
-  constexpr int H = Prob::H, C = Prob::C, PAD = Pad16<R>::value;
+  constexpr int H = Prob::H, C = Prob::C, PAD = Pad16<R>::value, ROWS = Prob::ROWS;
+  static_assert(ROWS == 2 || (ROWS == Prob::SIGMA && C == 1), "rows = tier modulo ROWS; u^n in row 0");
   extern __shared__ __align__(128) unsigned char smem_raw[];
   const int n = a.n;
   const int RS = n + 4 * PAD;  // padded row stride: body starts 16 bytes in; room for the wall gap (see below)
   R* rows = reinterpret_cast<R*>(smem_raw);
-  uint64_t* mbar = reinterpret_cast<uint64_t*>(smem_raw + (size_t)2 * C * RS * sizeof(R));
-  R* xtr = reinterpret_cast<R*>(smem_raw + (size_t)2 * C * RS * sizeof(R) + 16);  // Euler: pressures, fluxes
+  uint64_t* mbar = reinterpret_cast<uint64_t*>(smem_raw + (size_t)ROWS * C * RS * sizeof(R));
+  R* xtr = reinterpret_cast<R*>(smem_raw + (size_t)ROWS * C * RS * sizeof(R) + 16);  // Euler: pressures, fluxes
   (void)xtr;
   const int64_t N = a.N;
   const int tid = threadIdx.x;
@@ -76,7 +81,7 @@ __global__ void __launch_bounds__(Prob::TIER_MAX_THREADS) swept_tier_kernel(cons
   if (S >= N) S -= N;
   const int len1 = (int)((N - S) < (int64_t)n ? (N - S) : (int64_t)n);  // part before the periodic wrap
   const int len2 = n - len1;
-  constexpr int NROWS_IN = (KIND == KIND_UP) ? 1 : 2;
+  constexpr int NROWS_IN = (KIND == KIND_UP) ? 1 : ROWS;
   // Non-periodic ends ("node 0 is split across the spatial boundary and must apply the boundary conditions at its
   // center"): the tile that wraps holds the last n/2 and the first n/2 points of the domain with the
   // two walls between them.  Its halves are staged 2*PAD slots apart and the gap holds each wall's h ghost values;
@@ -98,7 +103,7 @@ __global__ void __launch_bounds__(Prob::TIER_MAX_THREADS) swept_tier_kernel(cons
     mbar_arrive_expect_tx(mbar, (uint32_t)(NROWS_IN * C * n * sizeof(R)));
 #pragma unroll
     for (int r = 0; r < NROWS_IN; ++r) {
-      const R* src = r == 0 ? a.in0 : a.in1;
+      const R* src = r == 0 ? a.in0 : (r == 1 ? a.in1 : a.in2);
 #pragma unroll
       for (int c = 0; c < C; ++c) {
         R* dst = rows + (r * C + c) * RS + PAD;
@@ -108,13 +113,14 @@ __global__ void __launch_bounds__(Prob::TIER_MAX_THREADS) swept_tier_kernel(cons
     }
   }
   if (KIND == KIND_UP) {
-    // tier -1 does not exist: give row1 a defined value (its edge slots are stored but never used)
-    for (int i = tid; i < C * RS; i += blockDim.x) rows[C * RS + i] = (R)0;
+    // tiers before the cycle's first do not exist: give the other rows a defined value (their edge slots are
+    // stored but never used)
+    for (int i = tid; i < (ROWS - 1) * C * RS; i += blockDim.x) rows[C * RS + i] = (R)0;
   } else {
-    // halo: H points either side of the tile, both rows, plain loads (periodic, or mirrored at a wall)
-    for (int i = tid; i < 2 * C * 2 * H; i += blockDim.x) {
+    // halo: H points either side of the tile, every row, plain loads (periodic, or mirrored at a wall)
+    for (int i = tid; i < ROWS * C * 2 * H; i += blockDim.x) {
       const int r = i / (C * 2 * H), c = (i / (2 * H)) % C, j = i % (2 * H);
-      const R* src = (r == 0 ? a.in0 : a.in1) + (int64_t)c * N;
+      const R* src = (r == 0 ? a.in0 : (r == 1 ? a.in1 : a.in2)) + (int64_t)c * N;
       int64_t g = (j < H) ? (S - H + j) : (S + n + (j - H));
       if (len2 > 0 && j >= H) g = len2 + (j - H);  // the wrapping tile continues at point n/2 (no wall there)
       const bool fixed = a.bc == BC_FIXED && (g < 0 || g >= N);
@@ -142,8 +148,11 @@ __global__ void __launch_bounds__(Prob::TIER_MAX_THREADS) swept_tier_kernel(cons
   const int j0 = tid * P;
   const int sb = slot_of(j0);  // a thread's P points lie on one side of the wrap (n/2 is a multiple of P)
   for (int t = 1; t <= a.ntiers; ++t) {
-    const int par = t & 1;  // phases start on even global tiers (m is even): odd = predictor
-    const R* src = rows + (1 - par) * C * RS;
+    // global tier g = tmod + t (mod ROWS): reads row (g-1) % ROWS, writes row g % ROWS; the stage is g % SIGMA
+    // (two-row schemes: phases start on even global tiers, m is even, so par = t & 1: odd = predictor)
+    const int gm = (a.tmod + t) % ROWS;
+    const int par = ROWS == 2 ? (t & 1) : gm;
+    const R* src = rows + (ROWS == 2 ? 1 - par : (gm + ROWS - 1) % ROWS) * C * RS;
     R* dst = rows + par * C * RS;
     int lo, hi;
     tier_range<KIND>(t, n, H, m, lo, hi);
@@ -189,7 +198,7 @@ __global__ void __launch_bounds__(Prob::TIER_MAX_THREADS) swept_tier_kernel(cons
       for (int c = 0; c < C; ++c)
 #pragma unroll
         for (int j = 0; j < P; ++j)
-          bs[c][j] = (Prob::SIGMA == 2 && !par) ? dst[c * RS + sb + j] : win[c][H + j];
+          bs[c][j] = (Prob::SIGMA >= 2 && par != 1) ? rows[c * RS + sb + j] : win[c][H + j];  // u^n: row 0
       Prob::template stage<P>(win, bs, o, par, a.k);
 #pragma unroll
       for (int j = 0; j < P; ++j)
@@ -215,10 +224,10 @@ __global__ void __launch_bounds__(Prob::TIER_MAX_THREADS) swept_tier_kernel(cons
   fence_proxy_async_smem();
   __syncthreads();
   if (tid == 0) {
-    constexpr int NROWS_OUT = (KIND == KIND_DOWN) ? 1 : 2;
+    constexpr int NROWS_OUT = (KIND == KIND_DOWN) ? 1 : ROWS;
 #pragma unroll
     for (int r = 0; r < NROWS_OUT; ++r) {
-      R* dstg = r == 0 ? a.out0 : a.out1;
+      R* dstg = r == 0 ? a.out0 : (r == 1 ? a.out1 : a.out2);
 #pragma unroll
       for (int c = 0; c < C; ++c) {
         const R* s = rows + (r * C + c) * RS + PAD;
@@ -235,7 +244,7 @@ template <class Prob>
 inline size_t tier_smem_bytes(int n) {
   using R = typename Prob::R;
   const size_t row = ((size_t)n + 4 * Pad16<R>::value) * sizeof(R);
-  return (size_t)2 * Prob::C * row + 16 + (Prob::C == 3 ? 4 * row : 0);  // Euler: + one pressure and three flux rows
+  return (size_t)Prob::ROWS * Prob::C * row + 16 + (Prob::C == 3 ? 4 * row : 0);  // Euler: + one pressure and three flux rows
 }
 
 }  // namespace swept

@@ -36,7 +36,7 @@ def gpu_run(w, nsteps, variant, tile_width=0, flavor=sw.FLAVOR_AUTO, group=0, dt
 
 
 CHAR = tuple((sw.FLAVOR_CHAR, L) for L in (8, 16, 32))
-FLOW = ((sw.FLAVOR_FLOW, 0),)   # heat / KS, n in {256, 512, 1024}
+FLOW = ((sw.FLAVOR_FLOW, 0), (sw.FLAVOR_FLOW, 16))   # heat / KS, n in {256, 512, 1024}; group 16 = TMA staging
 TIER12 = ((sw.FLAVOR_TIER, 1), (sw.FLAVOR_TIER, 2))
 
 
@@ -72,7 +72,7 @@ def admissible(w, n, flavor, group, dtype=np.float64):
                 return True
         return False
     if flavor == sw.FLAVOR_FLOW:  # persistent launch: periodic heat / KS, 32 lanes per tile, B = n/32 in {8, 16, 32}
-        return problem != si.EULER and not bc and n in (256, 512, 1024) and N % 256 == 0 and group <= 16
+        return problem != si.EULER and not bc and n in (256, 512, 1024) and N % 256 == 0 and (group & 15) <= 12 and group < 32
     raise ValueError(flavor)
 
 
@@ -168,7 +168,7 @@ def test_wide_tiles():
     check(w, 600, [1024, 2048], flavors=((sw.FLAVOR_TIER, 1), (sw.FLAVOR_TIER, 2), (sw.FLAVOR_TIER, 4)))
 
 
-@pytest.mark.parametrize("warps", [0, 1, 3])  # resident CTAs per SM (0 = default policy)
+@pytest.mark.parametrize("warps", [0, 1, 3, 16, 18])  # resident CTAs per SM (0 = default policy); +16 = TMA staging
 def test_flow_flavour_many_cycles_and_small_grids(warps):
     # FLOW: one persistent launch per Up..Down cycle, rows chained by per-tile flags.  K = N/n = 1, 2 and
     # many tiles per row; D = 0 (Up + Down only), odd and even D; remainder levels; both RK2 flavours
