@@ -38,7 +38,11 @@ extern "C" {
 
 typedef struct swept_state swept_state; /* opaque; owns its device buffers */
 
-enum { SWEPT_HEAT = 0, SWEPT_KS = 1, SWEPT_EULER = 2 };     /* problem (App. B-D)  */
+enum { SWEPT_HEAT = 0, SWEPT_KS = 1, SWEPT_EULER = 2,       /* problem (App. B-D)  */
+       SWEPT_KS3 = 3 };  /* the KS discretisation (C.2) with THREE sub-timesteps per timestep (Shu-Osher SSP-RK3):
+                            the case PAPER.md:131 says the two-row decomposition "must be adjusted" for — the
+                            inter-launch state has three rows (tier modulo 3).  FP64, periodic; per-step and the
+                            swept TIER flavour */
 enum { SWEPT_PER_STEP = 0, SWEPT_SWEPT = 1 };               /* variant                           */
 enum { SWEPT_F64 = 0, SWEPT_F32 = 1 };                      /* dtype                             */
 enum { SWEPT_RK2_MIDPOINT = 0, SWEPT_RK2_HEUN = 1 };        /* KS/Euler integrator (
@@ -93,7 +97,9 @@ typedef struct {
  * N >= 32, see swept_run).  All device memory the state will ever use — four field slabs and the scratch of the
  * persistent flavours — is allocated here, through p->alloc when given; creation may synchronise p->stream.
  * p->stream = NULL means the CUDA legacy default stream (the Python binding passes torch's current stream and
- * re-sets it with swept_set_stream before every call).  Returns NULL on error. */
+ * re-sets it with swept_set_stream before every call).  Returns NULL on error.
+ * Debugging aid: with the environment variable SWEPT_POISON set, every field slab is filled with 0xFF bytes (NaNs)
+ * at creation, so that a kernel reading a value no kernel wrote yields a visibly wrong result. */
 swept_state* swept_create(int problem, int64_t N, double dx, double dt, const swept_params* p);
 
 /* swept_write — copy initial data from HOST memory (C*N REALs, layout above) to the device, asynchronously
@@ -212,6 +218,13 @@ typedef struct {
  * then a per-step remainder.  (swept_run additionally skips widths for which N has no kernel.)
  * Writes at most max_phases entries, returns the number of phases needed (or a negative error code). */
 int64_t swept_plan(int64_t nsub, int32_t n, int32_t h, swept_phase* out, int64_t max_phases);
+
+/* swept_plan_sigma — the same for a scheme with `sigma` sub-timesteps per timestep (1, 2 or 3; swept_plan is the
+ * sigma <= 2 case).  A cycle must end on a full timestep, i.e. T = (D+1) n/(2h) must be a multiple of sigma: with
+ * n/(2h) a power of two that is automatic for sigma = 1, 2 and means (D+1) % 3 == 0 for sigma = 3 (PAPER.md:131:
+ * the decomposition "must be adjusted" for more than two sub-timesteps).  Phases of a sigma = 3 cycle may start on
+ * any tier: tier0 % 3 tells the kernel which stage its first tier is. */
+int64_t swept_plan_sigma(int64_t nsub, int32_t n, int32_t h, int32_t sigma, swept_phase* out, int64_t max_phases);
 
 /* ---- measurement helpers --------------------------------------------------------------------------- */
 

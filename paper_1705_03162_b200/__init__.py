@@ -17,7 +17,9 @@ from ctypes import (CFUNCTYPE, POINTER, Structure, byref, c_char_p, c_double, c_
 
 import numpy as np
 
-HEAT, KS, EULER = 0, 1, 2
+HEAT, KS, EULER, KS3 = 0, 1, 2, 3   # KS3: (C.2) with three sub-timesteps per timestep (SSP-RK3), row f3
+#: problem -> (h, sigma, C): stencil half-width, sub-timesteps per timestep, components
+PROBLEM_SHAPE = {HEAT: (1, 1, 1), KS: (2, 2, 1), EULER: (2, 2, 3), KS3: (2, 3, 1)}
 PER_STEP, SWEPT = 0, 1
 F64, F32 = 0, 1
 RK2_MIDPOINT, RK2_HEUN = 0, 1
@@ -82,6 +84,8 @@ def load():
     lib.swept_last_error.restype = c_char_p
     lib.swept_plan.restype = c_int64
     lib.swept_plan.argtypes = [c_int64, c_int32, c_int32, POINTER(swept_phase), c_int64]
+    lib.swept_plan_sigma.restype = c_int64
+    lib.swept_plan_sigma.argtypes = [c_int64, c_int32, c_int32, c_int32, POINTER(swept_phase), c_int64]
     lib.swept_probe_fp64.argtypes = [c_int, c_void_p, POINTER(c_double)]
     lib.swept_probe_launch.argtypes = [c_int, c_void_p, c_int, POINTER(c_double)]
     lib.swept_set_phase_timing.argtypes = [c_void_p, c_int]
@@ -200,13 +204,20 @@ def swept_destroy(state: int) -> None:
     load().swept_destroy(state)
 
 
-def swept_plan(nsub: int, n: int, h: int):
+def swept_plan(nsub: int, n: int, h: int, sigma: int = 1):
+    """Phase list of ``swept_plan`` (sigma <= 2) / ``swept_plan_sigma`` (three sub-timesteps per timestep)."""
     lib = load()
-    cnt = lib.swept_plan(nsub, n, h, None, 0)
+    if sigma <= 2:
+        cnt = lib.swept_plan(nsub, n, h, None, 0)
+    else:
+        cnt = lib.swept_plan_sigma(nsub, n, h, sigma, None, 0)
     if cnt < 0:
         raise SweptError(f"swept_plan: {swept_last_error()}")
     arr = (swept_phase * max(cnt, 1))()
-    lib.swept_plan(nsub, n, h, arr, cnt)
+    if sigma <= 2:
+        lib.swept_plan(nsub, n, h, arr, cnt)
+    else:
+        lib.swept_plan_sigma(nsub, n, h, sigma, arr, cnt)
     return [(int(a.kind), int(a.shift), int(a.tier0), int(a.ntiers), int(a.n)) for a in arr[:cnt]]
 
 
@@ -229,9 +240,7 @@ class Swept:
                  alpha: float = 1.0, gamma: float = 1.4, bc: int = BC_PERIODIC):
         self.problem, self.N = problem, N
         self.np_dtype = np.dtype(dtype)
-        self.C = 3 if problem == EULER else 1
-        self.h = 1 if problem == HEAT else 2
-        self.sigma = 1 if problem == HEAT else 2
+        self.h, self.sigma, self.C = PROBLEM_SHAPE[problem]
         self._h = swept_create(problem, N, dx, dt, dtype=F64 if self.np_dtype == np.float64 else F32, rk2=rk2,
                                alpha=alpha, gamma=gamma, bc=bc)
 

@@ -37,6 +37,11 @@ struct TileLaunch {
   // CHAR leaves the first / last tile of the row unwritten
   int tile_base = 0, tile_step = 1, tile_count = 0;
   int skip_first = 0, skip_last = 0;
+  // three-row schemes (KS3: three sub-timesteps per timestep): the third row, and the global tier of the phase's
+  // relative tier 0 modulo 3 (which stage its first tier is)
+  const void* in2 = nullptr;
+  void* out2 = nullptr;
+  int tmod = 0;
 };
 
 // FLOW flavour: one whole Up / diamonds / Down cycle of tile width n in a single persistent launch
@@ -80,6 +85,9 @@ int launch_per_step_euler(int dtype, int rk2, const PerStepLaunch& a);
 int launch_tile_heat(int dtype, const TileLaunch& a);
 int launch_tile_ks(int dtype, int rk2, const TileLaunch& a);
 int launch_tile_euler(int dtype, int rk2, const TileLaunch& a);
+int launch_per_step_ks3(int dtype, const PerStepLaunch& a);  // a.odd = stage (1, 2, 0)
+int launch_tile_ks3(int dtype, const TileLaunch& a);
+bool tile_config_ok_ks3(int dtype, int flavor, int64_t N, int n, int P);
 // does a kernel exist for (flavor, n, P)?  (host-only query used by the autotuner and argument checks)
 int launch_resident_heat(int dtype, const ResidentLaunch& a);
 int launch_resident_ks(int dtype, int rk2, const ResidentLaunch& a);

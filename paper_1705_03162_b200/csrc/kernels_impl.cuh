@@ -82,6 +82,7 @@ inline int tier_go(const TileLaunch& a) {
   t.bc = a.bc;
   t.bv = round_bcvals<R>(a.bcv);
   t.tile_base = a.tile_base; t.tile_step = a.tile_step; t.skip_first = 0; t.skip_last = 0;
+  t.in2 = (const R*)a.in2; t.out2 = (R*)a.out2; t.tmod = a.tmod;
   const size_t smem = tier_smem_bytes<Prob>(a.n);
   auto kern = swept_tier_kernel<Prob, P, KIND>;
   if (smem > 48 * 1024) {

@@ -9,6 +9,7 @@
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <map>
 #include <mutex>
@@ -45,7 +46,8 @@ constexpr int KIND_UP = 0, KIND_SPLIT = 1, KIND_WHOLE = 2, KIND_DOWN = 3, KIND_R
 struct ProblemShape {
   int h, sigma, C;
 };
-const ProblemShape kShape[3] = {{1, 1, 1}, {2, 2, 1}, {2, 2, 3}};
+const ProblemShape kShape[4] = {{1, 1, 1}, {2, 2, 1}, {2, 2, 3}, {2, 3, 1}};
+constexpr int MAX_SLABS = 6;
 
 struct GraphKey {
   int threads, P, cur, steps;
@@ -79,7 +81,11 @@ struct swept_state {
   swept_free_fn free_ = nullptr;
   void* alloc_ctx = nullptr;
   size_t slab_bytes = 0;
-  void* slab[4] = {nullptr, nullptr, nullptr, nullptr};
+  // field slabs: twice the rows of the inter-launch state (phases ping-pong between two buffers): 4 for the two-row
+  // schemes, 6 for the three-row one (KS3)
+  void* slab[MAX_SLABS] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
+  int nslabs = 4;
+  int rows() const { return nslabs / 2; }
   int cur = 0;  // slab holding the current full time level
   int64_t steps_done = 0, last_launches = 0;
   // autotune results: [variant] -> tile width, flavour, P
@@ -99,6 +105,16 @@ struct swept_state {
   bool flow_pending_check = false;
   cudaStream_t wall_stream = nullptr;  // hybrid wall handling: the wall tiles run here, beside the CHAR launch
   cudaEvent_t wall_fork = nullptr, wall_join = nullptr;
+  // the phase list of the swept run being executed (swept_run plans and runs it in one go; the shard driver,
+  // swept_phase_begin / swept_phase_run, one phase at a time with edge exchanges in between)
+  struct Planned {
+    std::vector<swept_phase> plan;
+    std::map<int, std::pair<int, int>> cfg;  // tile width -> (flavour, group)
+    int rin[3] = {-1, -1, -1};               // slabs holding the rows written by the last phase
+    int nrows_valid = 0;                     // rows of `rin` that hold data (1 after Down: the full time level)
+    size_t next = 0;
+    int64_t nsteps = 0;
+  } pr;
   void* resident_scratch = nullptr;  // flags + exchange slots of the resident per-step kernel
   bool resident_pending_check = false;  // a FLOW launch has run since the error word was last read
   size_t elem() const { return dtype == SWEPT_F64 ? 8 : 4; }
@@ -119,6 +135,7 @@ int launch_per_step(swept_state* s, const void* in, const void* base, void* out,
   switch (s->problem) {
     case SWEPT_HEAT: rc = swept::launch_per_step_heat(s->dtype, a); break;
     case SWEPT_KS: rc = swept::launch_per_step_ks(s->dtype, s->rk2, a); break;
+    case SWEPT_KS3: rc = swept::launch_per_step_ks3(s->dtype, a); break;
     default: rc = swept::launch_per_step_euler(s->dtype, s->rk2, a); break;
   }
   if (rc == NO_KERNEL) return fail(SWEPT_EUNSUPPORTED, "no per-step kernel for this problem/dtype/P=%d", P);
@@ -136,6 +153,7 @@ int launch_tile(swept_state* s, swept::TileLaunch& a, cudaStream_t stream = null
   switch (s->problem) {
     case SWEPT_HEAT: rc = swept::launch_tile_heat(s->dtype, a); break;
     case SWEPT_KS: rc = swept::launch_tile_ks(s->dtype, s->rk2, a); break;
+    case SWEPT_KS3: rc = swept::launch_tile_ks3(s->dtype, a); break;
     default: rc = swept::launch_tile_euler(s->dtype, s->rk2, a); break;
   }
   if (rc == NO_KERNEL)
@@ -239,10 +257,11 @@ bool tile_ok(const swept_state* s, int flavor, int n, int P) {
   if (s->bc && flavor != SWEPT_FLAVOR_TIER && !(flavor == SWEPT_FLAVOR_CHAR && s->problem == SWEPT_HEAT)) return false;
   if (s->bc && flavor == SWEPT_FLAVOR_CHAR && !swept::tile_config_ok_heat(s->dtype, SWEPT_FLAVOR_TIER, s->N, n, 1))
     return false;
-  if (flavor == SWEPT_FLAVOR_FLOW && (s->problem == SWEPT_EULER || P < 0 || (P & 15) > 12 || P > 31 || !s->flow_scratch)) return false;
+  if (flavor == SWEPT_FLAVOR_FLOW && (s->problem == SWEPT_EULER || s->problem == SWEPT_KS3 || P < 0 || (P & 15) > 12 || P > 31 || !s->flow_scratch)) return false;
   switch (s->problem) {
     case SWEPT_HEAT: return swept::tile_config_ok_heat(s->dtype, flavor, s->N, n, P);
     case SWEPT_KS: return swept::tile_config_ok_ks(s->dtype, flavor, s->N, n, P);
+    case SWEPT_KS3: return swept::tile_config_ok_ks3(s->dtype, flavor, s->N, n, P);
     default: return swept::tile_config_ok_euler(s->dtype, flavor, s->N, n, P);
   }
 }
@@ -260,9 +279,15 @@ int per_step_P(const swept_state* s) {
 int enqueue_steps(swept_state* s, int64_t steps, int threads, int P, int* cur_io) {
   const int sigma = kShape[s->problem].sigma;
   int cur = *cur_io;
-  int nxt = (cur + 1) & 3, pred = (cur + 2) & 3;
+  const int ns = s->nslabs;
+  int nxt = (cur + 1) % ns, pred = (cur + 2) % ns, pred2 = (cur + 3) % ns;
   for (int64_t i = 0; i < steps; ++i) {
-    if (sigma == 1) {
+    if (sigma == 3) {
+      // three stages: u1 from u^n; u2 from u1 and u^n; u^{n+1} from u2 and u^n (stage index = tier modulo 3)
+      if (int rc = launch_per_step(s, s->slab[cur], s->slab[cur], s->slab[pred], 1, threads, P)) return rc;
+      if (int rc = launch_per_step(s, s->slab[pred], s->slab[cur], s->slab[pred2], 2, threads, P)) return rc;
+      if (int rc = launch_per_step(s, s->slab[pred2], s->slab[cur], s->slab[nxt], 0, threads, P)) return rc;
+    } else if (sigma == 1) {
       if (int rc = launch_per_step(s, s->slab[cur], s->slab[cur], s->slab[nxt], 0, threads, P)) return rc;
     } else if (s->problem == SWEPT_KS && P >= 2) {
       // both RK2 stages in one launch (north_star: "one launch per timestep or RK stage")
@@ -335,6 +360,8 @@ int run_resident(swept_state* s, int64_t steps) {
   if (!s->resident_scratch) return fail(SWEPT_EUNSUPPORTED, "no resident scratch (state creation failed to allocate it)");
   // flags restart from zero every launch; the error word behind them is sticky until swept_read looks at it
   CUDA_TRY(cudaMemsetAsync(s->resident_scratch, 0, (size_t)swept::RESIDENT_MAX_CTAS * 128, s->stream));
+  if (s->problem == SWEPT_KS3)
+    return fail(SWEPT_EUNSUPPORTED, "PS_RESIDENT is built for the paper's three problems, not for KS3");
   const int nxt = (s->cur + 1) & 3;
   swept::ResidentLaunch a{s->slab[s->cur], s->slab[nxt], s->N, steps, s->resident_scratch, s->consts, s->stream,
                           s->kernel_bc(), s->bcvals};
@@ -359,15 +386,20 @@ int run_resident(swept_state* s, int64_t steps) {
 // sub-timesteps a cycle of width w cannot cover (fewer than m_w = w/(2h)) go to the next narrower width, and
 // what is left below the narrowest one is finished with per-step launches.  Between cycles the state is a
 // plain time level, so every cycle starts with an UpTriangle from row 0.
-int64_t make_plan(int64_t nsub, const std::vector<int>& widths, int h, std::vector<swept_phase>* out) {
-  if (nsub < 0 || widths.empty()) return SWEPT_EINVAL;
+// A cycle must end on a full timestep: T = (D+1) m a multiple of sigma.  m is a power of two, so that is automatic
+// for sigma = 1, 2 (m even) and means (D+1) % 3 == 0 for sigma = 3 (more than two sub-timesteps).
+int64_t make_plan(int64_t nsub, const std::vector<int>& widths, int h, int sigma, std::vector<swept_phase>* out) {
+  if (nsub < 0 || widths.empty() || nsub % sigma) return SWEPT_EINVAL;
   int64_t done = 0;
   for (int n : widths) {
     if (n < 4 * h || (n & (n - 1))) return SWEPT_EINVAL;
     const int64_t m = n / (2 * h);
     const int64_t left = nsub - done;
-    if (left < m) continue;
-    const int64_t D = left / m - 1;
+    int64_t q = left / m;  // rows of tiles after the Up row, Down included: D + 1
+    if (sigma == 3) q -= q % 3;
+    else if (m % sigma) return SWEPT_EINVAL;
+    if (q < 1) continue;
+    const int64_t D = q - 1;
     out->push_back({KIND_UP, 0, done, m - 1, n, 0});
     for (int64_t k = 1; k <= D; ++k) {
       const bool split = (k & 1) != 0;
@@ -386,6 +418,7 @@ int tier_default_P(const swept_state* s, int n) {
   // Euler's TIER tiers spread their pressure / flux work over all threads of the CTA: one thread per point
   // (measured: 256 threads per tile are best, more only add barrier cost)
   if (s->problem == SWEPT_EULER) return n <= 256 ? 1 : (n <= 2048 ? 2 : 4);
+  if (s->problem == SWEPT_KS3) return n <= 1024 ? 1 : (n <= 2048 ? 2 : 4);
   const int pmax = 4, tmax = 1024;
   int P = std::min(pmax, std::max(1, n / 256));
   while (P < pmax && n / P > tmax) P *= 2;
@@ -406,7 +439,7 @@ void default_tile(const swept_state* s, int* n_io, int* flavor_io, int* P_io) {
   // CHAR flavour on wide tiles, Euler (about 250 live registers per point) with the TIER flavour
   // fully default call (no width, no flavour, nothing tuned) on a large periodic heat / KS problem: the persistent
   // FLOW launch at the width measured best on B200 (N >= 2^19)
-  if (n == 0 && flavor == SWEPT_FLAVOR_AUTO && !s->bc && s->problem != SWEPT_EULER && s->N >= (1 << 19)) {
+  if (n == 0 && flavor == SWEPT_FLAVOR_AUTO && !s->bc && (s->problem == SWEPT_HEAT || s->problem == SWEPT_KS) && s->N >= (1 << 19)) {
     const int cand = s->problem == SWEPT_HEAT ? 512 : 1024;
     if (tile_ok(s, SWEPT_FLAVOR_FLOW, cand, 0)) {
       *n_io = cand;
@@ -416,7 +449,7 @@ void default_tile(const swept_state* s, int* n_io, int* flavor_io, int* P_io) {
     }
   }
   const bool want_char = flavor == SWEPT_FLAVOR_CHAR ||
-                         (flavor == SWEPT_FLAVOR_AUTO && s->problem != SWEPT_EULER && !s->bc);
+                         (flavor == SWEPT_FLAVOR_AUTO && (s->problem == SWEPT_HEAT || s->problem == SWEPT_KS) && !s->bc);
   if (n == 0) {
     if (want_char) {
       for (int cand : {1024, 512, 256, 128, 64})
@@ -492,7 +525,8 @@ bool level_config(const swept_state* s, int n_top, int flavor_top, int P_top, in
   return false;
 }
 
-int run_swept(swept_state* s, int64_t nsteps, int n, int flavor, int P) {
+// Plan a swept run: the cycles (tile widths) and their kernel configurations, then the phase list.
+int plan_swept(swept_state* s, int64_t nsteps, int n, int flavor, int P) {
   const ProblemShape sh = kShape[s->problem];
   default_tile(s, &n, &flavor, &P);
   if (n <= 0) return fail(SWEPT_EUNSUPPORTED, "N=%lld has no admissible tile width", (long long)s->N);
@@ -501,104 +535,133 @@ int run_swept(swept_state* s, int64_t nsteps, int n, int flavor, int P) {
                 "tile_width=%d (flavor %d, P=%d) not admissible for N=%lld", n, flavor, P, (long long)s->N);
   // widths of the cycles: n, then every narrower power of two that has a kernel for this N
   std::vector<int> widths;
-  std::map<int, std::pair<int, int>> cfg;
+  swept_state::Planned& pr = s->pr;
+  pr.cfg.clear();
+  pr.plan.clear();
   for (int w = n; w >= MIN_LEVEL_WIDTH && w >= 8 * sh.h; w /= 2) {
     int fl = 0, Pl = 0;
     if (!level_config(s, n, flavor, P, w, &fl, &Pl)) continue;
     widths.push_back(w);
-    cfg[w] = {fl, Pl};
+    pr.cfg[w] = {fl, Pl};
   }
-  std::vector<swept_phase> plan;
-  const int64_t np = make_plan(nsteps * sh.sigma, widths, sh.h, &plan);
+  const int64_t np = make_plan(nsteps * sh.sigma, widths, sh.h, sh.sigma, &pr.plan);
   if (np < 0) return fail(SWEPT_EINVAL, "cannot plan tile_width=%d", n);
-  int r0 = -1, r1 = -1;  // slabs holding the current two-row state
-  for (size_t ip = 0; ip < plan.size(); ++ip) {
-    const swept_phase& ph = plan[ip];
-    if (ph.kind == KIND_UP && cfg[ph.n].first == SWEPT_FLAVOR_FLOW) {
-      // the whole cycle Up .. Down of this width in one persistent launch
-      size_t jp = ip;
-      while (plan[jp].kind != KIND_DOWN) ++jp;
-      swept::FlowLaunch f{};
-      f.n = ph.n;
-      f.rows = (int)(jp - ip + 1);
-      f.ctas_per_sm = cfg[ph.n].second;
-      f.init = s->slab[s->cur];
-      // buffer 0 = the two slabs after cur, buffer 1 = the third one and cur itself (swept_flow.cuh: hazards)
-      const int a0 = (s->cur + 1) & 3, a1 = (s->cur + 2) & 3, b0 = (s->cur + 3) & 3, b1 = s->cur;
-      f.buf[0][0] = s->slab[a0]; f.buf[0][1] = s->slab[a1];
-      f.buf[1][0] = s->slab[b0]; f.buf[1][1] = s->slab[b1];
-      {
-        TimedScope ts(s, KIND_FLOW, 1);
-        if (int rc = launch_flow(s, f)) return rc;
-      }
-      s->last_launches += 1;
-      s->cur = ((f.rows - 1) & 1) ? b0 : a0;  // the Down row wrote row 0 of its buffer
-      ip = jp;
-      continue;
-    }
-    if (ph.kind == KIND_REMAINDER) {
-      TimedScope ts(s, KIND_REMAINDER, ph.ntiers);
-      if (int rc = run_per_step(s, ph.ntiers / sh.sigma, 0)) return rc;
-      continue;
-    }
-    swept::TileLaunch a{};
-    a.kind = ph.kind;
-    a.n = ph.n;
-    a.shift = ph.shift;
-    a.ntiers = (int)ph.ntiers;
-    a.flavor = cfg[ph.n].first;
-    a.P = cfg[ph.n].second;
-    int o0, o1;
-    if (ph.kind == KIND_UP) {
-      o0 = (s->cur + 1) & 3;
-      o1 = (s->cur + 2) & 3;
-      a.in0 = s->slab[s->cur];
-      a.in1 = nullptr;
-    } else {
-      // the two slabs that are not the input rows
-      int f[2], k = 0;
-      for (int i = 0; i < 4; ++i)
-        if (i != r0 && i != r1) f[k++] = i;
-      o0 = f[0];
-      o1 = f[1];
-      a.in0 = s->slab[r0];
-      a.in1 = s->slab[r1];
-    }
-    a.out0 = s->slab[o0];
-    a.out1 = s->slab[o1];
-    const bool hybrid = s->bc && a.flavor == SWEPT_FLAVOR_CHAR && ph.kind != KIND_UP;  // Up reads no halo
-    if (hybrid) {
-      // The tiles that touch a wall (aligned rows: the first and the last tile; shifted rows: the tile split across
-      // the boundary) go to the TIER kernels, which apply the boundary condition, on a second
-      // stream beside the register-resident launch — the paper's Hybrid idea with a stream in
-      // place of the CPU.  Both read the same input rows and write disjoint ranges of the output rows.
-      if (!s->wall_stream) return fail(SWEPT_ECUDA, "no wall stream (swept_create makes it for SWEPT_BC_PAPER heat)");
-      CUDA_TRY(cudaEventRecord(s->wall_fork, s->stream));
-      CUDA_TRY(cudaStreamWaitEvent(s->wall_stream, s->wall_fork, 0));
-      a.skip_first = ph.shift == 0 ? 1 : 0;
-      a.skip_last = 1;
-      // wall tiles first, so that they are resident before the big launch takes every slot
-      const int K = (int)(s->N / ph.n);
-      swept::TileLaunch w = a;
-      w.flavor = SWEPT_FLAVOR_TIER;
-      w.P = 1;  // one thread per point: the shortest tier latency (measured), and the wall tile is a latency chain
-      w.skip_first = w.skip_last = 0;
-      if (ph.shift == 0) { w.tile_base = 0; w.tile_step = K - 1; w.tile_count = K > 1 ? 2 : 1; }
-      else { w.tile_base = K - 1; w.tile_step = 0; w.tile_count = 1; }
-      if (int rc = launch_tile(s, w, s->wall_stream)) return rc;
-      s->last_launches += 1;
-      CUDA_TRY(cudaEventRecord(s->wall_join, s->wall_stream));
-    }
+  pr.rin[0] = pr.rin[1] = pr.rin[2] = -1;
+  pr.nrows_valid = 0;
+  pr.next = 0;
+  pr.nsteps = nsteps;
+  return 0;
+}
+
+// Launch phase pr.next of the planned run (a FLOW cycle counts as one: it consumes its Up .. Down entries).
+int run_next_phase(swept_state* s) {
+  const ProblemShape sh = kShape[s->problem];
+  swept_state::Planned& pr = s->pr;
+  if (pr.next >= pr.plan.size()) return fail(SWEPT_EINVAL, "no phase left in the planned run");
+  const size_t ip = pr.next;
+  const swept_phase& ph = pr.plan[ip];
+  const int ns = s->nslabs, R = s->rows();
+  if (ph.kind == KIND_UP && pr.cfg[ph.n].first == SWEPT_FLAVOR_FLOW) {
+    // the whole cycle Up .. Down of this width in one persistent launch
+    size_t jp = ip;
+    while (pr.plan[jp].kind != KIND_DOWN) ++jp;
+    swept::FlowLaunch f{};
+    f.n = ph.n;
+    f.rows = (int)(jp - ip + 1);
+    f.ctas_per_sm = pr.cfg[ph.n].second;
+    f.init = s->slab[s->cur];
+    // buffer 0 = the two slabs after cur, buffer 1 = the third one and cur itself (swept_flow.cuh: hazards)
+    const int a0 = (s->cur + 1) & 3, a1 = (s->cur + 2) & 3, b0 = (s->cur + 3) & 3, b1 = s->cur;
+    f.buf[0][0] = s->slab[a0]; f.buf[0][1] = s->slab[a1];
+    f.buf[1][0] = s->slab[b0]; f.buf[1][1] = s->slab[b1];
     {
-      TimedScope ts(s, ph.kind, 1);
-      if (int rc = launch_tile(s, a)) return rc;
+      TimedScope ts(s, KIND_FLOW, 1);
+      if (int rc = launch_flow(s, f)) return rc;
     }
     s->last_launches += 1;
-    if (hybrid) CUDA_TRY(cudaStreamWaitEvent(s->stream, s->wall_join, 0));
-    r0 = o0;
-    r1 = o1;
-    if (ph.kind == KIND_DOWN) s->cur = o0;  // row0 holds the full time level (T is even)
+    s->cur = ((f.rows - 1) & 1) ? b0 : a0;  // the Down row wrote row 0 of its buffer
+    pr.rin[0] = s->cur;
+    pr.nrows_valid = 1;
+    pr.next = jp + 1;
+    return 0;
   }
+  pr.next = ip + 1;
+  if (ph.kind == KIND_REMAINDER) {
+    TimedScope ts(s, KIND_REMAINDER, ph.ntiers);
+    if (int rc = run_per_step(s, ph.ntiers / sh.sigma, 0)) return rc;
+    pr.rin[0] = s->cur;
+    pr.nrows_valid = 1;
+    return 0;
+  }
+  swept::TileLaunch a{};
+  a.kind = ph.kind;
+  a.n = ph.n;
+  a.shift = ph.shift;
+  a.ntiers = (int)ph.ntiers;
+  a.flavor = pr.cfg[ph.n].first;
+  a.P = pr.cfg[ph.n].second;
+  int o[3] = {-1, -1, -1};
+  if (ph.kind == KIND_UP) {
+    for (int r = 0; r < R; ++r) o[r] = (s->cur + 1 + r) % ns;
+    a.in0 = s->slab[s->cur];
+    a.in1 = nullptr;
+  } else {
+    // the slabs that are not the input rows
+    int k = 0;
+    for (int i = 0; i < ns && k < R; ++i)
+      if (i != pr.rin[0] && i != pr.rin[1] && i != pr.rin[2]) o[k++] = i;
+    a.in0 = s->slab[pr.rin[0]];
+    a.in1 = s->slab[pr.rin[1]];
+    if (R == 3) a.in2 = s->slab[pr.rin[2]];
+  }
+  a.out0 = s->slab[o[0]];
+  a.out1 = s->slab[o[1]];
+  if (R == 3) {
+    a.out2 = s->slab[o[2]];
+    a.tmod = (int)(ph.tier0 % 3);  // which stage the phase's first tier is
+  }
+  const bool hybrid = s->bc && a.flavor == SWEPT_FLAVOR_CHAR && ph.kind != KIND_UP;  // Up reads no halo
+  if (hybrid) {
+    // The tiles that touch a wall (aligned rows: the first and the last tile; shifted rows: the tile split across
+    // the boundary) go to the TIER kernels, which apply the boundary condition, on a second
+    // stream beside the register-resident launch — the paper's Hybrid idea with a stream in
+    // place of the CPU.  Both read the same input rows and write disjoint ranges of the output rows.
+    if (!s->wall_stream) return fail(SWEPT_ECUDA, "no wall stream (swept_create makes it for SWEPT_BC_PAPER heat)");
+    CUDA_TRY(cudaEventRecord(s->wall_fork, s->stream));
+    CUDA_TRY(cudaStreamWaitEvent(s->wall_stream, s->wall_fork, 0));
+    a.skip_first = ph.shift == 0 ? 1 : 0;
+    a.skip_last = 1;
+    // wall tiles first, so that they are resident before the big launch takes every slot
+    const int K = (int)(s->N / ph.n);
+    swept::TileLaunch w = a;
+    w.flavor = SWEPT_FLAVOR_TIER;
+    w.P = 1;  // one thread per point: the shortest tier latency (measured), and the wall tile is a latency chain
+    w.skip_first = w.skip_last = 0;
+    if (ph.shift == 0) { w.tile_base = 0; w.tile_step = K - 1; w.tile_count = K > 1 ? 2 : 1; }
+    else { w.tile_base = K - 1; w.tile_step = 0; w.tile_count = 1; }
+    if (int rc = launch_tile(s, w, s->wall_stream)) return rc;
+    s->last_launches += 1;
+    CUDA_TRY(cudaEventRecord(s->wall_join, s->wall_stream));
+  }
+  {
+    TimedScope ts(s, ph.kind, 1);
+    if (int rc = launch_tile(s, a)) return rc;
+  }
+  s->last_launches += 1;
+  if (hybrid) CUDA_TRY(cudaStreamWaitEvent(s->stream, s->wall_join, 0));
+  for (int r = 0; r < 3; ++r) pr.rin[r] = o[r];
+  pr.nrows_valid = R;
+  if (ph.kind == KIND_DOWN) {
+    s->cur = o[0];  // row 0 holds the full time level (T is a multiple of sigma)
+    pr.nrows_valid = 1;
+  }
+  return 0;
+}
+
+int run_swept(swept_state* s, int64_t nsteps, int n, int flavor, int P) {
+  if (int rc = plan_swept(s, nsteps, n, flavor, P)) return rc;
+  while (s->pr.next < s->pr.plan.size())
+    if (int rc = run_next_phase(s)) return rc;
   return 0;
 }
 
@@ -610,7 +673,7 @@ extern "C" {
 const char* swept_last_error(void) { return g_err.c_str(); }
 
 swept_state* swept_create(int problem, int64_t N, double dx, double dt, const swept_params* p) {
-  if (problem < 0 || problem > 2) { fail(SWEPT_EINVAL, "unknown problem %d", problem); return nullptr; }
+  if (problem < 0 || problem > 3) { fail(SWEPT_EINVAL, "unknown problem %d", problem); return nullptr; }
   if (N < 8 || N > (int64_t)1 << 31) { fail(SWEPT_EINVAL, "N out of range"); return nullptr; }
   if (!(dx > 0) || !(dt > 0)) { fail(SWEPT_EINVAL, "dx and dt must be positive"); return nullptr; }
   swept_params q;
@@ -626,12 +689,13 @@ swept_state* swept_create(int problem, int64_t N, double dx, double dt, const sw
   }
   if (q.dtype != SWEPT_F64 && q.dtype != SWEPT_F32) { fail(SWEPT_EINVAL, "bad dtype"); return nullptr; }
   if (q.rk2 != SWEPT_RK2_MIDPOINT && q.rk2 != SWEPT_RK2_HEUN) { fail(SWEPT_EINVAL, "bad rk2"); return nullptr; }
+  if (problem == SWEPT_KS3) q.rk2 = 0;  // its integrator is fixed (SSP-RK3)
   if (q.dtype == SWEPT_F32 && problem != SWEPT_HEAT) {
     fail(SWEPT_EUNSUPPORTED, "FP32 is provided for the heat problem only (BASELINE.json config 2)");
     return nullptr;
   }
   if (q.bc != SWEPT_BC_PERIODIC && q.bc != SWEPT_BC_PAPER) { fail(SWEPT_EINVAL, "bad bc"); return nullptr; }
-  if (q.bc == SWEPT_BC_PAPER && problem == SWEPT_KS) {
+  if (q.bc == SWEPT_BC_PAPER && (problem == SWEPT_KS || problem == SWEPT_KS3)) {
     fail(SWEPT_EUNSUPPORTED, "SWEPT_BC_PAPER: the paper's KS runs are periodic (PAPER.md:356); heat and Euler only");
     return nullptr;
   }
@@ -655,7 +719,7 @@ swept_state* swept_create(int problem, int64_t N, double dx, double dt, const sw
     const double Fo = q.alpha * dt / (dx * dx);
     s->consts[0] = Fo;
     s->consts[1] = 1.0 - 2.0 * Fo;
-  } else if (problem == SWEPT_KS) {
+  } else if (problem == SWEPT_KS || problem == SWEPT_KS3) {
     s->consts[0] = 1.0 / (4.0 * dx);
     s->consts[1] = 1.0 / (dx * dx);
     s->consts[2] = 1.0 / ((dx * dx) * (dx * dx));
@@ -679,7 +743,8 @@ swept_state* swept_create(int problem, int64_t N, double dx, double dt, const sw
     }
   }
   s->slab_bytes = (size_t)kShape[problem].C * (size_t)N * s->elem();
-  for (int i = 0; i < 4; ++i) {
+  s->nslabs = problem == SWEPT_KS3 ? 6 : 4;
+  for (int i = 0; i < s->nslabs; ++i) {
     void* ptr = dev_alloc(s, s->slab_bytes);
     if (!ptr) {
       fail(SWEPT_ENOMEM, "device allocation of %zu bytes failed", s->slab_bytes);
@@ -692,12 +757,15 @@ swept_state* swept_create(int problem, int64_t N, double dx, double dt, const sw
       swept_destroy(s);
       return nullptr;
     }
+    // debugging aid (include/swept.h): every field slab starts as NaNs, so that a kernel reading a value nobody
+    // wrote produces a wrong result instead of a plausible one
+    if (std::getenv("SWEPT_POISON")) cudaMemsetAsync(ptr, 0xFF, s->slab_bytes, s->stream);
   }
   // Scratch of the persistent flavours, sized here for the worst admissible plan so that swept_run never
   // allocates or synchronises: FLOW (periodic heat / KS, N a multiple of its narrowest tile) needs a ticket word,
   // a leave counter, an error word and 2 N/256 flags; PS_RESIDENT one flag line and two exchange lines per CTA.
   cudaError_t e = cudaSuccess;
-  if (problem != SWEPT_EULER && q.bc == SWEPT_BC_PERIODIC && N % FLOW_MIN_WIDTH == 0) {
+  if ((problem == SWEPT_HEAT || problem == SWEPT_KS) && q.bc == SWEPT_BC_PERIODIC && N % FLOW_MIN_WIDTH == 0) {
     s->flow_scratch_ints = 4 + 2 * (size_t)(N / FLOW_MIN_WIDTH);
     s->flow_scratch = (int*)dev_alloc(s, s->flow_scratch_ints * sizeof(int));
     if (s->flow_scratch) e = cudaMemsetAsync(s->flow_scratch, 0, s->flow_scratch_ints * sizeof(int), s->stream);
@@ -741,7 +809,7 @@ void swept_destroy(swept_state* s) {
   }
   if (s->wall_fork) cudaEventDestroy(s->wall_fork);
   if (s->wall_join) cudaEventDestroy(s->wall_join);
-  for (int i = 0; i < 4; ++i) dev_free(s, s->slab[i]);
+  for (int i = 0; i < MAX_SLABS; ++i) dev_free(s, s->slab[i]);
   delete s;
 }
 
@@ -876,12 +944,18 @@ int swept_run(swept_state* s, int64_t nsteps, int32_t tile_width, int variant) {
 }
 
 int64_t swept_plan(int64_t nsub, int32_t n, int32_t h, swept_phase* out, int64_t max_phases) {
+  return swept_plan_sigma(nsub, n, h, 1, out, max_phases);
+}
+
+int64_t swept_plan_sigma(int64_t nsub, int32_t n, int32_t h, int32_t sigma, swept_phase* out, int64_t max_phases) {
   if (h != 1 && h != 2) return fail(SWEPT_EINVAL, "h must be 1 or 2");
+  if (sigma < 1 || sigma > 3) return fail(SWEPT_EINVAL, "sigma must be 1, 2 or 3");
+  if (nsub % sigma) return fail(SWEPT_EINVAL, "nsub must be a whole number of timesteps (a multiple of sigma)");
   if (n < 8 * h || (n & (n - 1))) return fail(SWEPT_EINVAL, "tile width %d not plannable for h=%d", n, h);
   std::vector<int> widths;
   for (int w = n; w == n || (w >= MIN_LEVEL_WIDTH && w >= 8 * h); w /= 2) widths.push_back(w);
   std::vector<swept_phase> plan;
-  const int64_t np = make_plan(nsub, widths, h, &plan);
+  const int64_t np = make_plan(nsub, widths, h, sigma, &plan);
   if (np < 0) return fail(SWEPT_EINVAL, "tile width %d not plannable for h=%d", n, h);
   if (out)
     for (int64_t i = 0; i < np && i < max_phases; ++i) out[i] = plan[(size_t)i];

@@ -1,8 +1,9 @@
 """P10 — exact-integer simulation of the swept schedule, driven by the phase list the
 LIBRARY's host-side planner (`swept_plan`, C ABI, no GPU needed) produces.
 
-State: two ping-pong buffers of two global rows; row p holds, per point, the tier index of the latest value
-of parity p (or None).  Each phase does what a tile kernel does: load rows over [S-h, S+n+h) from the input
+State: two ping-pong buffers of R global rows (R = 2 for one or two sub-timesteps per timestep, R = 3 for the
+three-sub-timestep scheme of row f3); row p holds, per point, the tier index of the latest value
+with tier = p (mod R) (or None).  Each phase does what a tile kernel does: load rows over [S-h, S+n+h) from the input
 buffer, compute its tiers, write rows over [S, S+n) to the output buffer.  Every stencil read is asserted to
 carry exactly the tier the scheme needs (t-1 for the 2h+1 window, t-2 for the own-point base of a final
 stage), so a wrong range, shift, tier count or parity anywhere fails.  Counts are pinned to the paper's
@@ -24,8 +25,9 @@ def active_range(kind, t, n, h):
 
 
 def simulate(N, n, h, sigma, nsub):
-    plan = sw.swept_plan(nsub, n, h)
-    bufs = [[[None] * N, [None] * N], [[None] * N, [None] * N]]
+    R = 3 if sigma == 3 else 2
+    plan = sw.swept_plan(nsub, n, h, sigma)
+    bufs = [[[None] * N for _ in range(R)] for _ in range(2)]
     bufs[0][0] = [0] * N  # tier 0 everywhere in row 0
     cur, updates, launches = 0, 0, 0
     field_tier = 0
@@ -40,31 +42,37 @@ def simulate(N, n, h, sigma, nsub):
         assert n_ph <= n and n % n_ph == 0
         n = n_ph  # remainder cycles use narrower tiles (reading G5)
         src, dst = bufs[cur], bufs[1 - cur]
-        new_dst = [list(dst[0]), list(dst[1])]
+        new_dst = [list(row) for row in dst]
         assert N % n == 0 and shift in (0, n // 2)
         for tile in range(N // n):
             S = (shift + tile * n) % N
             # local copy of [S-h, S+n+h)
-            loc = [[src[r][(S - h + j) % N] for j in range(n + 2 * h)] for r in range(2)]
+            loc = [[src[r][(S - h + j) % N] for j in range(n + 2 * h)] for r in range(R)]
             if kind == UP:
-                loc[1] = [None] * (n + 2 * h)
+                assert tier0 % sigma == 0, "a cycle starts from a full time level"
+                for r in range(1, R):
+                    loc[r] = [None] * (n + 2 * h)
             for t in range(1, ntiers + 1):
                 g = tier0 + t  # global tier
-                par = g % 2
-                assert par == t % 2, "phases must start on even tiers"
+                par = g % R
+                if R == 2:
+                    assert par == t % 2, "phases of the two-row schemes must start on even tiers"
+                stage = g % sigma  # 1 = first stage ... 0 = final stage of the timestep
                 lo, hi = active_range(kind, t, n, h)
                 assert 0 <= lo < hi <= n
                 new_vals = {}
                 for j in range(lo, hi):
                     for d in range(-h, h + 1):
-                        assert loc[1 - par][h + j + d] == g - 1, (kind, t, j, d, loc[1 - par][h + j + d], g - 1)
-                    if sigma == 2 and par == 0:
-                        assert loc[par][h + j] == g - 2
+                        assert loc[(g - 1) % R][h + j + d] == g - 1, (kind, t, j, d, loc[(g - 1) % R][h + j + d], g - 1)
+                    if sigma >= 2 and stage != 1:
+                        # own-point value at the start of the timestep (u^n): always in row 0
+                        back = sigma if stage == 0 else stage
+                        assert (g - back) % R == 0 and loc[0][h + j] == g - back, (kind, t, j, loc[0][h + j], g - back)
                     new_vals[j] = g
                 for j, v in new_vals.items():
                     loc[par][h + j] = v
                 updates += hi - lo
-            rows_out = (0,) if kind == DOWN else (0, 1)
+            rows_out = (0,) if kind == DOWN else tuple(range(R))
             for r in rows_out:
                 for j in range(n):
                     new_dst[r][(S + j) % N] = loc[r][h + j]
@@ -72,7 +80,7 @@ def simulate(N, n, h, sigma, nsub):
         cur = 1 - cur
         if kind == DOWN:
             field_tier = tier0 + ntiers
-            assert field_tier % 2 == 0
+            assert field_tier % sigma == 0 and field_tier % R == 0
             assert all(v == field_tier for v in bufs[cur][0]), "Down must leave a full time level in row 0"
     assert field_tier == nsub
     assert updates == N * nsub, "the swept schedule performs exactly the per-step work (PAPER.md:37)"
@@ -164,3 +172,27 @@ def test_plan_rejects_bad_arguments():
         sw.swept_plan(10, 48, 1)  # not a power of two
     with pytest.raises(sw.SweptError):
         sw.swept_plan(10, 64, 3)
+
+
+@pytest.mark.parametrize("N,n,h,D", [(128, 32, 2, 2), (128, 32, 2, 5), (64, 32, 2, 8), (32, 32, 2, 2), (256, 64, 2, 5),
+                                     (256, 128, 2, 2)])
+def test_schedule_three_subtimesteps(N, n, h, D):
+    # Row f3: three sub-timesteps per timestep on a three-row state.  m = n/(2h) is a power of two,
+    # so a cycle ends on a full timestep only when (D+1) is a multiple of 3, and diamonds start on any stage.
+    m = n // (2 * h)
+    plan, _ = simulate(N, n, h, 3, (D + 1) * m)
+    kinds = [p[0] for p in plan]
+    assert kinds[0] == UP and kinds[-1] == DOWN and len(plan) == D + 2
+    assert {p[2] % 3 for p in plan[1:]} == {0, 1, 2} or D < 3
+
+
+@pytest.mark.parametrize("nsub", [0, 3, 21, 24, 27, 48, 3 * 61, 3 * 200])
+def test_three_subtimesteps_remainder(nsub):
+    # the widest cycle takes the largest multiple of 3 rows of tiles; narrower cycles and per-step stages the rest
+    N, n, h = 128, 64, 2
+    plan, _ = simulate(N, n, h, 3, nsub)
+    for w in {p[4] for p in plan if p[0] != REM}:
+        rows = [p for p in plan if p[4] == w and p[0] != REM]
+        assert (len(rows) - 1) % 3 == 0
+    rem = sum(p[3] for p in plan if p[0] == REM)
+    assert rem % 3 == 0 and rem < 3 * (32 // (2 * h))
