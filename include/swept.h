@@ -226,6 +226,71 @@ int64_t swept_plan(int64_t nsub, int32_t n, int32_t h, swept_phase* out, int64_t
  * any tier: tier0 % 3 tells the kernel which stage its first tier is. */
 int64_t swept_plan_sigma(int64_t nsub, int32_t n, int32_t h, int32_t sigma, swept_phase* out, int64_t max_phases);
 
+/* ---- sharding over several GPUs ------------------------------------------
+ * The paper's motivation is distributed memory: a swept phase needs ONE exchange with the neighbour where a
+ * per-step scheme needs one per sub-timestep.  Here the N points are cut into `nshards`
+ * contiguous blocks of n_local = N / nshards points (a whole number of tiles), one swept_state per block, normally
+ * one per GPU.  A shard keeps its own points 0 .. n_local-1 and a ghost zone of `tile_width` points behind them
+ * (local points n_local .. n_local + tile_width - 1, which is also where its negative local points -1, -2, ... live:
+ * the shard's array is periodic in n_local + tile_width).  On a shifted row of tiles the shard computes the tile that
+ * straddles its right end, i.e. the first half tile of its right neighbour, and hands it over afterwards; before a
+ * shifted row it receives the neighbour's first half tile (plus h halo points).  So there is exactly one message per
+ * phase and neighbour pair, alternating in direction, of rows x C x (tile_width/2 + h) values — the paper's edge
+ * hand-off across the GPU boundary.  The per-step remainder (fewer than 16 sub-timesteps) is done
+ * with one exchange of ntiers*h points each way, after which the shards step independently.  Results are bit-identical
+ * to the unsharded run (tests/test_gpu_shard.py).  The tiles a shard computes inside its ghost zone are redundant work
+ * (one tile in n_local/tile_width + 1); whatever they write is overwritten by the next message before it is read.
+ *
+ * A shard state supports swept_write / swept_read / swept_sync / swept_device_ptr-free use as below; swept_run on it
+ * fails (a shard cannot advance alone).  Only the phase-wise flavours (TIER, CHAR) exist for shards. */
+
+/* One edge exchange of a sharded run.  Coordinates are LOCAL points of the sender / receiver (0 = first own point;
+ * n_local .. = ghost zone; negative = left halo, stored at the end of the ghost zone). */
+typedef struct {
+  int32_t after_phase; /* happens after this entry of the phase list and before the next one (-1: before the first) */
+  int32_t dir;         /* +1: every shard sends to its right neighbour (shard+1 mod nshards), -1: to its left one   */
+  int64_t src_off;     /* first point sent, sender's local coordinates                                              */
+  int64_t dst_off;     /* where it lands, receiver's local coordinates                                              */
+  int32_t count;       /* points                                                                                    */
+  int32_t rows;        /* rows of the inter-launch state sent (all of them, or 1 = the full time level)             */
+} swept_exchange;
+
+/* swept_shard_exchanges — host-only: the exchanges that go with a phase list from swept_plan / swept_plan_sigma for
+ * shards of n_local points (rows_state = 2, or 3 for sigma = 3).  Writes at most max_out entries, returns the number
+ * needed (or a negative error code).  The same list holds for every shard. */
+int64_t swept_shard_exchanges(const swept_phase* plan, int64_t nphases, int32_t h, int32_t sigma, int64_t n_local,
+                              swept_exchange* out, int64_t max_out);
+
+/* swept_shard_create — one shard (index `shard` of `nshards`) of a problem of N periodic points advanced with swept
+ * tile width `tile_width`; N % (nshards * tile_width) == 0.  Parameters as swept_create (periodic problems only).
+ * swept_write / swept_read on the returned state move the shard's OWN n_local = N / nshards points per component
+ * (host layout: C arrays of n_local REALs). */
+swept_state* swept_shard_create(int problem, int64_t N, int32_t nshards, int32_t shard, int32_t tile_width, double dx,
+                                double dt, const swept_params* p);
+
+/* Phase-wise execution, for a caller that owns the transport (one process per GPU: torch.distributed / NCCL):
+ *   swept_shard_begin(s, nsteps, flavor)  plan `nsteps` timesteps (flavor: SWEPT_FLAVOR_AUTO / _TIER / _CHAR with the
+ *                                         group in bits 8..15); returns the number of phases, the same on every shard
+ *   swept_shard_exchange_list(s, out, max) the exchanges of that plan (as swept_shard_exchanges)
+ *   swept_shard_phase(s)                  enqueue the next phase on the state's stream
+ *   swept_shard_pack(s, x, buf)           enqueue the gather of exchange x into the DEVICE buffer buf
+ *                                         (swept_shard_message_bytes(s, x) bytes)
+ *   swept_shard_unpack(s, x, buf)         enqueue the scatter of a received message
+ *   swept_shard_end(s)                    close the run (step counter)
+ * Order per phase i: phase; then for every exchange x with after_phase == i: pack, transport, unpack. */
+int64_t swept_shard_begin(swept_state* s, int64_t nsteps, int flavor);
+int64_t swept_shard_exchange_list(swept_state* s, swept_exchange* out, int64_t max_out);
+int64_t swept_shard_message_bytes(swept_state* s, int64_t x);
+int swept_shard_phase(swept_state* s);
+int swept_shard_pack(swept_state* s, int64_t x, void* device_buf);
+int swept_shard_unpack(swept_state* s, int64_t x, const void* device_buf);
+int swept_shard_end(swept_state* s);
+
+/* swept_shard_run — all shards in ONE process (shards[i] = shard i; on one device or on several with peer access):
+ * runs the phases of every shard on its own stream and moves each message with one cudaMemcpyAsync between the
+ * shards' staging buffers, ordered by events (no host synchronisation).  Asynchronous like swept_run. */
+int swept_shard_run(swept_state* const* shards, int32_t nshards, int64_t nsteps, int flavor);
+
 /* ---- measurement helpers --------------------------------------------------------------------------- */
 
 /* swept_probe_fp64 — run a register-only DFMA chain on every SM of `device` and return FP64 pipe

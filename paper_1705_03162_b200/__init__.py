@@ -44,6 +44,11 @@ class swept_phase(Structure):
                 ("n", c_int32), ("reserved", c_int32)]
 
 
+class swept_exchange(Structure):
+    _fields_ = [("after_phase", c_int32), ("dir", c_int32), ("src_off", c_int64), ("dst_off", c_int64),
+                ("count", c_int32), ("rows", c_int32)]
+
+
 class SweptError(RuntimeError):
     pass
 
@@ -86,6 +91,23 @@ def load():
     lib.swept_plan.argtypes = [c_int64, c_int32, c_int32, POINTER(swept_phase), c_int64]
     lib.swept_plan_sigma.restype = c_int64
     lib.swept_plan_sigma.argtypes = [c_int64, c_int32, c_int32, c_int32, POINTER(swept_phase), c_int64]
+    lib.swept_shard_exchanges.restype = c_int64
+    lib.swept_shard_exchanges.argtypes = [POINTER(swept_phase), c_int64, c_int32, c_int32, c_int64,
+                                          POINTER(swept_exchange), c_int64]
+    lib.swept_shard_create.restype = c_void_p
+    lib.swept_shard_create.argtypes = [c_int, c_int64, c_int32, c_int32, c_int32, c_double, c_double,
+                                       POINTER(swept_params)]
+    lib.swept_shard_begin.restype = c_int64
+    lib.swept_shard_begin.argtypes = [c_void_p, c_int64, c_int]
+    lib.swept_shard_exchange_list.restype = c_int64
+    lib.swept_shard_exchange_list.argtypes = [c_void_p, POINTER(swept_exchange), c_int64]
+    lib.swept_shard_message_bytes.restype = c_int64
+    lib.swept_shard_message_bytes.argtypes = [c_void_p, c_int64]
+    lib.swept_shard_phase.argtypes = [c_void_p]
+    lib.swept_shard_pack.argtypes = [c_void_p, c_int64, c_void_p]
+    lib.swept_shard_unpack.argtypes = [c_void_p, c_int64, c_void_p]
+    lib.swept_shard_end.argtypes = [c_void_p]
+    lib.swept_shard_run.argtypes = [POINTER(c_void_p), c_int32, c_int64, c_int]
     lib.swept_probe_fp64.argtypes = [c_int, c_void_p, POINTER(c_double)]
     lib.swept_probe_launch.argtypes = [c_int, c_void_p, c_int, POINTER(c_double)]
     lib.swept_set_phase_timing.argtypes = [c_void_p, c_int]
@@ -221,6 +243,22 @@ def swept_plan(nsub: int, n: int, h: int, sigma: int = 1):
     return [(int(a.kind), int(a.shift), int(a.tier0), int(a.ntiers), int(a.n)) for a in arr[:cnt]]
 
 
+def swept_shard_exchanges(plan, h: int, sigma: int, n_local: int):
+    """Host-only: the edge exchanges that go with a phase list (tuples as returned by :func:`swept_plan`) for shards
+    of ``n_local`` points: [(after_phase, dir, src_off, dst_off, count, rows), ...]."""
+    lib = load()
+    arr = (swept_phase * max(len(plan), 1))()
+    for a, (kind, shift, tier0, ntiers, n) in zip(arr, plan):
+        a.kind, a.shift, a.tier0, a.ntiers, a.n = kind, shift, tier0, ntiers, n
+    cnt = lib.swept_shard_exchanges(arr, len(plan), h, sigma, n_local, None, 0)
+    if cnt < 0:
+        raise SweptError(f"swept_shard_exchanges: {swept_last_error()}")
+    out = (swept_exchange * max(cnt, 1))()
+    lib.swept_shard_exchanges(arr, len(plan), h, sigma, n_local, out, cnt)
+    return [(int(x.after_phase), int(x.dir), int(x.src_off), int(x.dst_off), int(x.count), int(x.rows))
+            for x in out[:cnt]]
+
+
 def swept_probe_fp64(device: int = -1) -> float:
     out = c_double(0)
     _check(load().swept_probe_fp64(device, _current_stream(), byref(out)))
@@ -307,3 +345,132 @@ class Swept:
             self.close()
         except Exception:
             pass
+
+
+class SweptShards:
+    """A problem of N periodic points cut into contiguous shards (include/swept.h "sharding").
+
+    ``ranks=None``: every shard lives in this process (``swept_shard_run``: one cudaMemcpyAsync per message).
+    ``ranks=(rank, world)``: this process owns shard ``rank`` of ``world`` (one process per GPU) and the messages
+    travel through :func:`_transport` — torch.distributed point-to-point — the only place an 8-GPU box differs.
+    """
+
+    def __init__(self, problem: int, N: int, nshards: int, tile_width: int, dx: float, dt: float, *, rk2: int = RK2_MIDPOINT,
+                 alpha: float = 1.0, gamma: float = 1.4, dtype=np.float64, ranks=None):
+        import torch
+        if not torch.cuda.is_available():
+            raise SweptError("no CUDA device: the swept library has no CPU fallback")
+        lib = load()
+        self.problem, self.N, self.nshards, self.n = problem, N, nshards, tile_width
+        self.np_dtype = np.dtype(dtype)
+        self.h, self.sigma, self.C = PROBLEM_SHAPE[problem]
+        self.n_local = N // nshards
+        self.ranks = ranks
+        a, f = _torch_hooks()
+        self._states = []
+        for k in (range(nshards) if ranks is None else (ranks[0],)):
+            p = swept_params()
+            p.struct_size = ctypes.sizeof(swept_params)
+            p.dtype = F64 if self.np_dtype == np.float64 else F32
+            p.rk2, p.device, p.alpha, p.gamma, p.bc = rk2, -1, alpha, gamma, BC_PERIODIC
+            p.alloc, p.free, p.stream = a, f, _current_stream()
+            h = lib.swept_shard_create(problem, N, nshards, k, tile_width, dx, dt, byref(p))
+            if not h:
+                self.close()
+                raise SweptError(f"swept_shard_create failed: {swept_last_error()}")
+            self._states.append(h)
+
+    @classmethod
+    def from_workload(cls, w, nshards: int, tile_width: int, ranks=None) -> "SweptShards":
+        s = cls(w.problem, w.N, nshards, tile_width, w.dx, w.dt, rk2=w.rk2, alpha=w.alpha, gamma=w.gamma, ranks=ranks)
+        s.write(w.u0)
+        return s
+
+    def _own(self, k: int, field: np.ndarray) -> np.ndarray:
+        """Shard k's points of a global component-major field."""
+        f = field.reshape(self.C, self.N)[:, k * self.n_local:(k + 1) * self.n_local]
+        return np.ascontiguousarray(f, dtype=self.np_dtype).reshape(-1)
+
+    def write(self, u0: np.ndarray) -> None:
+        self._keep = []
+        ks = range(self.nshards) if self.ranks is None else (self.ranks[0],)
+        for h, k in zip(self._states, ks):
+            buf = self._own(k, np.asarray(u0))
+            swept_set_stream(h, _current_stream())
+            swept_write(h, buf)
+            self._keep.append(buf)
+
+    def read(self) -> np.ndarray:
+        """The global field (single process) or this rank's own points (one process per shard)."""
+        parts = []
+        for h in self._states:
+            out = np.empty(self.C * self.n_local, dtype=self.np_dtype)
+            swept_set_stream(h, _current_stream())
+            swept_read(h, out)
+            parts.append(out.reshape(self.C, self.n_local))
+        return np.concatenate(parts, axis=1).reshape(-1)
+
+    def run(self, nsteps: int, flavor: int = FLAVOR_AUTO, group: int = 0) -> None:
+        lib = load()
+        for h in self._states:
+            swept_set_stream(h, _current_stream())
+        if self.ranks is None:
+            arr = (c_void_p * len(self._states))(*self._states)
+            _check(lib.swept_shard_run(arr, len(self._states), nsteps, flavor | (group << 8)))
+            return
+        import torch
+        h = self._states[0]
+        nph = lib.swept_shard_begin(h, nsteps, flavor | (group << 8))
+        if nph < 0:
+            raise SweptError(f"swept_shard_begin: {swept_last_error()}")
+        nx = lib.swept_shard_exchange_list(h, None, 0)
+        xs = (swept_exchange * max(nx, 1))()
+        lib.swept_shard_exchange_list(h, xs, nx)
+        ix = 0
+        for i in range(-1, nph):
+            if i >= 0:
+                _check(lib.swept_shard_phase(h))
+            while ix < nx and xs[ix].after_phase == i:
+                nbytes = lib.swept_shard_message_bytes(h, ix)
+                send = torch.empty(nbytes, dtype=torch.uint8, device="cuda")
+                recv = torch.empty(nbytes, dtype=torch.uint8, device="cuda")
+                _check(lib.swept_shard_pack(h, ix, c_void_p(send.data_ptr())))
+                _transport(send, recv, int(xs[ix].dir), self.ranks[0], self.ranks[1])
+                _check(lib.swept_shard_unpack(h, ix, c_void_p(recv.data_ptr())))
+                ix += 1
+        _check(lib.swept_shard_end(h))
+
+    @property
+    def last_launches(self) -> int:
+        return sum(int(load().swept_last_launches(h)) for h in self._states)
+
+    def close(self) -> None:
+        for h in getattr(self, "_states", []):
+            swept_destroy(h)
+        self._states = []
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+def _transport(send, recv, direction: int, rank: int, world: int) -> None:
+    """Move one edge message to the neighbour in `direction` (+1 right, -1 left) and receive the matching one from
+    the other side, with torch.distributed point-to-point operations on the current stream's tensors.  NCCL moves
+    device tensors directly (NVLink / NVSwitch); gloo (CPU tests, hosts without NCCL) goes through host copies."""
+    import torch
+    import torch.distributed as dist
+    dst, src = (rank + direction) % world, (rank - direction) % world
+    if dist.get_backend() == "nccl":
+        ops = [dist.P2POp(dist.isend, send, dst), dist.P2POp(dist.irecv, recv, src)]
+        for r in dist.batch_isend_irecv(ops):
+            r.wait()
+        return
+    s_host = send.cpu()
+    r_host = torch.empty_like(s_host)
+    reqs = [dist.isend(s_host, dst), dist.irecv(r_host, src)]
+    for r in reqs:
+        r.wait()
+    recv.copy_(r_host)

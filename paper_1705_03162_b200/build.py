@@ -17,7 +17,7 @@ CSRC = os.path.join(HERE, "csrc")
 BUILD = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libswept_b200.so")
 # (source, object stem, extra defines); the Euler swept kernels are compiled in six parallel slices
-SOURCES = [("swept_api.cu", "swept_api", []), ("probes.cu", "probes", []),
+SOURCES = [("swept_api.cu", "swept_api", []), ("probes.cu", "probes", []), ("shard_kernels.cu", "shard_kernels", []),
            ("kernels_heat.cu", "kernels_heat", []), ("kernels_ks.cu", "kernels_ks", []),
            ("kernels_ks3.cu", "kernels_ks3", []),
            ("kernels_euler.cu", "kernels_euler", [])]

@@ -76,6 +76,20 @@ inline size_t resident_scratch_bytes(int max_ctas) {
 }
 constexpr int RESIDENT_MAX_CTAS = 4096;
 
+// edge of a shard <-> contiguous message buffer (shard_kernels.cu)
+struct ShardCopy {
+  void* rows[3];   // row slabs (nrows of them used), component c at rows[r] + c * Next elements
+  int nrows, C;
+  int64_t Next;    // points of the shard's extended (own + ghost) array
+  int64_t off;     // first local point of the edge (periodic in Next; may be negative)
+  int count;       // points
+  void* buf;       // device buffer of nrows * C * count elements, [row][component][point]
+  int elem;        // bytes per element (8 or 4)
+  cudaStream_t stream;
+  bool pack;       // true: rows -> buf; false: buf -> rows
+};
+int launch_shard_copy(const ShardCopy& a);
+
 // dtype: 0 f64, 1 f32.  rk2: 0 midpoint, 1 Heun.  Return cudaError_t as int, or -1000 if the
 // combination has no kernel.
 int launch_per_step_heat(int dtype, const PerStepLaunch& a);

@@ -8,6 +8,7 @@
 #include <algorithm>
 #include <cmath>
 #include <cstdarg>
+#include <cstddef>
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
@@ -115,6 +116,17 @@ struct swept_state {
     size_t next = 0;
     int64_t nsteps = 0;
   } pr;
+  // shard mode (swept_shard_create): this state holds n_local own points and a ghost zone of shard_n points behind
+  // them; N = shard_nloc + shard_n is the extent of its (periodic) arrays
+  int64_t shard_nloc = 0;
+  int shard_n = 0, nshards = 0, shard_index = 0;
+  void* shard_send = nullptr;  // staging buffers of swept_shard_run: one message each
+  void* shard_recv = nullptr;
+  size_t shard_buf_bytes = 0;
+  std::vector<swept_exchange> xch;  // exchanges of the planned run
+  cudaEvent_t shard_packed = nullptr, shard_send_free = nullptr;
+  bool shard_send_busy = false;
+  bool is_shard() const { return nshards > 0; }
   void* resident_scratch = nullptr;  // flags + exchange slots of the resident per-step kernel
   bool resident_pending_check = false;  // a FLOW launch has run since the error word was last read
   size_t elem() const { return dtype == SWEPT_F64 ? 8 : 4; }
@@ -803,6 +815,10 @@ void swept_destroy(swept_state* s) {
   for (cudaEvent_t e : s->event_pool) cudaEventDestroy(e);
   dev_free(s, s->flow_scratch);
   dev_free(s, s->resident_scratch);
+  dev_free(s, s->shard_send);
+  dev_free(s, s->shard_recv);
+  if (s->shard_packed) cudaEventDestroy(s->shard_packed);
+  if (s->shard_send_free) cudaEventDestroy(s->shard_send_free);
   if (s->wall_stream) {
     cudaStreamSynchronize(s->wall_stream);
     cudaStreamDestroy(s->wall_stream);
@@ -851,6 +867,19 @@ int swept_sync(swept_state* s) {
   return check_flow_error(s);
 }
 
+// The field between a slab and a caller's buffer.  A shard's slab has N = n_local + ghost points per component, the
+// caller's buffer only the n_local own points (include/swept.h): a strided copy.
+static int copy_field(swept_state* s, void* dst, const void* src, bool to_slab, cudaMemcpyKind kind) {
+  if (!s->is_shard()) {
+    CUDA_TRY(cudaMemcpyAsync(dst, src, s->slab_bytes, kind, s->stream));
+    return 0;
+  }
+  const size_t own = (size_t)s->shard_nloc * s->elem(), ext = (size_t)s->N * s->elem();
+  CUDA_TRY(cudaMemcpy2DAsync(dst, to_slab ? ext : own, src, to_slab ? own : ext, own, (size_t)kShape[s->problem].C, kind,
+                             s->stream));
+  return 0;
+}
+
 // Dirichlet end states of the Euler tube = the initial states of the first and last cell.  The
 // captured per-step graphs hold them as kernel arguments: new values invalidate the cache.
 static int set_end_states(swept_state* s, const double (&v)[6]) {
@@ -875,7 +904,7 @@ int swept_write(swept_state* s, const void* host_buf) {
     }
     if (int rc = set_end_states(s, v)) return rc;
   }
-  CUDA_TRY(cudaMemcpyAsync(s->slab[s->cur], host_buf, s->slab_bytes, cudaMemcpyHostToDevice, s->stream));
+  if (int rc = copy_field(s, s->slab[s->cur], host_buf, true, cudaMemcpyHostToDevice)) return rc;
   s->steps_done = 0;
   return 0;
 }
@@ -894,7 +923,7 @@ int swept_write_device(swept_state* s, const void* device_buf) {
     CUDA_TRY(cudaStreamSynchronize(s->stream));
     if (int rc = set_end_states(s, v)) return rc;
   }
-  CUDA_TRY(cudaMemcpyAsync(s->slab[s->cur], device_buf, s->slab_bytes, cudaMemcpyDeviceToDevice, s->stream));
+  if (int rc = copy_field(s, s->slab[s->cur], device_buf, true, cudaMemcpyDeviceToDevice)) return rc;
   s->steps_done = 0;
   return 0;
 }
@@ -902,7 +931,7 @@ int swept_write_device(swept_state* s, const void* device_buf) {
 int swept_read(swept_state* s, void* host_buf) {
   if (!s || !host_buf) return fail(SWEPT_EINVAL, "null argument");
   if (int rc = set_device(s)) return rc;
-  CUDA_TRY(cudaMemcpyAsync(host_buf, s->slab[s->cur], s->slab_bytes, cudaMemcpyDeviceToHost, s->stream));
+  if (int rc = copy_field(s, host_buf, s->slab[s->cur], false, cudaMemcpyDeviceToHost)) return rc;
   CUDA_TRY(cudaStreamSynchronize(s->stream));
   return check_flow_error(s);
 }
@@ -915,6 +944,8 @@ int swept_run_flavor(swept_state* s, int64_t nsteps, int32_t tile_width, int var
   if (!s) return fail(SWEPT_EINVAL, "null state");
   if (nsteps < 0) return fail(SWEPT_EINVAL, "nsteps must be >= 0");
   if (tile_width < 0) return fail(SWEPT_EINVAL, "tile_width must be >= 0");
+  if (s->is_shard())
+    return fail(SWEPT_EINVAL, "a shard cannot advance alone: use swept_shard_run or the swept_shard_* phase calls");
   if (int rc = set_device(s)) return rc;
   s->last_launches = 0;
   int rc;
@@ -962,6 +993,205 @@ int64_t swept_plan_sigma(int64_t nsub, int32_t n, int32_t h, int32_t sigma, swep
   return np;
 }
 
+// ---- sharding (include/swept.h: "sharding over several GPUs") ---------------------------------------------------
+int64_t swept_shard_exchanges(const swept_phase* plan, int64_t nphases, int32_t h, int32_t sigma, int64_t n_local,
+                              swept_exchange* out, int64_t max_out) {
+  if (!plan || nphases < 0 || (h != 1 && h != 2) || sigma < 1 || sigma > 3 || n_local <= 0)
+    return fail(SWEPT_EINVAL, "bad argument");
+  const int R = sigma == 3 ? 3 : 2;
+  int64_t cnt = 0;
+  auto emit = [&](int after, int dir, int64_t src, int64_t dst, int count, int rows) {
+    if (out && cnt < max_out) out[cnt] = swept_exchange{after, dir, src, dst, count, rows};
+    ++cnt;
+  };
+  for (int64_t i = 0; i < nphases; ++i) {
+    const swept_phase& ph = plan[i];
+    if (ph.kind == KIND_REMAINDER) {
+      // per-step stages: one exchange of ntiers * h points each way, then every shard steps on its own (the valid
+      // part of the ghost zone shrinks by h per sub-timestep and never reaches the own points)
+      const int g = (int)ph.ntiers * h;
+      emit((int)i - 1, +1, n_local - g, -g, g, 1);
+      emit((int)i - 1, -1, 0, n_local, g, 1);
+    } else if (ph.kind == KIND_DOWN) {
+      // shifted Down: the tile straddling the right end left the neighbour's first half tile at the final level
+      if (ph.shift != 0) emit((int)i, +1, n_local, 0, ph.n / 2, 1);
+    } else if (ph.shift == 0) {
+      // aligned row done, a shifted row follows: its straddling tile needs the right neighbour's first half tile + halo
+      emit((int)i, -1, 0, n_local, ph.n / 2 + h, R);
+    } else {
+      // shifted row done, an aligned row follows: hand the neighbour its first half tile back, with its left halo
+      emit((int)i, +1, n_local - h, -h, ph.n / 2 + h, R);
+    }
+  }
+  return cnt;
+}
+
+swept_state* swept_shard_create(int problem, int64_t N, int32_t nshards, int32_t shard, int32_t tile_width, double dx,
+                                double dt, const swept_params* p) {
+  if (nshards < 1 || shard < 0 || shard >= nshards) { fail(SWEPT_EINVAL, "bad shard index %d of %d", shard, nshards); return nullptr; }
+  if (tile_width < 32 || (tile_width & (tile_width - 1)) || tile_width > 4096) {
+    fail(SWEPT_EINVAL, "tile_width must be a power of two in 32..4096");
+    return nullptr;
+  }
+  if (N <= 0 || N % ((int64_t)nshards * tile_width)) {
+    fail(SWEPT_EINVAL, "N must be a multiple of nshards * tile_width");
+    return nullptr;
+  }
+  if (p && p->struct_size >= offsetof(swept_params, bc) + sizeof(int32_t) && p->bc != SWEPT_BC_PERIODIC) {
+    fail(SWEPT_EUNSUPPORTED, "shards are built for the periodic problems");
+    return nullptr;
+  }
+  const int64_t nloc = N / nshards;
+  swept_state* s = swept_create(problem, nloc + tile_width, dx, dt, p);
+  if (!s) return nullptr;
+  s->shard_nloc = nloc;
+  s->shard_n = tile_width;
+  s->nshards = nshards;
+  s->shard_index = shard;
+  const ProblemShape sh = kShape[problem];
+  s->shard_buf_bytes = (size_t)s->rows() * sh.C * (size_t)(tile_width / 2 + sh.h) * s->elem();
+  s->shard_send = dev_alloc(s, s->shard_buf_bytes);
+  s->shard_recv = dev_alloc(s, s->shard_buf_bytes);
+  cudaError_t e = cudaEventCreateWithFlags(&s->shard_packed, cudaEventDisableTiming);
+  if (e == cudaSuccess) e = cudaEventCreateWithFlags(&s->shard_send_free, cudaEventDisableTiming);
+  if (!s->shard_send || !s->shard_recv || e != cudaSuccess) {
+    fail(e != cudaSuccess ? SWEPT_ECUDA : SWEPT_ENOMEM, "swept_shard_create: staging buffers / events");
+    swept_destroy(s);
+    return nullptr;
+  }
+  return s;
+}
+
+int64_t swept_shard_begin(swept_state* s, int64_t nsteps, int flavor) {
+  if (!s || !s->is_shard()) return fail(SWEPT_EINVAL, "not a shard state");
+  if (nsteps < 0) return fail(SWEPT_EINVAL, "nsteps must be >= 0");
+  if (int rc = set_device(s)) return rc;
+  const int fl = flavor & 0xff, P = (flavor >> 8) & 0xff;
+  if (fl != SWEPT_FLAVOR_AUTO && fl != SWEPT_FLAVOR_TIER && fl != SWEPT_FLAVOR_CHAR)
+    return fail(SWEPT_EUNSUPPORTED, "shards run the phase-wise flavours (TIER, CHAR); flavor %d is not one", fl);
+  s->last_launches = 0;
+  if (int rc = plan_swept(s, nsteps, s->shard_n, fl, P)) return rc;
+  const ProblemShape sh = kShape[s->problem];
+  const int64_t nx = swept_shard_exchanges(s->pr.plan.data(), (int64_t)s->pr.plan.size(), sh.h, sh.sigma, s->shard_nloc,
+                                           nullptr, 0);
+  if (nx < 0) return nx;
+  s->xch.resize((size_t)nx);
+  swept_shard_exchanges(s->pr.plan.data(), (int64_t)s->pr.plan.size(), sh.h, sh.sigma, s->shard_nloc, s->xch.data(), nx);
+  for (const swept_exchange& x : s->xch)
+    // both halves of the per-step remainder's exchange (dst_off != 0, one row) land in the ghost zone
+    if ((size_t)x.rows * sh.C * (size_t)x.count * s->elem() > s->shard_buf_bytes ||
+        (x.rows == 1 && x.dst_off != 0 && 2 * x.count > s->shard_n))
+      return fail(SWEPT_EINVAL, "exchange of %d points does not fit the ghost zone of %d", x.count, s->shard_n);
+  return (int64_t)s->pr.plan.size();
+}
+
+int64_t swept_shard_exchange_list(swept_state* s, swept_exchange* out, int64_t max_out) {
+  if (!s || !s->is_shard()) return fail(SWEPT_EINVAL, "not a shard state");
+  for (int64_t i = 0; out && i < (int64_t)s->xch.size() && i < max_out; ++i) out[i] = s->xch[(size_t)i];
+  return (int64_t)s->xch.size();
+}
+
+int64_t swept_shard_message_bytes(swept_state* s, int64_t x) {
+  if (!s || !s->is_shard() || x < 0 || x >= (int64_t)s->xch.size()) return fail(SWEPT_EINVAL, "bad exchange index");
+  const swept_exchange& e = s->xch[(size_t)x];
+  return (int64_t)e.rows * kShape[s->problem].C * (int64_t)e.count * (int64_t)s->elem();
+}
+
+int swept_shard_phase(swept_state* s) {
+  if (!s || !s->is_shard()) return fail(SWEPT_EINVAL, "not a shard state");
+  if (int rc = set_device(s)) return rc;
+  return run_next_phase(s);
+}
+
+static int shard_copy(swept_state* s, int64_t x, void* buf, bool pack) {
+  if (!s || !s->is_shard() || !buf) return fail(SWEPT_EINVAL, "bad argument");
+  if (x < 0 || x >= (int64_t)s->xch.size()) return fail(SWEPT_EINVAL, "bad exchange index");
+  if (int rc = set_device(s)) return rc;
+  const swept_exchange& e = s->xch[(size_t)x];
+  swept::ShardCopy c{};
+  if (e.rows == 1) {
+    c.rows[0] = s->slab[s->cur];  // the full time level (after Down, and before the per-step remainder)
+  } else {
+    for (int r = 0; r < e.rows; ++r) {
+      if (s->pr.rin[r] < 0) return fail(SWEPT_EINVAL, "exchange %lld before its phase has run", (long long)x);
+      c.rows[r] = s->slab[s->pr.rin[r]];
+    }
+  }
+  c.nrows = e.rows;
+  c.C = kShape[s->problem].C;
+  c.Next = s->N;
+  c.off = pack ? e.src_off : e.dst_off;
+  c.count = e.count;
+  c.buf = buf;
+  c.elem = (int)s->elem();
+  c.stream = s->stream;
+  c.pack = pack;
+  const int rc = swept::launch_shard_copy(c);
+  if (rc != 0) return fail(SWEPT_ECUDA, "shard %s: %s", pack ? "pack" : "unpack", cudaGetErrorString((cudaError_t)rc));
+  s->last_launches += 1;
+  return 0;
+}
+
+int swept_shard_pack(swept_state* s, int64_t x, void* device_buf) { return shard_copy(s, x, device_buf, true); }
+int swept_shard_unpack(swept_state* s, int64_t x, const void* device_buf) {
+  return shard_copy(s, x, const_cast<void*>(device_buf), false);
+}
+
+int swept_shard_end(swept_state* s) {
+  if (!s || !s->is_shard()) return fail(SWEPT_EINVAL, "not a shard state");
+  if (s->pr.next != s->pr.plan.size()) return fail(SWEPT_EINVAL, "the planned run has phases left");
+  s->steps_done += s->pr.nsteps;
+  return 0;
+}
+
+int swept_shard_run(swept_state* const* shards, int32_t nshards, int64_t nsteps, int flavor) {
+  if (!shards || nshards < 1) return fail(SWEPT_EINVAL, "bad argument");
+  int64_t np = -1;
+  for (int i = 0; i < nshards; ++i) {
+    swept_state* s = shards[i];
+    if (!s || !s->is_shard() || s->nshards != nshards || s->shard_index != i)
+      return fail(SWEPT_EINVAL, "shards[%d] is not shard %d of %d", i, i, nshards);
+    const int64_t n = swept_shard_begin(s, nsteps, flavor);
+    if (n < 0) return (int)n;
+    if (np >= 0 && (n != np || s->xch.size() != shards[0]->xch.size()))
+      return fail(SWEPT_EINVAL, "the shards planned different runs (different problems or sizes?)");
+    np = n;
+  }
+  const std::vector<swept_exchange>& xch = shards[0]->xch;
+  size_t ix = 0;
+  for (int64_t i = -1; i < np; ++i) {
+    if (i >= 0)
+      for (int k = 0; k < nshards; ++k)
+        if (int rc = swept_shard_phase(shards[k])) return rc;
+    for (; ix < xch.size() && xch[ix].after_phase == (int)i; ++ix) {
+      const int64_t bytes = swept_shard_message_bytes(shards[0], (int64_t)ix);
+      // gather on every sender (after whoever still reads its staging buffer has finished) ...
+      for (int k = 0; k < nshards; ++k) {
+        swept_state* s = shards[k];
+        if (int rc = set_device(s)) return rc;
+        if (s->shard_send_busy) CUDA_TRY(cudaStreamWaitEvent(s->stream, s->shard_send_free, 0));
+        if (int rc = swept_shard_pack(s, (int64_t)ix, s->shard_send)) return rc;
+        CUDA_TRY(cudaEventRecord(s->shard_packed, s->stream));
+      }
+      // ... then ONE copy per message on the receiver's stream (peer-to-peer when the shards sit on two devices),
+      // and the scatter into the receiver's rows
+      for (int k = 0; k < nshards; ++k) {
+        swept_state* s = shards[k];
+        swept_state* d = shards[((k + xch[ix].dir) % nshards + nshards) % nshards];
+        if (int rc = set_device(d)) return rc;
+        CUDA_TRY(cudaStreamWaitEvent(d->stream, s->shard_packed, 0));
+        CUDA_TRY(cudaMemcpyAsync(d->shard_recv, s->shard_send, (size_t)bytes, cudaMemcpyDefault, d->stream));
+        CUDA_TRY(cudaEventRecord(s->shard_send_free, d->stream));
+        s->shard_send_busy = true;
+        if (int rc = swept_shard_unpack(d, (int64_t)ix, d->shard_recv)) return rc;
+      }
+    }
+  }
+  for (int k = 0; k < nshards; ++k)
+    if (int rc = swept_shard_end(shards[k])) return rc;
+  return 0;
+}
+
 int swept_tuned(const swept_state* s, int variant, int32_t* tile_width, int32_t* flavor, int32_t* group) {
   if (!s || (variant != SWEPT_PER_STEP && variant != SWEPT_SWEPT)) return fail(SWEPT_EINVAL, "bad argument");
   if (tile_width) *tile_width = s->tuned_width[variant];
@@ -972,6 +1202,7 @@ int swept_tuned(const swept_state* s, int variant, int32_t* tile_width, int32_t*
 
 int swept_autotune(swept_state* s, int variant, int32_t* best_tile_width) {
   if (!s) return fail(SWEPT_EINVAL, "null state");
+  if (s->is_shard()) return fail(SWEPT_EUNSUPPORTED, "autotune an unsharded state of the same size per GPU instead");
   if (variant != SWEPT_PER_STEP && variant != SWEPT_SWEPT) return fail(SWEPT_EINVAL, "unknown variant");
   if (int rc = set_device(s)) return rc;
   const ProblemShape sh = kShape[s->problem];
