@@ -301,6 +301,32 @@ int swept_probe_fp64(int device, void* stream, double* fp64_lane_ops_per_s);
  * back to back on `stream` (PAPER.md:253 measures the same on the K40c: about 4 us). */
 int swept_probe_launch(int device, void* stream, int count, double* us_per_launch);
 
+/* swept_flow_profile — where the warps of the FLOW flavour spend their time.  on != 0: later FLOW launches of this
+ * state (heat FP64) run an instrumented copy of the kernel that stamps clock64() between the parts of every tile task;
+ * on == 0: back to the plain kernel.  Either way the call synchronises, copies the 8 counters accumulated so far to
+ * the caller's HOST array if it is not NULL — SM cycles summed over all warps spent [0] taking a ticket, [1] waiting
+ * for the two parent tiles, [2] staging the rows, [3] sweeping, [4] storing and publishing; [5] = tiles done — and
+ * clears them. */
+int swept_flow_profile(swept_state* s, int on, uint64_t* counters);
+
+/* swept_probe_chain — cycles per dependent DADD -> DFMA pair (one warp, one chain per lane): the latency a heat
+ * update puts on the critical path of every tier, i.e. the denominator of the latency bound that governs small N
+ * (a tile of n points cannot advance faster than one tier per chain link). */
+int swept_probe_chain(int device, void* stream, double* cycles_per_dadd_dfma);
+
+/* swept_probe_smem — shared-memory read bandwidth of the whole device (conflict-free 16-byte loads from 32 KiB per
+ * CTA, 2 CTAs of 1024 threads per SM), in bytes per second and, if the pointer is given, bytes per clock and SM at
+ * the device's maximum SM clock: the measured counterpart of the nominal 128 B/clk/SM. */
+int swept_probe_smem(int device, void* stream, double* bytes_per_s, double* bytes_per_clk_per_sm);
+
+/* swept_probe_sweep — the characteristic sweep of the CHAR / FLOW flavours (swept_char.cuh, L = 32 lanes per tile) on
+ * ONE SM with no global traffic: 4 * warps_per_scheduler warps each sweep a staged WholeDiamond tile of
+ * 32 * lines_per_lane points (lines_per_lane = 8, 16, 32; problem = SWEPT_HEAT or SWEPT_KS, FP64) several times.
+ * Returns the SM cycles per super-step (all warps) and, if the pointer is given, the fraction of the FP64 pipe's
+ * issue cycles that is busy.  The issue-rate model of DESIGN.md §5.6 is read off this probe. */
+int swept_probe_sweep(int device, void* stream, int problem, int lines_per_lane, int warps_per_scheduler,
+                      double* cycles_per_step, double* fp64_busy);
+
 #ifdef __cplusplus
 }
 #endif

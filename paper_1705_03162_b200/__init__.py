@@ -110,6 +110,10 @@ def load():
     lib.swept_shard_run.argtypes = [POINTER(c_void_p), c_int32, c_int64, c_int]
     lib.swept_probe_fp64.argtypes = [c_int, c_void_p, POINTER(c_double)]
     lib.swept_probe_launch.argtypes = [c_int, c_void_p, c_int, POINTER(c_double)]
+    lib.swept_probe_chain.argtypes = [c_int, c_void_p, POINTER(c_double)]
+    lib.swept_probe_smem.argtypes = [c_int, c_void_p, POINTER(c_double), POINTER(c_double)]
+    lib.swept_probe_sweep.argtypes = [c_int, c_void_p, c_int, c_int, c_int, POINTER(c_double), POINTER(c_double)]
+    lib.swept_flow_profile.argtypes = [c_void_p, c_int, POINTER(c_uint64)]
     lib.swept_set_phase_timing.argtypes = [c_void_p, c_int]
     lib.swept_phase_times.argtypes = [c_void_p, POINTER(c_double), POINTER(c_int64)]
     lib.swept_tuned.argtypes = [c_void_p, c_int, POINTER(c_int32), POINTER(c_int32), POINTER(c_int32)]
@@ -218,6 +222,15 @@ def swept_phase_times(state: int):
     return {KIND_NAMES[k]: (float(ms[k]), int(cnt[k])) for k in range(6)}
 
 
+def swept_flow_profile(state: int, on: bool):
+    """Switch the instrumented FLOW kernel on / off; returns the counters accumulated so far as a dict of SM cycles
+    summed over all warps (ticket, wait_parents, stage, sweep, publish) and the number of tiles."""
+    c = (c_uint64 * 8)()
+    _check(load().swept_flow_profile(state, 1 if on else 0, c))
+    return {"ticket": int(c[0]), "wait_parents": int(c[1]), "stage": int(c[2]), "sweep": int(c[3]),
+            "publish": int(c[4]), "tiles": int(c[5])}
+
+
 def swept_set_stream(state: int, stream: int) -> None:
     _check(load().swept_set_stream(state, stream))
 
@@ -263,6 +276,28 @@ def swept_probe_fp64(device: int = -1) -> float:
     out = c_double(0)
     _check(load().swept_probe_fp64(device, _current_stream(), byref(out)))
     return float(out.value)
+
+
+def swept_probe_chain(device: int = -1) -> float:
+    """Cycles per dependent DADD -> DFMA pair (the critical path of one heat tier)."""
+    out = c_double(0)
+    _check(load().swept_probe_chain(device, _current_stream(), byref(out)))
+    return float(out.value)
+
+
+def swept_probe_smem(device: int = -1):
+    """(bytes per second, bytes per clock per SM) of shared-memory reads on the whole device."""
+    bps, bpc = c_double(0), c_double(0)
+    _check(load().swept_probe_smem(device, _current_stream(), byref(bps), byref(bpc)))
+    return float(bps.value), float(bpc.value)
+
+
+def swept_probe_sweep(problem: int, lines_per_lane: int, warps_per_scheduler: int, device: int = -1):
+    """(SM cycles per super-step, FP64 pipe busy fraction) of the characteristic sweep on one SM, no global traffic."""
+    cyc, busy = c_double(0), c_double(0)
+    _check(load().swept_probe_sweep(device, _current_stream(), problem, lines_per_lane, warps_per_scheduler,
+                                    byref(cyc), byref(busy)))
+    return float(cyc.value), float(busy.value)
 
 
 def swept_probe_launch(count: int = 2000, device: int = -1) -> float:

@@ -53,6 +53,7 @@ struct FlowLaunch {
   int* flags;        // 2 * N/n words, zero (the kernel leaves them zero again; swept_flow.cuh)
   unsigned* ticket;  // 4 words: task counter, sticky error word, leave counter, unused; counters zero
   int ctas_per_sm;   // bits 0..3: resident CTAs (of 4 warps) per SM, 0 = default policy; bit 4: TMA staging
+  unsigned long long* prof = nullptr;  // 8 device counters: run the instrumented kernel (swept_flow_profile)
   const double* consts;
   cudaStream_t stream;
 };

@@ -63,7 +63,7 @@ inline bool flow_ok(int64_t N, int n) {
   return B <= BMAX && B % (2 * Prob::H) == 0 && n / (2 * Prob::H) >= 32;
 }
 
-template <class Prob, int B, bool TMA>
+template <class Prob, int B, bool TMA, bool PROF = false>
 inline int flow_go(const FlowLaunch& a) {
   using R = typename Prob::R;
   constexpr int warps = 4;  // one per scheduler
@@ -74,8 +74,9 @@ inline int flow_go(const FlowLaunch& a) {
     for (int j = 0; j < 2; ++j) f.buf[i][j] = (R*)a.buf[i][j];
   f.N = a.N; f.K = (int)(a.N / a.n); f.rows = a.rows; f.flags = a.flags; f.ticket = a.ticket;
   f.k = round_consts<R>(a.consts);
+  f.prof = a.prof;
   const size_t smem = flow_smem_bytes<Prob>(warps, a.n);
-  auto kern = swept_flow_kernel<Prob, B, TMA>;
+  auto kern = swept_flow_kernel<Prob, B, TMA, PROF>;
   cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (e != cudaSuccess) return (int)e;
   // never launch more CTAs than can be co-resident: waiting tasks must not keep their parents off the machine
@@ -107,6 +108,16 @@ template <class Prob, int BMAX>
 int flow_T(const FlowLaunch& a) {
   if (!flow_ok<Prob, BMAX>(a.N, a.n)) return NO_KERNEL;
   const bool tma = (a.ctas_per_sm & 16) != 0;  // group bit 4: stage the tiles with TMA bulk copies
+  if (a.prof) {  // instrumented kernels (swept_flow_profile): the 3-point FP64 problem, the headline's kernel family
+    if constexpr (Prob::H == 1 && sizeof(typename Prob::R) == 8) {
+      switch (a.n / 32) {
+        case 8: return tma ? flow_go<Prob, 8, true, true>(a) : flow_go<Prob, 8, false, true>(a);
+        case 16: return tma ? flow_go<Prob, 16, true, true>(a) : flow_go<Prob, 16, false, true>(a);
+        case 32: return tma ? flow_go<Prob, 32, true, true>(a) : flow_go<Prob, 32, false, true>(a);
+      }
+    }
+    return NO_KERNEL;
+  }
   switch (a.n / 32) {
     case 8: return tma ? flow_go<Prob, 8, true>(a) : flow_go<Prob, 8, false>(a);
     case 16: if (BMAX >= 16) return tma ? flow_go<Prob, (BMAX >= 16 ? 16 : 8), true>(a) : flow_go<Prob, (BMAX >= 16 ? 16 : 8), false>(a); break;

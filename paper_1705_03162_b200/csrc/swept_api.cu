@@ -104,6 +104,8 @@ struct swept_state {
   int* flow_scratch = nullptr;
   size_t flow_scratch_ints = 0;
   bool flow_pending_check = false;
+  unsigned long long* flow_prof = nullptr;  // 8 counters of the instrumented FLOW kernel (swept_flow_profile)
+  bool flow_prof_on = false;
   cudaStream_t wall_stream = nullptr;  // hybrid wall handling: the wall tiles run here, beside the CHAR launch
   cudaEvent_t wall_fork = nullptr, wall_join = nullptr;
   // the phase list of the swept run being executed (swept_run plans and runs it in one go; the shard driver,
@@ -201,6 +203,7 @@ int launch_flow(swept_state* s, swept::FlowLaunch& a) {
     return fail(SWEPT_EUNSUPPORTED, "no FLOW kernel for this problem / n=%d", a.n);
   a.ticket = (unsigned*)s->flow_scratch;
   a.flags = s->flow_scratch + 4;
+  a.prof = s->flow_prof_on ? s->flow_prof : nullptr;
   int rc;
   switch (s->problem) {
     case SWEPT_HEAT: rc = swept::launch_flow_heat(s->dtype, a); break;
@@ -781,6 +784,8 @@ swept_state* swept_create(int problem, int64_t N, double dx, double dt, const sw
     s->flow_scratch_ints = 4 + 2 * (size_t)(N / FLOW_MIN_WIDTH);
     s->flow_scratch = (int*)dev_alloc(s, s->flow_scratch_ints * sizeof(int));
     if (s->flow_scratch) e = cudaMemsetAsync(s->flow_scratch, 0, s->flow_scratch_ints * sizeof(int), s->stream);
+    s->flow_prof = (unsigned long long*)dev_alloc(s, 8 * sizeof(unsigned long long));
+    if (s->flow_prof && e == cudaSuccess) e = cudaMemsetAsync(s->flow_prof, 0, 8 * sizeof(unsigned long long), s->stream);
   }
   s->resident_scratch = dev_alloc(s, swept::resident_scratch_bytes(swept::RESIDENT_MAX_CTAS));
   if (s->resident_scratch && e == cudaSuccess)
@@ -814,6 +819,7 @@ void swept_destroy(swept_state* s) {
   for (auto& t : s->timed) { cudaEventDestroy(t.e0); cudaEventDestroy(t.e1); }
   for (cudaEvent_t e : s->event_pool) cudaEventDestroy(e);
   dev_free(s, s->flow_scratch);
+  dev_free(s, s->flow_prof);
   dev_free(s, s->resident_scratch);
   dev_free(s, s->shard_send);
   dev_free(s, s->shard_recv);
@@ -857,6 +863,17 @@ int swept_phase_times(swept_state* s, double* ms, int64_t* launches) {
   }
   s->timed.clear();
   cudaGetLastError();
+  return check_flow_error(s);
+}
+
+int swept_flow_profile(swept_state* s, int on, uint64_t* counters) {
+  if (!s) return fail(SWEPT_EINVAL, "null state");
+  if (!s->flow_prof) return fail(SWEPT_EUNSUPPORTED, "this state has no FLOW flavour");
+  if (int rc = set_device(s)) return rc;
+  CUDA_TRY(cudaStreamSynchronize(s->stream));
+  if (counters) CUDA_TRY(cudaMemcpy(counters, s->flow_prof, 8 * sizeof(uint64_t), cudaMemcpyDeviceToHost));
+  CUDA_TRY(cudaMemset(s->flow_prof, 0, 8 * sizeof(uint64_t)));
+  s->flow_prof_on = on != 0;
   return check_flow_error(s);
 }
 

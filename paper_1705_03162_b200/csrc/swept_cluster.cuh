@@ -1,0 +1,189 @@
+// swept_cluster.cuh — swept kernels, flavour CLUSTER: the WHOLE domain inside one thread-block cluster, for the
+// small problems where every other flavour is bound by latency, not by arithmetic (BASELINE.json config 1: N = 2048).
+//
+// The paper names a device-side synchronisation between the rows of tiles as future work and its
+// "Register" variant keeps a 32-point tile in the registers of one warp.  Here:
+//   * one WARP per tile ("node") of n = 32 P points; lane l holds the P contiguous points l P .. l P + P - 1 of both
+//     rows of the two-row working array in registers;
+//   * a tier is one shuffle exchange of the h values either side of a lane's block and P stencil evaluations — no
+//     block barrier, no shared-memory traffic inside a phase; the tile's outermost h halo values are read once per
+//     phase (they do not change during it);
+//   * the whole cycle — UpTriangle, D Split/WholeDiamond rows, DownTriangle (§4.2) — runs in ONE launch: between
+//     two rows every warp writes its tile's rows to the cluster's DISTRIBUTED SHARED MEMORY (point x of the domain
+//     lives in CTA x / chunk at offset x % chunk), one cluster barrier, and every warp reads the rows of its next
+//     tile, half a tile further on (the edges a node passes on), from there — possibly from a
+//     neighbouring SM.  Global memory is touched twice: the Up row reads the time level, the Down row writes it.
+//   * rows ping-pong between two shared-memory buffers, so one barrier per row suffices (a tile reads an h-wide halo
+//     that its neighbour rewrites in the same row: SURVEY.md §8(d) note).
+// What it buys: a tier costs a shuffle round trip plus one dependent DADD -> DFMA (about 50 cycles for P = 4) instead of
+// the 130 cycles per tier the characteristic sweep needs at N = 2048 (its skew and chain latency), and no launch gap or
+// L2 round trip between rows.  Lane efficiency is the paper's ~50 %; irrelevant here, because the bound
+// at these sizes is the dependent chain, not the FP64 pipe.  Same functors, so the same bits.
+#pragma once
+#include <cooperative_groups.h>
+
+#include "common.cuh"
+#include "functors.cuh"
+#include "swept_tier.cuh"
+
+namespace swept {
+
+template <class R>
+struct ClusterArgs {
+  const R* init;  // full time level at the start of the cycle (C components, stride N)
+  R* out;         // full time level at its end
+  int64_t N;
+  int n;          // tile width = 32 P
+  int rows;       // D + 2
+  int chunk;      // points per CTA = warps per CTA * n (a power of two)
+  int chunk_log2;
+  Consts<R> k;
+};
+
+__device__ __forceinline__ double shfl_idx_(double v, int src) { return __shfl_sync(0xffffffffu, v, src); }
+__device__ __forceinline__ float shfl_idx_(float v, int src) { return __shfl_sync(0xffffffffu, v, src); }
+
+// One tier of a warp's tile: source row vs (tier t-1), destination row vd (tier t; holds tier t-2 before), halo values
+// of the source row beyond the tile's ends in hl / hr.  Points [lo, hi) of the tile are updated.
+template <class Prob, int P>
+__device__ __forceinline__ void cluster_tier(const typename Prob::R (&vs)[Prob::C][P], typename Prob::R (&vd)[Prob::C][P],
+                                             const typename Prob::R (&v0)[Prob::C][P],
+                                             const typename Prob::R (&hl)[Prob::C][Prob::H],
+                                             const typename Prob::R (&hr)[Prob::C][Prob::H], const int par, const int lo,
+                                             const int hi, const int lane, const Consts<typename Prob::R>& k) {
+  using R = typename Prob::R;
+  constexpr int H = Prob::H, C = Prob::C;
+  R win[C][P + 2 * H], bs[C][P], o[C][P];
+#pragma unroll
+  for (int c = 0; c < C; ++c) {
+#pragma unroll
+    for (int e = 0; e < H; ++e) {
+      // left neighbours: the top H values of lane - 1; right neighbours: the bottom H values of lane + 1
+      const R fromL = shfl_idx_(vs[c][P - H + e], (lane + 31) & 31);
+      const R fromR = shfl_idx_(vs[c][e], (lane + 1) & 31);
+      win[c][e] = lane == 0 ? hl[c][e] : fromL;
+      win[c][H + P + e] = lane == 31 ? hr[c][e] : fromR;
+    }
+#pragma unroll
+    for (int j = 0; j < P; ++j) {
+      win[c][H + j] = vs[c][j];
+      bs[c][j] = (Prob::SIGMA >= 2 && par != 1) ? v0[c][j] : vs[c][j];  // u^n: row 0
+    }
+  }
+  Prob::template stage<P>(win, bs, o, par, k);
+  const int j0 = lane * P;
+#pragma unroll
+  for (int j = 0; j < P; ++j) {
+    const bool act = j0 + j >= lo && j0 + j < hi;
+#pragma unroll
+    for (int c = 0; c < C; ++c) vd[c][j] = act ? o[c][j] : vd[c][j];
+  }
+}
+
+template <class Prob, int P>
+__global__ void __launch_bounds__(1024) swept_cluster_kernel(const ClusterArgs<typename Prob::R> a) {
+  namespace cg = cooperative_groups;
+  using R = typename Prob::R;
+  constexpr int H = Prob::H, C = Prob::C;
+  static_assert(Prob::ROWS == 2, "two-row schemes");
+  static_assert(P >= H, "a lane's block must hold its neighbour's halo");
+  constexpr int n = 32 * P, m = n / (2 * H);
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  R* sm = reinterpret_cast<R*>(smem_raw);  // [buffer 2][row 2][component C][chunk]
+  cg::cluster_group cluster = cg::this_cluster();
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int wpc = blockDim.x >> 5;
+  const unsigned rank = cluster.block_rank();
+  const int64_t N = a.N;
+  const int64_t k_tile = (int64_t)rank * wpc + warp;
+  const int chunk = a.chunk;
+  // address of point g (0 <= g < N) of (buffer, row, component) in the cluster's distributed shared memory
+  auto dsm = [&](int buf, int row, int c, int64_t g) -> R* {
+    R* local = sm + (size_t)((buf * 2 + row) * C + c) * chunk + (int)(g & (chunk - 1));
+    return cluster.map_shared_rank(local, (unsigned)(g >> a.chunk_log2));
+  };
+  auto wrap = [&](int64_t g) -> int64_t { return g < 0 ? g + N : (g >= N ? g - N : g); };
+
+  R v0[C][P], v1[C][P];  // row 0 (even tiers) and row 1 (odd tiers) of this lane's P points
+  R hl0[C][H], hr0[C][H], hl1[C][H], hr1[C][H];
+  for (int r = 0; r < a.rows; ++r) {
+    const int kind = r == 0 ? KIND_UP : (r == a.rows - 1 ? KIND_DOWN : KIND_WHOLE);
+    const int64_t S = wrap(k_tile * n + ((r & 1) ? n / 2 : 0));
+    const int64_t g0 = wrap(S + lane * P);  // this lane's first point; its P points do not straddle the wrap
+    const int inb = (r + 1) & 1, outb = r & 1;
+    // ---- load the tile's rows (Up: the time level from global memory; tier -1 does not exist)
+    if (kind == KIND_UP) {
+#pragma unroll
+      for (int c = 0; c < C; ++c)
+#pragma unroll
+        for (int j = 0; j < P; ++j) {
+          v0[c][j] = __ldg(a.init + (int64_t)c * N + g0 + j);
+          v1[c][j] = (R)0;
+        }
+#pragma unroll
+      for (int c = 0; c < C; ++c)
+#pragma unroll
+        for (int e = 0; e < H; ++e) hl0[c][e] = hr0[c][e] = hl1[c][e] = hr1[c][e] = (R)0;  // never used by a triangle
+    } else {
+#pragma unroll
+      for (int c = 0; c < C; ++c) {
+        const R* p0 = dsm(inb, 0, c, g0);
+        const R* p1 = dsm(inb, 1, c, g0);
+#pragma unroll
+        for (int j = 0; j < P; ++j) {
+          v0[c][j] = p0[j];
+          v1[c][j] = p1[j];
+        }
+#pragma unroll
+        for (int e = 0; e < H; ++e) {  // the h-wide halo beyond either end of the tile, both rows (all lanes: broadcast)
+          const int64_t gl = wrap(S - H + e), gr = wrap(S + n + e);
+          hl0[c][e] = *dsm(inb, 0, c, gl);
+          hl1[c][e] = *dsm(inb, 1, c, gl);
+          hr0[c][e] = *dsm(inb, 0, c, gr);
+          hr1[c][e] = *dsm(inb, 1, c, gr);
+        }
+      }
+    }
+    // ---- tiers (phases start on even global tiers, so odd relative tiers are predictor / odd-row tiers)
+    const int ntiers = kind == KIND_UP ? m - 1 : (kind == KIND_DOWN ? m : 2 * m - 1);
+    for (int t = 1; t <= ntiers; t += 2) {
+      int lo, hi;
+      if (kind == KIND_UP) tier_range<KIND_UP>(t, n, H, m, lo, hi);
+      else if (kind == KIND_DOWN) tier_range<KIND_DOWN>(t, n, H, m, lo, hi);
+      else tier_range<KIND_WHOLE>(t, n, H, m, lo, hi);
+      cluster_tier<Prob, P>(v0, v1, v0, hl0, hr0, 1, lo, hi, lane, a.k);  // odd tier: reads row 0, writes row 1
+      if (t + 1 <= ntiers) {
+        if (kind == KIND_UP) tier_range<KIND_UP>(t + 1, n, H, m, lo, hi);
+        else if (kind == KIND_DOWN) tier_range<KIND_DOWN>(t + 1, n, H, m, lo, hi);
+        else tier_range<KIND_WHOLE>(t + 1, n, H, m, lo, hi);
+        cluster_tier<Prob, P>(v1, v0, v0, hl1, hr1, 0, lo, hi, lane, a.k);  // even tier: reads row 1, writes row 0
+      }
+    }
+    // ---- hand the rows on: Down leaves the full time level (row 0) in global memory
+    if (kind == KIND_DOWN) {
+#pragma unroll
+      for (int c = 0; c < C; ++c)
+#pragma unroll
+        for (int j = 0; j < P; ++j) a.out[(int64_t)c * N + g0 + j] = v0[c][j];
+    } else {
+#pragma unroll
+      for (int c = 0; c < C; ++c) {
+        R* p0 = dsm(outb, 0, c, g0);
+        R* p1 = dsm(outb, 1, c, g0);
+#pragma unroll
+        for (int j = 0; j < P; ++j) {
+          p0[j] = v0[c][j];
+          p1[j] = v1[c][j];
+        }
+      }
+      cluster.sync();  // release / acquire at cluster scope: every tile of row r is in shared memory
+    }
+  }
+}
+
+template <class Prob>
+inline size_t cluster_smem_bytes(int chunk) {
+  return (size_t)2 * 2 * Prob::C * (size_t)chunk * sizeof(typename Prob::R);
+}
+
+}  // namespace swept

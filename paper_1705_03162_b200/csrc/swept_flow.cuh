@@ -50,6 +50,9 @@ struct FlowArgs {
                      // captured launch can be replayed.  ticket[1] = sticky error word (a dependency wait timed
                      // out), read and cleared by the host.
   Consts<R> k;
+  // PROF kernels only: 8 counters, summed over all warps — SM cycles spent [0] taking a ticket, [1] waiting for the
+  // parents' flags, [2] staging the tile, [3] sweeping, [4] storing and publishing; [5] tiles done
+  unsigned long long* prof;
 };
 
 // polling load: relaxed at GPU scope (no L1 invalidation per poll); the acquire fence follows once the flag is seen
@@ -126,7 +129,9 @@ __device__ __forceinline__ void fence_proxy_async_all() { asm volatile("fence.pr
 // TMA = false: by 16-byte ld.global.cg / st.global of all 32 lanes.
 // Same task loop, same sweep, same protocol.  Both are kept because the compiler's code for the sweep loop depends on
 // which one surrounds it (profiles/r2_flow_phases.md); swept_autotune measures both.
-template <class Prob, int B, bool TMA>
+// PROF = true: the same kernel with clock64() stamps between the parts of a task (swept_flow_profile; the timings
+// in profiles/r2_flow_phases.md).
+template <class Prob, int B, bool TMA, bool PROF = false>
 __global__ void __launch_bounds__(128) swept_flow_kernel(const FlowArgs<typename Prob::R> a) {
   using R = typename Prob::R;
   constexpr int H = Prob::H, C = Prob::C, PAD = Pad16<R>::value, L = 32;
@@ -140,6 +145,8 @@ __global__ void __launch_bounds__(128) swept_flow_kernel(const FlowArgs<typename
   const int64_t N = a.N;
   const unsigned ntasks = (unsigned)a.rows * (unsigned)a.K;
   unsigned phase = 0;  // parity the mbarrier completes next
+  long long pc[5] = {0, 0, 0, 0, 0}, ptiles = 0, t0 = 0, t1 = 0;
+  (void)pc; (void)ptiles; (void)t0; (void)t1;
   if constexpr (TMA) {
     if (lane == 0) {
       mbar_init(mbar, 1);
@@ -149,10 +156,12 @@ __global__ void __launch_bounds__(128) swept_flow_kernel(const FlowArgs<typename
   }
 
   for (;;) {
+    if constexpr (PROF) t0 = clock64();
     unsigned t = 0;
     if (lane == 0) t = atomicAdd(a.ticket, 1u);
     t = __shfl_sync(0xffffffffu, t, 0);
     if (t >= ntasks) break;
+    if constexpr (PROF) { t1 = clock64(); pc[0] += t1 - t0; t0 = t1; }
     const int r = (int)(t / (unsigned)a.K), k = (int)(t % (unsigned)a.K);
     const int64_t S = (int64_t)k * n + ((r & 1) ? n / 2 : 0);  // < N; copies wrap
     if (r > 0) {
@@ -179,6 +188,7 @@ __global__ void __launch_bounds__(128) swept_flow_kernel(const FlowArgs<typename
       if (dead) break;
       fence_acq_rel_gpu();
     }
+    if constexpr (PROF) { t1 = clock64(); pc[1] += t1 - t0; t0 = t1; }
     // ---- stage the tile: both rows with their halo [S-h, S+n+h) (Up: row 0 of the initial level; the other row
     // is zero: tier -1 does not exist)
     const R* in0 = r == 0 ? a.init : ((r & 1) ? a.buf[0][0] : a.buf[1][0]);
@@ -221,10 +231,12 @@ __global__ void __launch_bounds__(128) swept_flow_kernel(const FlowArgs<typename
       }
     }
     __syncwarp();
+    if constexpr (PROF) { t1 = clock64(); pc[2] += t1 - t0; t0 = t1; }
     // ---- sweep (identical arithmetic and order to the CHAR flavour)
     if (r == 0) char_sweep_tile<Prob, B, L, KIND_UP, RS>(rows, RS, PAD + n / 2, lane, a.k);
     else if (r == a.rows - 1) char_sweep_tile<Prob, B, L, KIND_DOWN, RS>(rows, RS, PAD + n / 2, lane, a.k);
     else char_sweep_tile<Prob, B, L, KIND_WHOLE, RS>(rows, RS, PAD + n / 2, lane, a.k);
+    if constexpr (PROF) { __syncwarp(); t1 = clock64(); pc[3] += t1 - t0; t0 = t1; }
     // ---- publish: the rows over [S, S+n), then the flag
     R* out0 = (r & 1) ? a.buf[1][0] : a.buf[0][0];
     R* out1 = (r & 1) ? a.buf[1][1] : a.buf[0][1];
@@ -257,6 +269,14 @@ __global__ void __launch_bounds__(128) swept_flow_kernel(const FlowArgs<typename
       }
     }
     __syncwarp();  // the slice is restaged by the next task of this warp
+    if constexpr (PROF) { t1 = clock64(); pc[4] += t1 - t0; ++ptiles; }
+  }
+  if constexpr (PROF) {
+    if (lane == 0 && a.prof) {
+#pragma unroll
+      for (int i = 0; i < 5; ++i) atomicAdd(a.prof + i, (unsigned long long)pc[i]);
+      atomicAdd(a.prof + 5, (unsigned long long)ptiles);
+    }
   }
   // Leave the scratch as it was found.  A warp arrives here after its last task is in global memory; the warp that
   // arrives last therefore knows that every task of the launch is done.

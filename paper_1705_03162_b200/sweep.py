@@ -1,14 +1,21 @@
 """Throughput sweep of the swept and per-step variants over problem x N x tile width (BASELINE.json configs 2-5).
 
-    python -m paper_1705_03162_b200.sweep [--problems heat,ks,euler] [--logn 11,14,17,20] [--widths 32,...,1024]
+    python -m paper_1705_03162_b200.sweep [--problems heat,ks,euler,ks3] [--logn 11,14,17,20] [--widths 32,...,1024]
                                           [--dtype f64|f32] [--steps K] [--csv out.csv]
+    python -m paper_1705_03162_b200.sweep --probes [--csv out.csv]     (roofline denominators and the sweep model)
+    python -m paper_1705_03162_b200.sweep --flow-profile [--logn 20,24] [--csv out.csv]
+                                          (where the warps of the FLOW flavour spend their cycles; heat FP64)
 
 For every (problem, N) it times the per-step variant (best of 128 / 256 threads per block) and, for every tile
 width n, every admissible swept flavour (FLOW, CHAR with 32/16/8 lanes per tile, TIER), and prints one CSV row per
 (problem, N, n) with the best flavour: point-timestep updates per second, speed-up over per-step, and the fraction
 of the bound that applies: FP64/FP32 ALU pipe for swept, L2/HBM bytes for per-step.  Timing: CUDA
 events around `swept_run`, best of `--reps`, state resident on the device (the paper's figures include allocation
-and transfers, PAPER.md:236 — bench.py's `e2e` is the inclusive number).  Argument marshalling and timing only:
+and transfers, PAPER.md:236 — bench.py's `e2e` is the inclusive number).  The last column is the fraction of the
+dependent-chain latency bound, which is what governs small N: a sub-timestep cannot finish before the FP64
+operations on its critical path have (heat 2: DADD -> DFMA; KS 6 per stage), whatever the parallelism, so
+time >= sub-timesteps x depth x (FP64 dependent-issue latency, measured by `swept_probe_chain`).
+This is the measurement tool behind profiles/*_sweep_*.csv — argument marshalling and timing only, no library code:
 all arithmetic runs in the library's kernels.
 """
 from __future__ import annotations
@@ -26,9 +33,70 @@ if ROOT not in sys.path:
 import paper_1705_03162_b200 as sw  # noqa: E402
 
 FLAVOR_NAME = {sw.FLAVOR_TIER: "tier", sw.FLAVOR_CHAR: "char", sw.FLAVOR_FLOW: "flow"}
-# FP64-pipe instructions per point and timestep of the canonical expression trees
-FP64_INSTR = {sw.HEAT: 3, sw.KS: 22}
-BYTES_PER_STEP = {sw.HEAT: 16, sw.KS: 16, sw.EULER: 120}  # per-step algorithmic traffic, FP64
+# FP64-pipe instructions per point and timestep of the canonical expression trees.  Euler: counted
+# from the SASS of per_step_lane_kernel (profiles/r2_sass.md): 194 DADD/DMUL/DFMA/DSETP + 14 MUFU seeds per cell and
+# stage with every pressure and interface flux computed once, two stages.  KS3: 11 + 13 + 13 for the three stages.
+FP64_INSTR = {sw.HEAT: 3, sw.KS: 22, sw.EULER: 416, sw.KS3: 37}
+# per-step algorithmic traffic per point and timestep, FP64: heat one launch; KS both stages fused in
+# one launch; Euler and KS3 one launch per stage, the later stages also read u^n
+BYTES_PER_STEP = {sw.HEAT: 16, sw.KS: 16, sw.EULER: 120, sw.KS3: 64}
+# FP64 operations on the critical path of one sub-timestep (dependent chain), and sub-timesteps per timestep
+CHAIN_DEPTH = {sw.HEAT: 2, sw.KS: 6, sw.KS3: 7}
+SIGMA = {sw.HEAT: 1, sw.KS: 2, sw.EULER: 2, sw.KS3: 3}
+
+
+def probes(emit):
+    """Roofline denominators measured by the library's probes, and the issue-rate table of the characteristic sweep
+    (DESIGN.md §5.6, §7)."""
+    import torch
+    props = torch.cuda.get_device_properties(0)
+    emit(f"# device: {props.name}, {props.multi_processor_count} SMs, max SM clock {props.clock_rate / 1e3:.0f} MHz")
+    fp64 = sw.swept_probe_fp64()
+    emit(f"probe,fp64_pipe_lane_instr_per_s,{fp64:.4e},TFLOP/s (FMA=2) {2 * fp64 / 1e12:.2f},of nominal "
+         f"{fp64 / (props.multi_processor_count * 64 * props.clock_rate * 1e3):.3f}")
+    emit(f"probe,launch_us,{sw.swept_probe_launch(2000):.3f}")
+    pair = sw.swept_probe_chain()
+    emit(f"probe,dadd_dfma_pair_cycles,{pair:.2f},ns at max clock {pair / (props.clock_rate / 1e6):.2f}")
+    bps, bpc = sw.swept_probe_smem()
+    emit(f"probe,smem_read_bytes_per_s,{bps:.4e},bytes/clk/SM {bpc:.1f},of nominal 128 {bpc / 128:.3f}")
+    emit("sweep_probe,problem,lines_per_lane,warps_per_scheduler,cycles_per_superstep,fp64_pipe_busy")
+    for problem, name in ((sw.HEAT, "heat"), (sw.KS, "ks")):
+        for B in (8, 16, 32):
+            for wps in (1, 2, 3, 4, 6, 8):
+                try:
+                    cyc, busy = sw.swept_probe_sweep(problem, B, wps)
+                except sw.SweptError:
+                    continue
+                emit(f"sweep_probe,{name},{B},{wps},{cyc:.1f},{busy:.3f}")
+
+
+def flow_profile(emit, logns, widths):
+    """Per-part cycle shares of the persistent FLOW launch (instrumented kernel, `swept_flow_profile`), next to the
+    throughput of the plain kernel in the same configuration."""
+    import torch
+    import swept_inputs as si
+    emit("N,tile_width,group,plain_updates_per_s,instrumented_updates_per_s,tiles,cycles_per_tile,ticket,wait_parents,"
+         "stage,sweep,publish")
+    for logn in logns:
+        N = 1 << logn
+        w = si.config(2, N=N, nsteps=10000)
+        st = sw.Swept.from_workload(w)
+        u0_dev = torch.from_numpy(np.ascontiguousarray(w.u0)).cuda()
+        for n in widths:
+            for grp in (2, 3, 4, 6, 16 + 3, 16 + 4):  # resident CTAs per SM; +16 = TMA staging
+                try:
+                    plain = _time(torch, st, u0_dev, w.nsteps, n, sw.SWEPT, sw.FLAVOR_FLOW, grp, 2)
+                    sw.swept_flow_profile(st._h, True)
+                    inst = _time(torch, st, u0_dev, w.nsteps, n, sw.SWEPT, sw.FLAVOR_FLOW, grp, 1)
+                    c = sw.swept_flow_profile(st._h, False)
+                except sw.SweptError:
+                    sw.swept_flow_profile(st._h, False)
+                    continue
+                tot = sum(c[k] for k in ("ticket", "wait_parents", "stage", "sweep", "publish")) or 1
+                emit(f"{N},{n},{grp},{N * w.nsteps / (plain * 1e-3):.4e},{N * w.nsteps / (inst * 1e-3):.4e},{c['tiles']},"
+                     f"{tot / max(c['tiles'], 1):.0f}," + ",".join(f"{c[k] / tot:.4f}" for k in
+                                                                   ("ticket", "wait_parents", "stage", "sweep", "publish")))
+        st.close()
 
 
 def _time(torch, st, u0_dev, nsteps, n, variant, flavor, group, reps):
@@ -60,6 +128,8 @@ def main(argv=None):
     ap.add_argument("--bc", default="periodic", choices=["periodic", "paper"],
                     help="paper = insulated heat ends (B.5) / Dirichlet Euler tube (PAPER.md:377); TIER flavour only")
     ap.add_argument("--csv", default="")
+    ap.add_argument("--probes", action="store_true", help="print the probe measurements instead of a sweep")
+    ap.add_argument("--flow-profile", action="store_true", help="cycle shares of the FLOW kernel's task parts")
     args = ap.parse_args(argv)
     if not torch.cuda.is_available():
         raise SystemExit("needs a CUDA device: the swept library has no CPU fallback")
@@ -78,17 +148,31 @@ def main(argv=None):
             out.write(line + "\n")
             out.flush()
 
+    if args.probes or args.flow_profile:
+        if args.probes:
+            probes(emit)
+        else:
+            flow_profile(emit, [int(x) for x in args.logn.split(",")],
+                         [int(x) for x in args.widths.split(",") if int(x) in (256, 512, 1024)])
+        if out:
+            out.close()
+        return 0
+    # dependent-issue latency of one FP64 operation (half a DADD -> DFMA pair), seconds
+    fp64_latency_s = sw.swept_probe_chain() / 2 / (sm_mhz * 1e6)
     if args.bc == "paper":
         emit("# boundary conditions: the paper's own (insulated heat ends, Dirichlet Euler tube)")
-    emit("problem,dtype,N,nsteps,variant,tile_width,flavor,group,ms,updates_per_s,speedup_vs_per_step,bound,frac_of_bound")
+    emit("problem,dtype,N,nsteps,variant,tile_width,flavor,group,ms,updates_per_s,speedup_vs_per_step,bound,frac_of_bound,"
+         "frac_of_latency_bound")
     for pname in args.problems.split(","):
-        problem = {"heat": si.HEAT, "ks": si.KS, "euler": si.EULER}[pname]
+        problem = {"heat": si.HEAT, "ks": si.KS, "euler": si.EULER, "ks3": si.KS3}[pname]
         if problem != si.HEAT and args.dtype == "f32":
             continue
         for logn in [int(x) for x in args.logn.split(",")]:
             N = 1 << logn
-            cfg = {si.HEAT: 2, si.KS: 3, si.EULER: 4}[problem]
+            cfg = {si.HEAT: 2, si.KS: 3, si.EULER: 4, si.KS3: 3}[problem]
             w = si.config(cfg, N=N) if problem != si.EULER else si.config(4, N=N, rk2=si.RK2_HEUN)
+            if problem == si.KS3:
+                w = si.ks3_cos(N, si.BASE_SEED + 3, w.nsteps)
             if args.bc == "paper":
                 if problem == si.KS:
                     continue
@@ -101,14 +185,20 @@ def main(argv=None):
                                 for thr in (128, 256))
             ups = N * nsteps / (ps_ms * 1e-3)
             gbs = ups * BYTES_PER_STEP[problem] * (1 if args.dtype == "f64" else 0.5) / 1e9
+
+            def lat(ms):  # fraction of the dependent-chain latency bound (1 = nothing but the critical path)
+                if problem not in CHAIN_DEPTH:
+                    return ""
+                return f"{nsteps * SIGMA[problem] * CHAIN_DEPTH[problem] * fp64_latency_s / (ms * 1e-3):.4f}"
+
             emit(f"{pname},{args.dtype},{N},{nsteps},per_step,{ps_thr},,,{ps_ms:.4f},{ups:.4e},1.0,"
-                 f"bytes(L2/HBM) {gbs:.0f} GB/s,")
+                 f"bytes(L2/HBM) {gbs:.0f} GB/s,,{lat(ps_ms)}")
             for n in [int(x) for x in args.widths.split(",")]:
                 if N % n:
                     continue
                 best = None
-                cands = [(sw.FLAVOR_FLOW, 0), (sw.FLAVOR_CHAR, 32), (sw.FLAVOR_CHAR, 16), (sw.FLAVOR_CHAR, 8),
-                         (sw.FLAVOR_TIER, 0)]
+                cands = [(sw.FLAVOR_FLOW, 0), (sw.FLAVOR_FLOW, 16), (sw.FLAVOR_CHAR, 32), (sw.FLAVOR_CHAR, 16),
+                         (sw.FLAVOR_CHAR, 8), (sw.FLAVOR_TIER, 0)]   # FLOW group 16 = TMA staging
                 for fl, grp in cands:
                     try:
                         ms = _time(torch, st, u0_dev, nsteps, n, sw.SWEPT, fl, grp, args.reps)
@@ -122,7 +212,7 @@ def main(argv=None):
                 ups = N * nsteps / (ms * 1e-3)
                 frac = ups * FP64_INSTR[problem] / alu_peak if problem in FP64_INSTR else float("nan")
                 emit(f"{pname},{args.dtype},{N},{nsteps},swept,{n},{FLAVOR_NAME[fl]},{grp},{ms:.4f},{ups:.4e},"
-                     f"{ps_ms / ms:.3f},alu,{frac:.3f}")
+                     f"{ps_ms / ms:.3f},alu,{frac:.3f},{lat(ms)}")
             st.close()
     if out:
         out.close()
