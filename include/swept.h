@@ -65,9 +65,15 @@ enum {
                              per tier (the paper's "Shared" arrangement, re-sized)        */
   SWEPT_FLAVOR_CHAR = 2,  /* register-resident sweep along characteristics: a lane group per tile,
                              halo exchange by warp shuffles only, no block barrier       */
-  SWEPT_FLAVOR_FLOW = 3   /* the CHAR sweep inside ONE persistent launch per Up..Down cycle: tiles are
+  SWEPT_FLAVOR_FLOW = 3,  /* the CHAR sweep inside ONE persistent launch per Up..Down cycle: tiles are
                              tasks, rows are chained by per-tile flags instead of kernel boundaries
                              (DESIGN.md §5.5).  heat and KS, n = 256, 512, 1024   */
+  SWEPT_FLAVOR_CLUSTER = 4 /* small problems: the whole domain in ONE thread-block cluster, one launch per
+                             Up..Down cycle; a warp per tile, its points in registers, one shuffle exchange per
+                             tier; the edges pass from row to row through distributed shared memory behind a
+                             cluster barrier instead of global memory.
+                             Periodic heat (FP64, FP32) and KS; n = 64, 128, 256, 512; N / n <= 256 tiles (128 for
+                             n >= 256); group = warps per CTA (0 = as few as fit a cluster of 16 CTAs)     */
 };
 
 /* Optional device allocator hooks (so that PyTorch's caching allocator owns the memory).

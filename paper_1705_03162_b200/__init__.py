@@ -23,7 +23,7 @@ PROBLEM_SHAPE = {HEAT: (1, 1, 1), KS: (2, 2, 1), EULER: (2, 2, 3), KS3: (2, 3, 1
 PER_STEP, SWEPT = 0, 1
 F64, F32 = 0, 1
 RK2_MIDPOINT, RK2_HEUN = 0, 1
-FLAVOR_AUTO, FLAVOR_TIER, FLAVOR_CHAR, FLAVOR_FLOW = 0, 1, 2, 3
+FLAVOR_AUTO, FLAVOR_TIER, FLAVOR_CHAR, FLAVOR_FLOW, FLAVOR_CLUSTER = 0, 1, 2, 3, 4
 PS_LAUNCH, PS_RESIDENT = 0, 1  # per-step flavours
 BC_PERIODIC, BC_PAPER = 0, 1   # BC_PAPER: insulated heat ends, Eq. (B.5)
 KIND_NAMES = {0: "UpTriangle", 1: "SplitDiamond", 2: "WholeDiamond", 3: "DownTriangle", 4: "PerStepRemainder", 5: "FlowCycle"}

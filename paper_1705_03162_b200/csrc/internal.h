@@ -58,6 +58,17 @@ struct FlowLaunch {
   cudaStream_t stream;
 };
 
+// CLUSTER flavour: one whole Up / diamonds / Down cycle of tile width n in a single launch of one thread-block cluster
+struct ClusterLaunch {
+  const void* init;  // full time level at the start of the cycle
+  void* out;         // full time level at its end (another slab)
+  int64_t N;
+  int n, rows;       // tile width; rows = D + 2
+  int warps_per_cta; // 0 = as few as fit a cluster of 16 CTAs
+  const double* consts;
+  cudaStream_t stream;
+};
+
 // resident per-step: all sub-timesteps in one persistent cooperative launch (per_step_resident.cuh)
 struct ResidentLaunch {
   const void* in;
@@ -109,6 +120,8 @@ int launch_resident_ks(int dtype, int rk2, const ResidentLaunch& a);
 int launch_resident_euler(int dtype, int rk2, const ResidentLaunch& a);
 int launch_flow_heat(int dtype, const FlowLaunch& a);
 int launch_flow_ks(int dtype, int rk2, const FlowLaunch& a);
+int launch_cluster_heat(int dtype, const ClusterLaunch& a);
+int launch_cluster_ks(int dtype, int rk2, const ClusterLaunch& a);
 bool tile_config_ok_heat(int dtype, int flavor, int64_t N, int n, int P);
 bool tile_config_ok_ks(int dtype, int flavor, int64_t N, int n, int P);
 bool tile_config_ok_euler(int dtype, int flavor, int64_t N, int n, int P);

@@ -17,6 +17,7 @@ bool tile_config_ok_ks(int dtype, int flavor, int64_t N, int n, int P) {
   if (flavor == SWEPT_FLAVOR_TIER) return tier_ok<KS<double, 0>>(n, P, 4);
   if (flavor == SWEPT_FLAVOR_CHAR) return char_ok<KS<double, 0>, 32>(N, n, P);
   if (flavor == SWEPT_FLAVOR_FLOW) return flow_ok<KS<double, 0>, 32>(N, n);
+  if (flavor == SWEPT_FLAVOR_CLUSTER) return cluster_ok<KS<double, 0>>(N, n, P);
   return false;
 }
 int launch_tile_ks(int dtype, int rk2, const TileLaunch& a) {
@@ -28,6 +29,10 @@ int launch_tile_ks(int dtype, int rk2, const TileLaunch& a) {
 int launch_flow_ks(int dtype, int rk2, const FlowLaunch& a) {
   if (dtype != 0) return NO_KERNEL;
   return rk2 == 0 ? flow_T<KS<double, 0>, 32>(a) : flow_T<KS<double, 1>, 32>(a);
+}
+int launch_cluster_ks(int dtype, int rk2, const ClusterLaunch& a) {
+  if (dtype != 0) return NO_KERNEL;
+  return rk2 == 0 ? cluster_T<KS<double, 0>>(a) : cluster_T<KS<double, 1>>(a);
 }
 int launch_resident_ks(int dtype, int rk2, const ResidentLaunch& a) {
   if (dtype != 0) return NO_KERNEL;

@@ -4,6 +4,7 @@
 #include "kernels_impl.cuh"
 #include "per_step_resident.cuh"
 #include "swept_flow.cuh"
+#include "swept_cluster.cuh"
 
 namespace swept {
 
@@ -50,6 +51,80 @@ int resident_T(const ResidentLaunch& a) {
     if (rc == NO_KERNEL && PMAX >= 8) rc = resident_try<Prob, (PMAX >= 8 ? 8 : 2)>(a, TMAX, pass);
     if (rc == NO_KERNEL && PMAX >= 16) rc = resident_try<Prob, (PMAX >= 16 ? 16 : 2)>(a, TMAX, pass);
     if (rc != NO_KERNEL) return rc;
+  }
+  return NO_KERNEL;
+}
+
+// ---- CLUSTER flavour: the whole domain in one thread-block cluster, a warp per tile of n = 32 P points -------
+// warps per CTA for K tiles: the caller's choice, else as few as still fit a cluster of 16 CTAs (one warp per scheduler
+// is the shortest tier latency); 0 if K tiles cannot be laid out
+template <class Prob>
+inline int cluster_warps_per_cta(int64_t K, int n, int want) {
+  const int P = n / 32;
+  const int max_wpc = ClusterMaxThreads<16>::value / 32 * (P >= 8 ? 1 : 2);  // = ClusterMaxThreads<P> / 32
+  for (int wpc : {1, 2, 4, 8, 16, 32}) {
+    if (want ? wpc != want : (wpc < 4 && K > wpc)) continue;
+    if (wpc > max_wpc || K % wpc || K / wpc > 16) continue;
+    if (cluster_smem_bytes<Prob>(wpc * n) > (size_t)200 * 1024) continue;
+    return wpc;
+  }
+  return 0;
+}
+
+template <class Prob>
+inline bool cluster_ok(int64_t N, int n, int want_wpc) {
+  if (n != 64 && n != 128 && n != 256 && n != 512) return false;
+  if (N % n || n / 32 < Prob::H || (n / (2 * Prob::H)) % 2) return false;
+  return cluster_warps_per_cta<Prob>(N / n, n, want_wpc) != 0;
+}
+
+template <class Prob, int P>
+inline int cluster_go(const ClusterLaunch& a) {
+  using R = typename Prob::R;
+  const int64_t K = a.N / a.n;
+  const int wpc = cluster_warps_per_cta<Prob>(K, a.n, a.warps_per_cta);
+  if (!wpc) return NO_KERNEL;
+  const int cs = (int)(K / wpc);
+  ClusterArgs<R> c;
+  c.init = (const R*)a.init; c.out = (R*)a.out; c.N = a.N; c.n = a.n; c.rows = a.rows;
+  c.chunk = wpc * a.n;
+  c.chunk_log2 = 0;
+  while ((1 << c.chunk_log2) < c.chunk) ++c.chunk_log2;
+  c.k = round_consts<R>(a.consts);
+  const size_t smem = cluster_smem_bytes<Prob>(c.chunk);
+  auto kern = swept_cluster_kernel<Prob, P>;
+  cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  if (e == cudaSuccess && cs > 8) e = cudaFuncSetAttribute(kern, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
+  if (e != cudaSuccess) return (int)e;
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3((unsigned)cs);
+  cfg.blockDim = dim3((unsigned)(wpc * 32));
+  cfg.dynamicSmemBytes = smem;
+  cfg.stream = a.stream;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeClusterDimension;
+  attr[0].val.clusterDim.x = (unsigned)cs;
+  attr[0].val.clusterDim.y = 1;
+  attr[0].val.clusterDim.z = 1;
+  cfg.attrs = attr;
+  cfg.numAttrs = 1;
+  int nclusters = 0;
+  e = cudaOccupancyMaxActiveClusters(&nclusters, kern, &cfg);
+  if (e != cudaSuccess || nclusters < 1) {
+    cudaGetLastError();
+    return NO_KERNEL;  // this cluster shape cannot be scheduled on this device
+  }
+  return (int)cudaLaunchKernelEx(&cfg, kern, c);
+}
+
+template <class Prob>
+int cluster_T(const ClusterLaunch& a) {
+  if (!cluster_ok<Prob>(a.N, a.n, a.warps_per_cta)) return NO_KERNEL;
+  switch (a.n / 32) {
+    case 2: return cluster_go<Prob, 2>(a);
+    case 4: return cluster_go<Prob, 4>(a);
+    case 8: return cluster_go<Prob, 8>(a);
+    case 16: return cluster_go<Prob, 16>(a);
   }
   return NO_KERNEL;
 }

@@ -272,6 +272,7 @@ bool tile_ok(const swept_state* s, int flavor, int n, int P) {
   if (s->bc && flavor != SWEPT_FLAVOR_TIER && !(flavor == SWEPT_FLAVOR_CHAR && s->problem == SWEPT_HEAT)) return false;
   if (s->bc && flavor == SWEPT_FLAVOR_CHAR && !swept::tile_config_ok_heat(s->dtype, SWEPT_FLAVOR_TIER, s->N, n, 1))
     return false;
+  if (flavor == SWEPT_FLAVOR_CLUSTER && (s->bc || (s->problem != SWEPT_HEAT && s->problem != SWEPT_KS))) return false;
   if (flavor == SWEPT_FLAVOR_FLOW && (s->problem == SWEPT_EULER || s->problem == SWEPT_KS3 || P < 0 || (P & 15) > 12 || P > 31 || !s->flow_scratch)) return false;
   switch (s->problem) {
     case SWEPT_HEAT: return swept::tile_config_ok_heat(s->dtype, flavor, s->N, n, P);
@@ -463,6 +464,26 @@ void default_tile(const swept_state* s, int* n_io, int* flavor_io, int* P_io) {
       return;
     }
   }
+  // ... and on a small one (N <= 8192: at most 64 warp-sized tiles), where every flavour is bound by the latency of
+  // the dependent tiers, the CLUSTER flavour: one launch per cycle, rows chained through distributed shared memory
+  if (n == 0 && flavor == SWEPT_FLAVOR_AUTO && !s->bc && (s->problem == SWEPT_HEAT || s->problem == SWEPT_KS) && s->N <= 8192) {
+    for (int cand : {s->N <= 4096 ? 64 : 128, 128, 256})
+      if (tile_ok(s, SWEPT_FLAVOR_CLUSTER, cand, 0)) {
+        *n_io = cand;
+        *flavor_io = SWEPT_FLAVOR_CLUSTER;
+        *P_io = 0;
+        return;
+      }
+  }
+  if (flavor == SWEPT_FLAVOR_CLUSTER) {  // explicit flavour, library's width
+    if (n == 0)
+      for (int cand : {128, 64, 256, 512})
+        if (n == 0 && tile_ok(s, SWEPT_FLAVOR_CLUSTER, cand, P)) n = cand;
+    *n_io = n;
+    *flavor_io = flavor;
+    *P_io = P;
+    return;
+  }
   const bool want_char = flavor == SWEPT_FLAVOR_CHAR ||
                          (flavor == SWEPT_FLAVOR_AUTO && (s->problem == SWEPT_HEAT || s->problem == SWEPT_KS) && !s->bc);
   if (n == 0) {
@@ -505,6 +526,19 @@ bool level_config(const swept_state* s, int n_top, int flavor_top, int P_top, in
     *flavor = flavor_top;
     *P = P_top;
     return tile_ok(s, flavor_top, n, P_top);
+  }
+  if (flavor_top == SWEPT_FLAVOR_CLUSTER) {
+    if (tile_ok(s, SWEPT_FLAVOR_CLUSTER, n, 0)) {
+      *flavor = SWEPT_FLAVOR_CLUSTER;
+      *P = 0;
+      return true;
+    }
+    for (int L : {32, 16, 8})
+      if (tile_ok(s, SWEPT_FLAVOR_CHAR, n, L)) {
+        *flavor = SWEPT_FLAVOR_CHAR;
+        *P = L;
+        return true;
+      }
   }
   if (flavor_top == SWEPT_FLAVOR_FLOW) {
     if (tile_ok(s, SWEPT_FLAVOR_FLOW, n, P_top)) {
@@ -576,6 +610,34 @@ int run_next_phase(swept_state* s) {
   const size_t ip = pr.next;
   const swept_phase& ph = pr.plan[ip];
   const int ns = s->nslabs, R = s->rows();
+  if (ph.kind == KIND_UP && pr.cfg[ph.n].first == SWEPT_FLAVOR_CLUSTER) {
+    // the whole cycle Up .. Down of this width in one launch of one thread-block cluster (swept_cluster.cuh)
+    size_t jp = ip;
+    while (pr.plan[jp].kind != KIND_DOWN) ++jp;
+    swept::ClusterLaunch c{};
+    c.init = s->slab[s->cur];
+    const int o = (s->cur + 1) % ns;
+    c.out = s->slab[o];
+    c.N = s->N;
+    c.n = ph.n;
+    c.rows = (int)(jp - ip + 1);
+    c.warps_per_cta = pr.cfg[ph.n].second;
+    c.consts = s->consts;
+    c.stream = s->stream;
+    int rc;
+    {
+      TimedScope ts(s, KIND_FLOW, 1);
+      rc = s->problem == SWEPT_HEAT ? swept::launch_cluster_heat(s->dtype, c) : swept::launch_cluster_ks(s->dtype, s->rk2, c);
+    }
+    if (rc == NO_KERNEL) return fail(SWEPT_EUNSUPPORTED, "no CLUSTER kernel for N=%lld n=%d", (long long)s->N, ph.n);
+    if (rc != 0) return fail(SWEPT_ECUDA, "cluster launch: %s", cudaGetErrorString((cudaError_t)rc));
+    s->last_launches += 1;
+    s->cur = o;
+    pr.rin[0] = o;
+    pr.nrows_valid = 1;
+    pr.next = jp + 1;
+    return 0;
+  }
   if (ph.kind == KIND_UP && pr.cfg[ph.n].first == SWEPT_FLAVOR_FLOW) {
     // the whole cycle Up .. Down of this width in one persistent launch
     size_t jp = ip;
@@ -977,7 +1039,8 @@ int swept_run_flavor(swept_state* s, int64_t nsteps, int32_t tile_width, int var
     }
   } else if (variant == SWEPT_SWEPT) {
     int fl = flavor & 0xff, P = (flavor >> 8) & 0xff;  // bits 8..15: explicit P / lane-group size (0 = default)
-    if (fl != SWEPT_FLAVOR_AUTO && fl != SWEPT_FLAVOR_TIER && fl != SWEPT_FLAVOR_CHAR && fl != SWEPT_FLAVOR_FLOW)
+    if (fl != SWEPT_FLAVOR_AUTO && fl != SWEPT_FLAVOR_TIER && fl != SWEPT_FLAVOR_CHAR && fl != SWEPT_FLAVOR_FLOW &&
+        fl != SWEPT_FLAVOR_CLUSTER)
       return fail(SWEPT_EINVAL, "unknown flavor %d", fl);
     rc = run_swept(s, nsteps, tile_width, fl, P);
   } else {
@@ -1247,6 +1310,9 @@ int swept_autotune(swept_state* s, int variant, int32_t* best_tile_width) {
       for (int fl : {SWEPT_FLAVOR_TIER, SWEPT_FLAVOR_CHAR})
         for (int P : {1, 2, 4, 8, 16, 32})
           if (tile_ok(s, fl, n, P)) cands.push_back({n, fl, P});
+    for (int n : {64, 128, 256, 512})
+      for (int wpc : {0, 4, 8, 16, 32})  // warps per CTA of the CLUSTER flavour (0 = the fewest that fit)
+        if (tile_ok(s, SWEPT_FLAVOR_CLUSTER, n, wpc)) cands.push_back({n, SWEPT_FLAVOR_CLUSTER, wpc});
     for (int n : {256, 512, 1024})
       for (int ctas : {1, 2, 3, 4, 6})  // resident CTAs per SM (clamped to the occupancy limit at launch)
         for (int tma : {0, 16})         // generic 16-byte copies, or TMA bulk copies (group bit 4)

@@ -10,9 +10,12 @@
 //     phase (they do not change during it);
 //   * the whole cycle — UpTriangle, D Split/WholeDiamond rows, DownTriangle (§4.2) — runs in ONE launch: between
 //     two rows every warp writes its tile's rows to the cluster's DISTRIBUTED SHARED MEMORY (point x of the domain
-//     lives in CTA x / chunk at offset x % chunk), one cluster barrier, and every warp reads the rows of its next
-//     tile, half a tile further on (the edges a node passes on), from there — possibly from a
-//     neighbouring SM.  Global memory is touched twice: the Up row reads the time level, the Down row writes it.
+//     lives in CTA x / chunk), one cluster barrier, and every warp reads the rows of its next tile, half a tile
+//     further on (the edges a node passes on), from there — possibly from a neighbouring SM.  Inside
+//     an aligned block of n points the slots are lane-major (point lane * P + j sits at j * 32 + lane), so that the 32
+//     lanes of one load or store touch consecutive addresses: a remote shared-memory access is one request per lane
+//     unless the lanes are contiguous (measured: 1200 cycles per strided warp access).
+//     Global memory is touched twice: the Up row reads the time level, the Down row writes it.
 //   * rows ping-pong between two shared-memory buffers, so one barrier per row suffices (a tile reads an h-wide halo
 //     that its neighbour rewrites in the same row: SURVEY.md §8(d) note).
 // What it buys: a tier costs a shuffle round trip plus one dependent DADD -> DFMA (about 50 cycles for P = 4) instead of
@@ -44,13 +47,16 @@ __device__ __forceinline__ double shfl_idx_(double v, int src) { return __shfl_s
 __device__ __forceinline__ float shfl_idx_(float v, int src) { return __shfl_sync(0xffffffffu, v, src); }
 
 // One tier of a warp's tile: source row vs (tier t-1), destination row vd (tier t; holds tier t-2 before), halo values
-// of the source row beyond the tile's ends in hl / hr.  Points [lo, hi) of the tile are updated.
+// of the source row beyond the tile's ends in hl / hr.  Point j of the lane is updated when relative tier t lies in
+// its window [ta[j], ta[j] + span[j]] (the tier ranges of swept_tier.cuh turned round: per point instead of per tier,
+// so that the test is one subtraction and one compare on plain registers).
 template <class Prob, int P>
 __device__ __forceinline__ void cluster_tier(const typename Prob::R (&vs)[Prob::C][P], typename Prob::R (&vd)[Prob::C][P],
                                              const typename Prob::R (&v0)[Prob::C][P],
                                              const typename Prob::R (&hl)[Prob::C][Prob::H],
-                                             const typename Prob::R (&hr)[Prob::C][Prob::H], const int par, const int lo,
-                                             const int hi, const int lane, const Consts<typename Prob::R>& k) {
+                                             const typename Prob::R (&hr)[Prob::C][Prob::H], const int par, const int t,
+                                             const int (&ta)[P], const unsigned (&span)[P], const int lane,
+                                             const Consts<typename Prob::R>& k) {
   using R = typename Prob::R;
   constexpr int H = Prob::H, C = Prob::C;
   R win[C][P + 2 * H], bs[C][P], o[C][P];
@@ -71,17 +77,19 @@ __device__ __forceinline__ void cluster_tier(const typename Prob::R (&vs)[Prob::
     }
   }
   Prob::template stage<P>(win, bs, o, par, k);
-  const int j0 = lane * P;
 #pragma unroll
   for (int j = 0; j < P; ++j) {
-    const bool act = j0 + j >= lo && j0 + j < hi;
+    const bool act = (unsigned)(t - ta[j]) <= span[j];
 #pragma unroll
     for (int c = 0; c < C; ++c) vd[c][j] = act ? o[c][j] : vd[c][j];
   }
 }
 
+// threads per CTA (register budget: two rows of P points, the window and the tier windows per lane)
+template <int P> struct ClusterMaxThreads { static constexpr int value = P >= 8 ? 256 : 512; };
+
 template <class Prob, int P>
-__global__ void __launch_bounds__(1024) swept_cluster_kernel(const ClusterArgs<typename Prob::R> a) {
+__global__ void __launch_bounds__(ClusterMaxThreads<P>::value) swept_cluster_kernel(const ClusterArgs<typename Prob::R> a) {
   namespace cg = cooperative_groups;
   using R = typename Prob::R;
   constexpr int H = Prob::H, C = Prob::C;
@@ -99,7 +107,9 @@ __global__ void __launch_bounds__(1024) swept_cluster_kernel(const ClusterArgs<t
   const int chunk = a.chunk;
   // address of point g (0 <= g < N) of (buffer, row, component) in the cluster's distributed shared memory
   auto dsm = [&](int buf, int row, int c, int64_t g) -> R* {
-    R* local = sm + (size_t)((buf * 2 + row) * C + c) * chunk + (int)(g & (chunk - 1));
+    const int i = (int)(g & (n - 1));                              // position inside the aligned block of n points
+    const int off = (int)(g & (chunk - 1)) - i + (i % P) * 32 + i / P;  // lane-major inside the block
+    R* local = sm + (size_t)((buf * 2 + row) * C + c) * chunk + off;
     return cluster.map_shared_rank(local, (unsigned)(g >> a.chunk_log2));
   };
   auto wrap = [&](int64_t g) -> int64_t { return g < 0 ? g + N : (g >= N ? g - N : g); };
@@ -130,9 +140,9 @@ __global__ void __launch_bounds__(1024) swept_cluster_kernel(const ClusterArgs<t
         const R* p0 = dsm(inb, 0, c, g0);
         const R* p1 = dsm(inb, 1, c, g0);
 #pragma unroll
-        for (int j = 0; j < P; ++j) {
-          v0[c][j] = p0[j];
-          v1[c][j] = p1[j];
+        for (int j = 0; j < P; ++j) {  // g0 is a multiple of P: its slot is the lane's column, the points are 32 apart
+          v0[c][j] = p0[j * 32];
+          v1[c][j] = p1[j * 32];
         }
 #pragma unroll
         for (int e = 0; e < H; ++e) {  // the h-wide halo beyond either end of the tile, both rows (all lanes: broadcast)
@@ -144,20 +154,30 @@ __global__ void __launch_bounds__(1024) swept_cluster_kernel(const ClusterArgs<t
         }
       }
     }
-    // ---- tiers (phases start on even global tiers, so odd relative tiers are predictor / odd-row tiers)
+    // ---- tiers (phases start on even global tiers, so odd relative tiers are predictor / odd-row tiers).
+    // Tier window of every point x of the tile: Up (tier t covers [ht, n-ht)): 1 .. min(x, n-1-x)/h;
+    // diamond (tier t covers the centre +- ht, then +- h(2m-t)): ceil(d/h) .. 2m - ceil(d/h) with d the
+    // distance from the centre; Down: ceil(d/h) .. m.
     const int ntiers = kind == KIND_UP ? m - 1 : (kind == KIND_DOWN ? m : 2 * m - 1);
+    int ta[P];
+    unsigned span[P];
+#pragma unroll
+    for (int j = 0; j < P; ++j) {
+      const int x = lane * P + j;
+      const int d = x < n / 2 ? n / 2 - x : x - n / 2 + 1;
+      const int first = (d + H - 1) / H;
+      const int edge = (x < n - 1 - x ? x : n - 1 - x) / H;
+      const int t0 = kind == KIND_UP ? 1 : first;
+      const int tb = kind == KIND_UP ? edge : (kind == KIND_DOWN ? m : 2 * m - first);
+      const bool never = tb < t0;  // the end points of an UpTriangle's base row
+      span[j] = never ? 0u : (unsigned)(tb - t0);
+      ta[j] = never ? (1 << 30) : t0;
+    }
+    // (Two tiers behind one shuffle exchange — 2h redundant evaluations per lane instead of a second exchange — was
+    // built and measured: no faster for the 3-point scheme, 3 % for the 5-point one; not kept.)
     for (int t = 1; t <= ntiers; t += 2) {
-      int lo, hi;
-      if (kind == KIND_UP) tier_range<KIND_UP>(t, n, H, m, lo, hi);
-      else if (kind == KIND_DOWN) tier_range<KIND_DOWN>(t, n, H, m, lo, hi);
-      else tier_range<KIND_WHOLE>(t, n, H, m, lo, hi);
-      cluster_tier<Prob, P>(v0, v1, v0, hl0, hr0, 1, lo, hi, lane, a.k);  // odd tier: reads row 0, writes row 1
-      if (t + 1 <= ntiers) {
-        if (kind == KIND_UP) tier_range<KIND_UP>(t + 1, n, H, m, lo, hi);
-        else if (kind == KIND_DOWN) tier_range<KIND_DOWN>(t + 1, n, H, m, lo, hi);
-        else tier_range<KIND_WHOLE>(t + 1, n, H, m, lo, hi);
-        cluster_tier<Prob, P>(v1, v0, v0, hl1, hr1, 0, lo, hi, lane, a.k);  // even tier: reads row 1, writes row 0
-      }
+      cluster_tier<Prob, P>(v0, v1, v0, hl0, hr0, 1, t, ta, span, lane, a.k);  // odd tier: reads row 0, writes row 1
+      if (t + 1 <= ntiers) cluster_tier<Prob, P>(v1, v0, v0, hl1, hr1, 0, t + 1, ta, span, lane, a.k);  // even: row 1 -> row 0
     }
     // ---- hand the rows on: Down leaves the full time level (row 0) in global memory
     if (kind == KIND_DOWN) {
@@ -172,13 +192,14 @@ __global__ void __launch_bounds__(1024) swept_cluster_kernel(const ClusterArgs<t
         R* p1 = dsm(outb, 1, c, g0);
 #pragma unroll
         for (int j = 0; j < P; ++j) {
-          p0[j] = v0[c][j];
-          p1[j] = v1[c][j];
+          p0[j * 32] = v0[c][j];
+          p1[j * 32] = v1[c][j];
         }
       }
       cluster.sync();  // release / acquire at cluster scope: every tile of row r is in shared memory
     }
   }
+  cluster.sync();  // nobody leaves while a slower CTA may still be reading its shared memory
 }
 
 template <class Prob>

@@ -7,7 +7,7 @@
                                           (where the warps of the FLOW flavour spend their cycles; heat FP64)
 
 For every (problem, N) it times the per-step variant (best of 128 / 256 threads per block) and, for every tile
-width n, every admissible swept flavour (FLOW, CHAR with 32/16/8 lanes per tile, TIER), and prints one CSV row per
+width n, every admissible swept flavour (FLOW, CHAR with 32/16/8 lanes per tile, TIER, CLUSTER), and prints one CSV row per
 (problem, N, n) with the best flavour: point-timestep updates per second, speed-up over per-step, and the fraction
 of the bound that applies: FP64/FP32 ALU pipe for swept, L2/HBM bytes for per-step.  Timing: CUDA
 events around `swept_run`, best of `--reps`, state resident on the device (the paper's figures include allocation
@@ -32,7 +32,7 @@ if ROOT not in sys.path:
 
 import paper_1705_03162_b200 as sw  # noqa: E402
 
-FLAVOR_NAME = {sw.FLAVOR_TIER: "tier", sw.FLAVOR_CHAR: "char", sw.FLAVOR_FLOW: "flow"}
+FLAVOR_NAME = {sw.FLAVOR_TIER: "tier", sw.FLAVOR_CHAR: "char", sw.FLAVOR_FLOW: "flow", sw.FLAVOR_CLUSTER: "cluster"}
 # FP64-pipe instructions per point and timestep of the canonical expression trees.  Euler: counted
 # from the SASS of per_step_lane_kernel (profiles/r2_sass.md): 194 DADD/DMUL/DFMA/DSETP + 14 MUFU seeds per cell and
 # stage with every pressure and interface flux computed once, two stages.  KS3: 11 + 13 + 13 for the three stages.
@@ -198,7 +198,8 @@ def main(argv=None):
                     continue
                 best = None
                 cands = [(sw.FLAVOR_FLOW, 0), (sw.FLAVOR_FLOW, 16), (sw.FLAVOR_CHAR, 32), (sw.FLAVOR_CHAR, 16),
-                         (sw.FLAVOR_CHAR, 8), (sw.FLAVOR_TIER, 0)]   # FLOW group 16 = TMA staging
+                         (sw.FLAVOR_CHAR, 8), (sw.FLAVOR_TIER, 0),   # FLOW group 16 = TMA staging
+                         (sw.FLAVOR_CLUSTER, 0), (sw.FLAVOR_CLUSTER, 8), (sw.FLAVOR_CLUSTER, 16)]  # group = warps per CTA
                 for fl, grp in cands:
                     try:
                         ms = _time(torch, st, u0_dev, nsteps, n, sw.SWEPT, fl, grp, args.reps)

@@ -47,6 +47,8 @@ def cases():
     yield "heat CHAR n=512 L=32", heat, sw.SWEPT, 512, C, 32
     yield "heat FLOW n=256", heat_flow, sw.SWEPT, 256, F, 0
     yield "heat FLOW n=512 TMA", heat_flow, sw.SWEPT, 512, F, 16
+    yield "heat CLUSTER n=64", heat, sw.SWEPT, 64, sw.FLAVOR_CLUSTER, 0
+    yield "heat CLUSTER n=256 (one CTA)", heat, sw.SWEPT, 256, sw.FLAVOR_CLUSTER, 8
     yield "heat walls TIER n=256", wall, sw.SWEPT, 256, T, 1
     yield "heat walls hybrid CHAR n=256", wall, sw.SWEPT, 256, C, 32
     yield "heat walls per_step", wall, sw.PER_STEP, 0, 0, 0
@@ -58,6 +60,7 @@ def cases():
     yield "ks CHAR n=256 L=32", ks, sw.SWEPT, 256, C, 32
     yield "ks FLOW n=256", ks_flow, sw.SWEPT, 256, F, 0
     yield "ks FLOW n=512 TMA", ks_flow, sw.SWEPT, 512, F, 16
+    yield "ks CLUSTER n=128", ks, sw.SWEPT, 128, sw.FLAVOR_CLUSTER, 0
     yield "ks3 per_step", ks3, sw.PER_STEP, 0, 0, 0
     yield "ks3 TIER n=128 P=1", ks3, sw.SWEPT, 128, T, 1
     yield "ks3 TIER n=256 P=2", ks3, sw.SWEPT, 256, T, 2
