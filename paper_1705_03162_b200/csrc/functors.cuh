@@ -32,6 +32,20 @@ template <class R> __device__ __forceinline__ R inf_();
 template <> __device__ __forceinline__ double inf_<double>() { return __longlong_as_double(0x7ff0000000000000LL); }
 template <> __device__ __forceinline__ float inf_<float>() { return __int_as_float(0x7f800000); }
 
+// a / b, bit for bit the IEEE round-to-nearest quotient, arranged so that the common special operand does not leave
+// the fast path of the division.  nvcc expands an FP64 division into a reciprocal refinement (about 10 FP64
+// instructions) followed by a range check that sends a ZERO or tiny numerator, a zero / infinite / NaN operand or a
+// subnormal quotient to a subroutine of several dozen instructions.  A gas at rest has zero momentum in every cell, so
+// in the undisturbed part of the Sod tube (most of the domain for most of a run) every velocity M / rho went through
+// that subroutine.  The quotient of a zero by a finite non-zero number is a signed zero with the sign of the product:
+// a * b yields exactly that.  Every other case still runs the division itself.
+template <class R>
+__device__ __forceinline__ R div_(R a, R b) {
+  const bool zero = a == (R)0 && fabs_(b) > (R)0 && fabs_(b) < inf_<R>();
+  const R q = (zero ? (R)1 : a) / b;
+  return zero ? a * b : q;
+}
+
 // Scheme constants, computed once on the host in double and rounded once to REAL (host side: api).
 template <class R>
 struct Consts {
@@ -149,18 +163,30 @@ struct Euler {
   static constexpr int TIER_MAX_THREADS = 1024;  // the TIER kernel shares pressures and fluxes: 64 registers
 
   __device__ __forceinline__ static R pressure(R rho, R M, R E, const Consts<R>& k) {  // (D.4), X4
-    const R u = M / rho;
+    const R u = div_(M, rho);
     return k.a0 * fma_(-((R)0.5 * M), u, E);
   }
-  __device__ __forceinline__ static R half_minmod(R r) {  // min(r,1)/2 if 0 < r < inf else 0 (D.7)/(D.8)
-    return (r > (R)0 && r < inf_<R>()) ? (R)0.5 * fmin_(r, (R)1) : (R)0;
+  // min(r,1)/2 if 0 < r < inf else 0 (D.7)/(D.8), written with comparisons only: 0.5 * fmin(r, 1) is 0.5 r below 1 and
+  // 0.5 from 1 on; NaN fails every comparison and gives 0
+  __device__ __forceinline__ static R half_minmod(R r) {
+    const R half_r = (R)0.5 * r;
+    const R v = r < (R)1 ? half_r : (R)0.5;
+    return (r > (R)0 && r < inf_<R>()) ? v : (R)0;
+  }
+  // half_minmod(num / den).  Where the pressure is flat num or den is exactly zero and the quotient is 0, NaN or
+  // +-inf, each of which the limiter maps to 0: decided here, and the division runs on harmless operands instead of
+  // falling into its special-case subroutine (see div_).  NaN operands still reach the division.
+  __device__ __forceinline__ static R limiter(R num, R den) {
+    const bool flat = num == (R)0 || den == (R)0;
+    const R r = (flat ? (R)1 : num) / (flat ? (R)1 : den);
+    return flat ? (R)0 : half_minmod(r);
   }
   // flux at the interface between cells k (state vl) and k+1 (state vr);
   // dm = P_k - P_{k-1}, d0 = P_{k+1} - P_k, dp = P_{k+2} - P_{k+1}
   __device__ __forceinline__ static void flux(const R (&vl)[3], const R (&vr)[3], R dm, R d0, R dp,
                                               R (&F)[3], const Consts<R>& k) {
-    const R phiL = half_minmod(d0 / dm);  // P_r at cell k (D.6)
-    const R phiR = half_minmod(d0 / dp);  // 1/P_r at cell k+1 as the swapped quotient (X5)
+    const R phiL = limiter(d0, dm);  // P_r at cell k (D.6)
+    const R phiR = limiter(d0, dp);  // 1/P_r at cell k+1 as the swapped quotient (X5)
     R QL[3], QR[3];
 #pragma unroll
     for (int c = 0; c < 3; ++c) {
@@ -168,17 +194,17 @@ struct Euler {
       QL[c] = fma_(phiL, dq, vl[c]);   // (D.7)
       QR[c] = fma_(-phiR, dq, vr[c]);  // (D.8)
     }
-    const R uL = QL[1] / QL[0];
+    const R uL = div_(QL[1], QL[0]);
     const R PL = k.a0 * fma_(-((R)0.5 * QL[1]), uL, QL[2]);
     const R eL = QL[2] / QL[0];
-    const R uR = QR[1] / QR[0];
+    const R uR = div_(QR[1], QR[0]);
     const R PR = k.a0 * fma_(-((R)0.5 * QR[1]), uR, QR[2]);
     const R eR = QR[2] / QR[0];
     const R FL0 = QL[1], FL1 = fma_(QL[1], uL, PL), FL2 = uL * (QL[2] + PL);  // (D.3)
     const R FR0 = QR[1], FR1 = fma_(QR[1], uR, PR), FR2 = uR * (QR[2] + PR);
     const R sL = sqrt_(QL[0]), sR = sqrt_(QR[0]);
     const R den = sL + sR;
-    const R usp = (sL * uL + sR * uR) / den;  // (D.10), X3; products then one add: L<->R symmetric
+    const R usp = div_(sL * uL + sR * uR, den);  // (D.10), X3; products then one add: L<->R symmetric
     const R esp = (sL * eL + sR * eR) / den;
     const R c2 = k.a1 * fma_(-((R)0.5 * usp), usp, esp);
     const R rsp = sqrt_(c2) + fabs_(usp);     // (D.11)
