@@ -11,11 +11,12 @@ One bench "step" = one pass of the whole hot path over that batch = one `swept_r
 `value`   : N * nsteps * K / (device time of K steps), state resident in HBM, L2 flushed between steps.
 `e2e`     : the same metric through the C ABI with HOST buffers: swept_write (H2D from pinned memory) +
             swept_run + swept_read (D2H) inside the timed region, every step.
-`roofline`: the dominant kernels are the Split/WholeDiamond launches (D of the D+2 swept launches); they are
-            bound by the FP64 ALU pipe ("alu").  achieved = 3 FP64-pipe instructions per update (DADD, DMUL,
-            DFMA; SURVEY.md §8(d)) counted as FMA-equivalent flops (x2) / measured duration;
-            peak = 148 SMs x 64 FP64 lanes/clk x 2 x SM clock, and the live DFMA-chain probe
-            is reported beside it.
+`roofline`: the dominant kernel is the persistent FLOW launch (or the Split/WholeDiamond launches of the CHAR
+            flavour); it is bound by the FP64 ALU pipe ("alu").  achieved = FP64-pipe lane-instructions per
+            second = 3 per update (DADD, DMUL, DFMA; SURVEY.md §8(d)) x updates per launch / measured duration;
+            peak = 148 SMs x 64 FP64 lanes/clk x SM clock: `frac` is the useful share of the pipe's
+            issue slots.  The live DFMA-chain probe is reported beside the nominal peak, and the true flop rate
+            (4 flops per update: one add, one multiply, one fused multiply-add) separately.
 `cpu_baseline`: the oracle (oracle/, plain per-step C++) timed on this host's cores on a bounded sample.
 
 N > 1 (torchrun): the path does not shard (single GPU) — "replicas only": every rank runs the
@@ -320,7 +321,7 @@ def main():
     clocks = clk.summary()
     sm_max = float(peaks.get("sm_max_mhz") or clocks["sm_max_mhz"] or 1965.0)
     sms = torch.cuda.get_device_properties(local).multi_processor_count
-    peak_tflops = sms * FP64_LANES_PER_CLK_PER_SM * 2 * sm_max * 1e6 / 1e12
+    peak_tinstr = sms * FP64_LANES_PER_CLK_PER_SM * sm_max * 1e6 / 1e12  # FP64-pipe lane-instructions per second / 1e12
     probe = sw.swept_probe_fp64()
     plan = sw.swept_plan(nsteps * state.sigma, tile, state.h)
     m_top = tile // (2 * state.h)
@@ -341,28 +342,35 @@ def main():
             if p[4] in (256, 512, 1024) and p[0] in (1, 2, 3):   # each diamond row and the Down row close m tiers
                 t_flow += p[4] // (2 * state.h)
         avg_launch_ms = flow_ms / flow_cnt
-        ach_tflops = fp64_instr_per_update * 2 * w.N * t_flow * args.steps / (flow_ms * 1e-3) / 1e12
+        upd_per_s = w.N * t_flow * args.steps / (flow_ms * 1e-3)
         kernel_name = "swept_flow_kernel: persistent launch running whole Up..Down cycles (heat FP64)"
         how = "CUDA events around every FLOW launch of the timed region (swept_phase_times)"
     elif d_cnt and n_diamonds_all == n_diamonds_top:
         avg_launch_ms = d_ms / d_cnt
-        ach_tflops = fp64_instr_per_update * 2 * w.N * m_top / (avg_launch_ms * 1e-3) / 1e12
+        upd_per_s = w.N * m_top / (avg_launch_ms * 1e-3)
         how = "CUDA events around every Split/WholeDiamond launch of the timed region (swept_phase_times)"
     else:  # flavours without per-launch phases, or diamonds of several widths: whole-step figure
         avg_launch_ms = total_ms / args.steps
-        ach_tflops = fp64_instr_per_update * 2 * updates_per_step / (avg_launch_ms * 1e-3) / 1e12
+        upd_per_s = updates_per_step / (avg_launch_ms * 1e-3)
         how = "whole swept_run (all phases) timed with CUDA events"
-    step_tflops = fp64_instr_per_update * 2 * updates_per_step / (total_ms / args.steps * 1e-3) / 1e12
-    roofline = {"bound": "alu", "achieved": ach_tflops, "peak": peak_tflops, "unit": "TFLOP/s",
-                "frac": ach_tflops / peak_tflops, "traffic": None,
+    ach_tinstr = fp64_instr_per_update * upd_per_s / 1e12
+    step_tinstr = fp64_instr_per_update * updates_per_step / (total_ms / args.steps * 1e-3) / 1e12
+    units = (f"N x {t_flow} timesteps per FLOW launch (the cycles of widths 256-1024 of swept_plan)" if flow_cnt
+             else f"N x m = N x {m_top} updates per diamond launch")
+    roofline = {"bound": "alu", "achieved": ach_tinstr, "peak": peak_tinstr,
+                "unit": "Tinstr/s (FP64-pipe lane-instructions; x2 = FMA-equivalent TFLOP/s)",
+                "frac": ach_tinstr / peak_tinstr, "traffic": None,
                 "kernel": kernel_name, "timed_by": how,
-                "note": "FMA-equivalent FP64 flops = 2 x 3 FP64-pipe instructions per update, N*m updates per "
-                        f"launch (m = {m_top}); peak = {sms} SM x 64 lanes x 2 x {sm_max:.0f} MHz (nominal unit "
-                        "count, max clock); probe = live DFMA-chain measurement",
-                "peak_probe_tflops": probe * 2 / 1e12,
-                "frac_of_probe": ach_tflops / (probe * 2 / 1e12) if probe else None,
+                "note": "FP64 pipe issue utilisation: 3 FP64-pipe instructions per update (DADD, DMUL, DFMA), "
+                        f"{units}; peak = {sms} SM x 64 lanes x {sm_max:.0f} MHz (nominal unit count, max clock); "
+                        "probe = live DFMA-chain measurement of the same quantity",
+                "peak_probe": probe / 1e12,
+                "frac_of_probe": ach_tinstr / (probe / 1e12) if probe else None,
+                "true_tflops": 4 * upd_per_s / 1e12,
+                "true_tflops_note": "4 floating-point operations per update (add, multiply, fused multiply-add); the "
+                                    f"FMA peak 2 x {peak_tinstr:.1f} TFLOP/s is not reachable by this instruction mix",
                 "avg_launch_ms": avg_launch_ms, "diamond_launches_timed": d_cnt,
-                "whole_step_tflops": step_tflops, "whole_step_frac": step_tflops / peak_tflops,
+                "whole_step": step_tinstr, "whole_step_frac": step_tinstr / peak_tinstr,
                 "phase_ms_per_step": {k: v[0] / args.steps for k, v in phase.items()},
                 "phase_launches_per_step": {k: v[1] / args.steps for k, v in phase.items()}}
     try:  # DRAM bytes per launch of the dominant kernel, from the committed ncu --set full capture

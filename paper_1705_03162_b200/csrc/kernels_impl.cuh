@@ -45,8 +45,13 @@ inline int per_step_fused_go(const PerStepLaunch& a) {
   const int64_t nthreads = a.N / P;
   const int threads = a.threads < Prob::MAX_THREADS ? a.threads : Prob::MAX_THREADS;
   const unsigned grid = (unsigned)((nthreads + threads - 1) / threads);
-  per_step_fused_kernel<Prob, P><<<grid, threads, 0, a.stream>>>((const R*)a.in, (R*)a.out, a.N,
-                                                                   round_consts<R>(a.consts));
+  // halo by warp shuffles where the launch is throughput-bound (measured cross-over between N = 2^17 and 2^20)
+  if (a.N >= ((int64_t)1 << 19))
+    per_step_fused_kernel<Prob, P, true><<<grid, threads, 0, a.stream>>>((const R*)a.in, (R*)a.out, a.N,
+                                                                           round_consts<R>(a.consts));
+  else
+    per_step_fused_kernel<Prob, P, false><<<grid, threads, 0, a.stream>>>((const R*)a.in, (R*)a.out, a.N,
+                                                                            round_consts<R>(a.consts));
   return (int)cudaGetLastError();
 }
 

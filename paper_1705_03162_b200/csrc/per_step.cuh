@@ -90,7 +90,10 @@ per_step_kernel(const typename Prob::R* __restrict__ in, const typename Prob::R*
 // predictor stage on its P points and their h neighbours on either side (recomputed, not communicated), then
 // the final stage on its P points.  Same Prob::stage trees as the two-launch form, so the same bits; half the
 // launches and no predictor array in global memory (16 B instead of 40 B per point and timestep).
-template <class Prob, int P>
+// SHFL = true takes the halo from the neighbouring lanes (large N: the kernel is then bound by memory, not by the L1
+// tag stage); SHFL = false loads it (small N: one load latency instead of load + shuffle on the critical path of a
+// launch that is over in two microseconds).
+template <class Prob, int P, bool SHFL>
 __global__ void __launch_bounds__(Prob::MAX_THREADS)
 per_step_fused_kernel(const typename Prob::R* __restrict__ in, typename Prob::R* __restrict__ out, int64_t N,
                       Consts<typename Prob::R> k) {
@@ -98,22 +101,49 @@ per_step_fused_kernel(const typename Prob::R* __restrict__ in, typename Prob::R*
   constexpr int H = Prob::H;
   static_assert(Prob::C == 1 && Prob::SIGMA == 2, "fused two-stage kernel: scalar RK2 schemes");
   const int64_t i0 = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) * P;
-  if (i0 >= N) return;
   constexpr int Q = P + 2 * H;  // points whose predictor value this thread needs
   alignas(16) R win[1][Q + 2 * H];
   alignas(16) R body[P];
-  load_vec<R, P>(in + i0, body);
+  if constexpr (SHFL && P >= 2 * H && P % (2 * H) == 0) {
+    // The 2h values either side are the neighbouring lanes' bodies: warp shuffles, not loads.  (With eight scalar
+    // halo loads per thread this kernel was bound by the L1 tag stage — l1tex throughput 98 %, DRAM 44 % at N = 2^24,
+    // profiles/r2_ks_per_step.md — although every one of them hit L1.)  Only the two end lanes of a warp, and a lane
+    // whose neighbour lies beyond N, load their halo, as one vector; the whole warp stays for the shuffles.
+    const bool valid = i0 < N;
+    const int lane = threadIdx.x & 31;
+#pragma unroll
+    for (int j = 0; j < P; ++j) body[j] = (R)0;
+    const bool edge_l = valid && lane == 0, edge_r = valid && (lane == 31 || i0 + P >= N);
+    alignas(16) R left[2 * H], right[2 * H];
+#pragma unroll
+    for (int j = 0; j < 2 * H; ++j) left[j] = right[j] = (R)0;
+    // all loads first, so that the end lanes' halo loads travel with the body loads instead of after the shuffles
+    if (valid) load_vec<R, P>(in + i0, body);
+    if (edge_l) load_vec<R, 2 * H>(in + (i0 >= 2 * H ? i0 - 2 * H : N - 2 * H), left);
+    if (edge_r) load_vec<R, 2 * H>(in + (i0 + P < N ? i0 + P : 0), right);
+#pragma unroll
+    for (int j = 0; j < 2 * H; ++j) {
+      const R fromL = __shfl_up_sync(0xffffffffu, body[P - 2 * H + j], 1);
+      const R fromR = __shfl_down_sync(0xffffffffu, body[j], 1);
+      win[0][j] = edge_l ? left[j] : fromL;
+      win[0][2 * H + P + j] = edge_r ? right[j] : fromR;
+    }
+    if (!valid) return;
+  } else {
+    if (i0 >= N) return;
+    load_vec<R, P>(in + i0, body);
+#pragma unroll
+    for (int j = 0; j < 2 * H; ++j) {
+      int64_t il = i0 - 2 * H + j;
+      if (il < 0) il += N;
+      int64_t ir = i0 + P + j;
+      if (ir >= N) ir -= N;
+      win[0][j] = __ldg(in + il);
+      win[0][2 * H + P + j] = __ldg(in + ir);
+    }
+  }
 #pragma unroll
   for (int j = 0; j < P; ++j) win[0][2 * H + j] = body[j];
-#pragma unroll
-  for (int j = 0; j < 2 * H; ++j) {
-    int64_t il = i0 - 2 * H + j;
-    if (il < 0) il += N;
-    int64_t ir = i0 + P + j;
-    if (ir >= N) ir -= N;
-    win[0][j] = __ldg(in + il);
-    win[0][2 * H + P + j] = __ldg(in + ir);
-  }
   R ctr[1][Q], pred[1][Q];
 #pragma unroll
   for (int j = 0; j < Q; ++j) ctr[0][j] = win[0][H + j];

@@ -43,7 +43,7 @@ KERNELS = [
     ("TIER Euler f64 Heun P=2 WholeDiamond", "swept_tier_kernelINS_5EulerIdLi1EEELi2ELi2E"),
     ("TIER KS3 f64 P=1 WholeDiamond", "swept_tier_kernelINS_3KS3IdEELi1ELi2E"),
     ("per-step heat f64 P=4", "per_step_kernelINS_4HeatIdEELi4E"),
-    ("per-step KS f64 fused P=4", "per_step_fused_kernelINS_2KSIdLi0EEELi4E"),
+    ("per-step KS f64 fused P=4 (shuffle halo)", "per_step_fused_kernelINS_2KSIdLi0EEELi4ELb1E"),
     ("per-step Euler f64 Heun (one interface per lane)", "per_step_lane_kernelINS_5EulerIdLi1EEE"),
     ("per-step resident heat f64 P=16", "per_step_resident_kernelINS_4HeatIdEELi16E"),
 ]

@@ -106,3 +106,14 @@ def test_fp32_instantiation_tracks_fp64():
     u64 = oracle.run_workload(w)
     u32 = oracle.run_workload(w, dtype=np.float32)
     assert 0 < np.max(np.abs(u32 - u64)) < 1e-3
+
+
+def test_periodic_initial_data_variant():
+    # ADVICE r1 / reading X12: the literal config's smooth part jumps by O(1) at the wrap; the periodic variant does not
+    lit = si.ks_cos(4096, 1, 10, noise=0.0)
+    per = si.ks_cos(4096, 1, 10, noise=0.0, periodic=True)
+    assert abs(lit.u0[0] - lit.u0[-1]) > 1.0
+    assert abs(per.u0[0] - per.u0[-1]) < 0.05
+    for w in (lit, per):   # both stay bounded under the scheme (the jump is damped, |G| = 0.52 at Nyquist)
+        out = oracle.run_workload(w, nsteps=400)
+        assert np.all(np.isfinite(out)) and np.max(np.abs(out)) < 5.0
