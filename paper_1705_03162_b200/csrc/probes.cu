@@ -59,9 +59,9 @@ __global__ void __launch_bounds__(1024) smem_read_int_kernel(unsigned* sink, int
 #pragma unroll
     for (int u = 0; u < 8; ++u) {
       uint4 v;  // volatile: one LDS.128 per lane and iteration, never hoisted or merged
-      asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];"
+      asm volatile("ld.volatile.shared.v4.u32 {%0, %1, %2, %3}, [%4];"
                    : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w)
-                   : "r"(base + 16u * (uint32_t)((idx + u * 1024) & (nvec - 1))));
+                   : "r"(base + 16u * (uint32_t)((idx + u * 256) & (nvec - 1))));
       acc.x ^= v.x; acc.y ^= v.y; acc.z ^= v.z; acc.w ^= v.w;
     }
     idx = (idx + 32) & (nvec - 1);
