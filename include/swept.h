@@ -148,9 +148,10 @@ enum {
 
 /* swept_run_flavor — swept_run with an explicit kernel flavour in bits 0..7 of `flavor` (SWEPT_FLAVOR_* for
  * variant SWEPT_SWEPT, SWEPT_PS_* for SWEPT_PER_STEP) and the flavour's group parameter in bits 8..15
- * (TIER: points per thread; CHAR: lanes per tile; FLOW: resident CTAs per SM in its bits 0..3, 0 = default, and
- * in its bit 4 (value 16) how a tile's rows travel between global and shared memory: 1 = TMA bulk copies
- * (cp.async.bulk + mbarrier) issued by one lane, 0 = 16-byte loads / stores of all lanes; group 0 = defaults). */
+ * (TIER: points per thread; CHAR: lanes per tile; CLUSTER: warps per CTA; FLOW: resident CTAs per SM in its bits 0..3,
+ * 0 = default, and in its bit 4 (value 16) how a tile's rows travel between global and shared memory: 1 = TMA bulk
+ * copies (cp.async.bulk + mbarrier) issued by one lane, 0 = 16-byte loads / stores of all lanes; group 0 = the
+ * library's defaults: TMA copies, resident CTAs from the tiles per row). */
 int swept_run_flavor(swept_state* s, int64_t nsteps, int32_t tile_width, int variant, int flavor);
 
 /* swept_read — synchronise the stream and copy the current field to HOST memory (same layout as

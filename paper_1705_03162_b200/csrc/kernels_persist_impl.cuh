@@ -182,7 +182,9 @@ inline int flow_go(const FlowLaunch& a) {
 template <class Prob, int BMAX>
 int flow_T(const FlowLaunch& a) {
   if (!flow_ok<Prob, BMAX>(a.N, a.n)) return NO_KERNEL;
-  const bool tma = (a.ctas_per_sm & 16) != 0;  // group bit 4: stage the tiles with TMA bulk copies
+  // group bit 4: stage the tiles with TMA bulk copies; group 0 (library defaults) does too — measured faster at every
+  // size once the kernel around them compiled as tightly as the 16-byte-copy one (profiles/r2_flow_phases.md)
+  const bool tma = (a.ctas_per_sm & 16) != 0 || a.ctas_per_sm == 0;
   if (a.prof) {  // instrumented kernels (swept_flow_profile): the 3-point FP64 problem, the headline's kernel family
     if constexpr (Prob::H == 1 && sizeof(typename Prob::R) == 8) {
       switch (a.n / 32) {

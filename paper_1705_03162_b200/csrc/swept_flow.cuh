@@ -91,30 +91,56 @@ __device__ __forceinline__ void warp_store_row(R* __restrict__ dst, const R* src
   }
 }
 
+// Predicated forms of the bulk-copy primitives (common.cuh): the FLOW kernel issues them from lane 0 WITHOUT a C++
+// branch.  With `if (lane == 0) { ... }` around them the compiler could no longer prove the warp converged at the sweep's
+// shuffles and guarded each with a divergence test (BRA.DIV + out-of-line WARPSYNC.COLLECTIVE): 134 instead of 118
+// instructions per pair of steps and 78 registers.
+__device__ __forceinline__ void bulk_g2s_if(bool p, void* dst_smem, const void* src_gmem, uint32_t bytes, uint64_t* bar) {
+  asm volatile(
+      "{\n\t.reg .pred q;\n\tsetp.ne.u32 q, %4, 0;\n\t"
+      "@q cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];\n\t}" ::"r"(
+          smem_u32(dst_smem)),
+      "l"(src_gmem), "r"(bytes), "r"(smem_u32(bar)), "r"((uint32_t)p)
+      : "memory");
+}
+__device__ __forceinline__ void bulk_s2g_if(bool p, void* dst_gmem, const void* src_smem, uint32_t bytes) {
+  asm volatile(
+      "{\n\t.reg .pred q;\n\tsetp.ne.u32 q, %3, 0;\n\t"
+      "@q cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;\n\t}" ::"l"(dst_gmem),
+      "r"(smem_u32(src_smem)), "r"(bytes), "r"((uint32_t)p)
+      : "memory");
+}
+__device__ __forceinline__ void mbar_arrive_expect_tx_if(bool p, uint64_t* bar, uint32_t bytes) {
+  asm volatile(
+      "{\n\t.reg .pred q;\n\tsetp.ne.u32 q, %2, 0;\n\t"
+      "@q mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;\n\t}" ::"r"(smem_u32(bar)),
+      "r"(bytes), "r"((uint32_t)p)
+      : "memory");
+}
+__device__ __forceinline__ void st_release_gpu_if(bool p, int* ptr, int v) {
+  asm volatile(
+      "{\n\t.reg .pred q;\n\tsetp.ne.u32 q, %2, 0;\n\t"
+      "@q st.release.gpu.global.s32 [%0], %1;\n\t}" ::"l"(ptr),
+      "r"(v), "r"((uint32_t)p)
+      : "memory");
+}
+
 // TMA 1-D bulk copies of `len` elements starting at global element g0 of a periodic row of N elements (g0 may be
 // negative by less than N); g0, len and N are multiples of the 16-byte granule, so every piece is aligned.
 template <class R>
-__device__ __forceinline__ void bulk_load_wrapped(R* dst, const R* __restrict__ src, int64_t g0, int len, int64_t N,
+__device__ __forceinline__ void bulk_load_wrapped(bool p, R* dst, const R* __restrict__ src, int64_t g0, int len, int64_t N,
                                                   uint64_t* bar) {
-  int64_t g = g0 < 0 ? g0 + N : g0;
-  while (len > 0) {
-    const int piece = (int)((N - g) < (int64_t)len ? (N - g) : (int64_t)len);
-    bulk_g2s(dst, src + g, (uint32_t)(piece * sizeof(R)), bar);
-    dst += piece;
-    len -= piece;
-    g = 0;
-  }
+  // at most two pieces (len <= N): up to the end of the row, and the rest from its start
+  const int64_t g = g0 < 0 ? g0 + N : g0;
+  const int first = (int)((N - g) < (int64_t)len ? (N - g) : (int64_t)len);
+  bulk_g2s_if(p, dst, src + g, (uint32_t)(first * sizeof(R)), bar);
+  bulk_g2s_if(p && len > first, dst + first, src, (uint32_t)((len - first) * sizeof(R)), bar);
 }
 template <class R>
-__device__ __forceinline__ void bulk_store_wrapped(R* __restrict__ dst, const R* src, int64_t g0, int len, int64_t N) {
-  int64_t g = g0;
-  while (len > 0) {
-    const int piece = (int)((N - g) < (int64_t)len ? (N - g) : (int64_t)len);
-    bulk_s2g(dst + g, src, (uint32_t)(piece * sizeof(R)));
-    src += piece;
-    len -= piece;
-    g = 0;
-  }
+__device__ __forceinline__ void bulk_store_wrapped(bool p, R* __restrict__ dst, const R* src, int64_t g0, int len, int64_t N) {
+  const int first = (int)((N - g0) < (int64_t)len ? (N - g0) : (int64_t)len);
+  bulk_s2g_if(p, dst + g0, src, (uint32_t)(first * sizeof(R)));
+  bulk_s2g_if(p && len > first, dst, src + first, (uint32_t)((len - first) * sizeof(R)));
 }
 // orders this thread's generic-proxy view against the async (TMA) proxy, all state spaces: after a flag has been
 // acquired and before a bulk load of what it guards; after bulk stores have completed and before the flag is raised
@@ -195,19 +221,17 @@ __global__ void __launch_bounds__(128) swept_flow_kernel(const FlowArgs<typename
     const R* in1 = (r & 1) ? a.buf[0][1] : a.buf[1][1];
     if constexpr (TMA) {
       // bulk loads over [S-PAD, S+n+PAD): the 16-byte pad holds the halo (what lies beyond it is never used)
-      if (lane == 0) {
-        fence_proxy_async_all();  // what the flags guard is read through the async proxy
-        const int nrows = r == 0 ? 1 : 2;
-        mbar_arrive_expect_tx(mbar, (uint32_t)(nrows * C * RS * sizeof(R)));
+      const bool issuer = lane == 0;  // the copies are issued by one lane, by predication, not by a branch
+      fence_proxy_async_all();        // what the flags guard is read through the async proxy
+      mbar_arrive_expect_tx_if(issuer, mbar, (uint32_t)((r == 0 ? 1 : 2) * C * RS * sizeof(R)));
 #pragma unroll
-        for (int c = 0; c < C; ++c) {
-          bulk_load_wrapped<R>(rows + c * RS, in0 + (int64_t)c * N, S - PAD, RS, N, mbar);
-          if (r != 0) bulk_load_wrapped<R>(rows + (C + c) * RS, in1 + (int64_t)c * N, S - PAD, RS, N, mbar);
-        }
+      for (int c = 0; c < C; ++c) {
+        bulk_load_wrapped<R>(issuer, rows + c * RS, in0 + (int64_t)c * N, S - PAD, RS, N, mbar);
+        bulk_load_wrapped<R>(issuer && r != 0, rows + (C + c) * RS, in1 + (int64_t)c * N, S - PAD, RS, N, mbar);
       }
       if (r == 0)
         for (int i = lane; i < C * RS; i += 32) rows[C * RS + i] = (R)0;
-      mbar_wait(mbar, phase);
+      mbar_wait_warp(mbar, phase);
       phase ^= 1u;
     } else {
       if (r == 0) {
@@ -243,18 +267,17 @@ __global__ void __launch_bounds__(128) swept_flow_kernel(const FlowArgs<typename
     if constexpr (TMA) {
       fence_proxy_async_smem();
       __syncwarp();
-      if (lane == 0) {
+      const bool issuer = lane == 0;
 #pragma unroll
-        for (int c = 0; c < C; ++c) {
-          bulk_store_wrapped<R>(out0 + (int64_t)c * N, rows + c * RS + PAD, S, n, N);
-          if (r != a.rows - 1)  // Down leaves only row 0: the full time level
-            bulk_store_wrapped<R>(out1 + (int64_t)c * N, rows + (C + c) * RS + PAD, S, n, N);
-        }
-        bulk_commit();
-        bulk_wait_all();  // the writes are complete (not just the shared-memory reads)
-        fence_proxy_async_all();
-        st_release_gpu(a.flags + (size_t)(r & 1) * a.K + k, r + 1);
+      for (int c = 0; c < C; ++c) {
+        bulk_store_wrapped<R>(issuer, out0 + (int64_t)c * N, rows + c * RS + PAD, S, n, N);
+        // Down leaves only row 0: the full time level
+        bulk_store_wrapped<R>(issuer && r != a.rows - 1, out1 + (int64_t)c * N, rows + (C + c) * RS + PAD, S, n, N);
       }
+      bulk_commit();    // (a lane without copies commits and waits for an empty group)
+      bulk_wait_all();  // the writes are complete (not just the shared-memory reads)
+      fence_proxy_async_all();
+      st_release_gpu_if(issuer, a.flags + (size_t)(r & 1) * a.K + k, r + 1);
     } else {
       __syncwarp();
 #pragma unroll

@@ -83,7 +83,7 @@ def flow_profile(emit, logns, widths):
         st = sw.Swept.from_workload(w)
         u0_dev = torch.from_numpy(np.ascontiguousarray(w.u0)).cuda()
         for n in widths:
-            for grp in (2, 3, 4, 6, 16 + 3, 16 + 4):  # resident CTAs per SM; +16 = TMA staging
+            for grp in (2, 3, 4, 6, 16 + 2, 16 + 3, 16 + 4, 16 + 6):  # resident CTAs per SM; +16 = TMA staging
                 try:
                     plain = _time(torch, st, u0_dev, w.nsteps, n, sw.SWEPT, sw.FLAVOR_FLOW, grp, 2)
                     sw.swept_flow_profile(st._h, True)
@@ -197,8 +197,8 @@ def main(argv=None):
                 if N % n:
                     continue
                 best = None
-                cands = [(sw.FLAVOR_FLOW, 0), (sw.FLAVOR_FLOW, 16), (sw.FLAVOR_CHAR, 32), (sw.FLAVOR_CHAR, 16),
-                         (sw.FLAVOR_CHAR, 8), (sw.FLAVOR_TIER, 0),   # FLOW group 16 = TMA staging
+                cands = [(sw.FLAVOR_FLOW, 0), (sw.FLAVOR_FLOW, 3), (sw.FLAVOR_CHAR, 32), (sw.FLAVOR_CHAR, 16),
+                         (sw.FLAVOR_CHAR, 8), (sw.FLAVOR_TIER, 0),   # FLOW group 0 = defaults (TMA staging); 3 = 16-byte copies, 3 CTAs/SM
                          (sw.FLAVOR_CLUSTER, 0), (sw.FLAVOR_CLUSTER, 8), (sw.FLAVOR_CLUSTER, 16)]  # group = warps per CTA
                 for fl, grp in cands:
                     try:
