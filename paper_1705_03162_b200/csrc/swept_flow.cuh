@@ -130,11 +130,15 @@ __device__ __forceinline__ void st_release_gpu_if(bool p, int* ptr, int v) {
 template <class R>
 __device__ __forceinline__ void bulk_load_wrapped(bool p, R* dst, const R* __restrict__ src, int64_t g0, int len, int64_t N,
                                                   uint64_t* bar) {
-  // at most two pieces (len <= N): up to the end of the row, and the rest from its start
+  // at most three pieces (len <= N + 2 pads; a single tile, n = N, wraps at both ends): up to the end of the row, a
+  // whole row or the rest from its start, and what is still left from the start again
   const int64_t g = g0 < 0 ? g0 + N : g0;
   const int first = (int)((N - g) < (int64_t)len ? (N - g) : (int64_t)len);
+  const int second = (int)((int64_t)(len - first) < N ? (int64_t)(len - first) : N);
+  const int third = len - first - second;
   bulk_g2s_if(p, dst, src + g, (uint32_t)(first * sizeof(R)), bar);
-  bulk_g2s_if(p && len > first, dst + first, src, (uint32_t)((len - first) * sizeof(R)), bar);
+  bulk_g2s_if(p && second > 0, dst + first, src, (uint32_t)(second * sizeof(R)), bar);
+  bulk_g2s_if(p && third > 0, dst + first + second, src, (uint32_t)(third * sizeof(R)), bar);
 }
 template <class R>
 __device__ __forceinline__ void bulk_store_wrapped(bool p, R* __restrict__ dst, const R* src, int64_t g0, int len, int64_t N) {
