@@ -464,6 +464,15 @@ void default_tile(const swept_state* s, int* n_io, int* flavor_io, int* P_io) {
       return;
     }
   }
+  // ... on a medium one (2^14 <= N < 2^19, a multiple of 256) the same flavour at n = 256: with TMA staging the persistent
+  // launch beats a launch per row of tiles from N = 2^14 up (profiles/r2_sweep_heat_f64.csv, r2_sweep_ks.csv)
+  if (n == 0 && flavor == SWEPT_FLAVOR_AUTO && !s->bc && (s->problem == SWEPT_HEAT || s->problem == SWEPT_KS) &&
+      s->N >= (1 << 14) && s->N < (1 << 19) && tile_ok(s, SWEPT_FLAVOR_FLOW, 256, 0)) {
+    *n_io = 256;
+    *flavor_io = SWEPT_FLAVOR_FLOW;
+    *P_io = 0;
+    return;
+  }
   // ... and on a small one (N <= 8192: at most 64 warp-sized tiles), where every flavour is bound by the latency of
   // the dependent tiers, the CLUSTER flavour: one launch per cycle, rows chained through distributed shared memory
   if (n == 0 && flavor == SWEPT_FLAVOR_AUTO && !s->bc && (s->problem == SWEPT_HEAT || s->problem == SWEPT_KS) && s->N <= 8192) {

@@ -196,3 +196,14 @@ def test_three_subtimesteps_remainder(nsub):
         assert (len(rows) - 1) % 3 == 0
     rem = sum(p[3] for p in plan if p[0] == REM)
     assert rem % 3 == 0 and rem < 3 * (32 // (2 * h))
+
+
+def test_plan_sigma_rejects_bad_arguments():
+    with pytest.raises(sw.SweptError):
+        sw.swept_plan(10, 64, 2, 3)   # nsub must be a whole number of timesteps (a multiple of sigma)
+    with pytest.raises(sw.SweptError):
+        sw.swept_plan(12, 64, 2, 4)   # sigma must be 1, 2 or 3
+    # sigma = 3: every cycle has a multiple of 3 rows after the Up row
+    plan = sw.swept_plan(3 * 100, 64, 2, 3)
+    for w in {p[4] for p in plan if p[0] != REM}:
+        assert (sum(1 for p in plan if p[4] == w and p[0] != REM) - 1) % 3 == 0

@@ -76,3 +76,14 @@ def test_message_volume_per_phase_matches_the_survey():
     assert len(top) == sum(1 for p in plan if p[4] == n and p[0] != 3)
     per_step_messages = 2 * 10000          # a per-step scheme exchanges its halo every sub-timestep, both ways
     assert len(xch) < per_step_messages / 100
+
+
+def test_exchange_list_rejects_bad_arguments():
+    plan = sw.swept_plan(64, 32, 1)
+    with pytest.raises(sw.SweptError):
+        sw.swept_shard_exchanges(plan, 3, 1, 64)      # h must be 1 or 2
+    with pytest.raises(sw.SweptError):
+        sw.swept_shard_exchanges(plan, 1, 4, 64)      # sigma must be 1, 2 or 3
+    with pytest.raises(sw.SweptError):
+        sw.swept_shard_exchanges(plan, 1, 1, 0)       # n_local must be positive
+    assert sw.swept_shard_exchanges([], 1, 1, 64) == []
