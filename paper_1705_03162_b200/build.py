@@ -16,13 +16,13 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 BUILD = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libswept_b200.so")
-# (source, object stem, extra defines); the Euler swept kernels are compiled in six parallel slices
-SOURCES = [("swept_api.cu", "swept_api", []), ("probes.cu", "probes", []), ("shard_kernels.cu", "shard_kernels", []),
+# (source, object stem, extra defines); the Euler swept kernels are compiled in four parallel slices, slowest first
+SOURCES = [("kernels_euler_inst.cu", f"kernels_euler_i{i}r{r}", [f"-DSWEPT_INST={i}", f"-DSWEPT_RK2={r}"])
+           for i in (1, 0) for r in (0, 1)]
+SOURCES += [("swept_api.cu", "swept_api", []), ("probes.cu", "probes", []), ("shard_kernels.cu", "shard_kernels", []),
            ("kernels_heat.cu", "kernels_heat", []), ("kernels_ks.cu", "kernels_ks", []),
            ("kernels_ks3.cu", "kernels_ks3", []),
            ("kernels_euler.cu", "kernels_euler", [])]
-SOURCES += [("kernels_euler_inst.cu", f"kernels_euler_i{i}r{r}", [f"-DSWEPT_INST={i}", f"-DSWEPT_RK2={r}"])
-            for i in (2, 1, 0) for r in (0, 1)]
 NVCC_FLAGS = ["-std=c++17", "-O3", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "-fmad=false", "-prec-div=true", "-prec-sqrt=true", "-ftz=false",
               "-Xcompiler", "-fPIC"]

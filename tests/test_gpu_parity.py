@@ -65,7 +65,7 @@ def admissible(w, n, flavor, group, dtype=np.float64):
             if L not in (8, 16, 32) or n % L:
                 continue
             B = n // L
-            if B not in ((4, 8, 16, 32) if h == 1 else (8, 16, 32)) or B > (16 if problem == si.EULER else 32):
+            if B not in ((4, 8, 16, 32) if h == 1 else (8, 16, 32)) or B > (8 if problem == si.EULER else 32):
                 continue
             T = 64 if N % (64 * B) == 0 else 32 if N % (32 * B) == 0 else 0
             if T >= L:
