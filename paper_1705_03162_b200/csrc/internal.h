@@ -54,6 +54,7 @@ struct FlowLaunch {
   unsigned* ticket;  // 4 words: task counter, sticky error word, leave counter, unused; counters zero
   int ctas_per_sm;   // bits 0..3: resident CTAs (of 4 warps) per SM, 0 = default policy; bit 4: TMA staging
   unsigned long long* prof = nullptr;  // 8 device counters: run the instrumented kernel (swept_flow_profile)
+  int bc = 0;        // kernel boundary mode: 0 wrap, 1 mirror (insulated heat ends: wall tiles advance tier by tier)
   const double* consts;
   cudaStream_t stream;
 };

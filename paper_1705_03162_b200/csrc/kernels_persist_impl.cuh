@@ -138,7 +138,7 @@ inline bool flow_ok(int64_t N, int n) {
   return B <= BMAX && B % (2 * Prob::H) == 0 && n / (2 * Prob::H) >= 32;
 }
 
-template <class Prob, int B, bool TMA, bool PROF = false>
+template <class Prob, int B, bool TMA, bool PROF = false, bool WALLS = false>
 inline int flow_go(const FlowLaunch& a) {
   using R = typename Prob::R;
   constexpr int warps = 4;  // one per scheduler
@@ -150,8 +150,9 @@ inline int flow_go(const FlowLaunch& a) {
   f.N = a.N; f.K = (int)(a.N / a.n); f.rows = a.rows; f.flags = a.flags; f.ticket = a.ticket;
   f.k = round_consts<R>(a.consts);
   f.prof = a.prof;
+  f.bc = a.bc;
   const size_t smem = flow_smem_bytes<Prob>(warps, a.n);
-  auto kern = swept_flow_kernel<Prob, B, TMA, PROF>;
+  auto kern = swept_flow_kernel<Prob, B, TMA, PROF, WALLS>;
   cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (e != cudaSuccess) return (int)e;
   // never launch more CTAs than can be co-resident: waiting tasks must not keep their parents off the machine
@@ -185,6 +186,17 @@ int flow_T(const FlowLaunch& a) {
   // group bit 4: stage the tiles with TMA bulk copies; group 0 (library defaults) does too — measured faster at every
   // size once the kernel around them compiled as tightly as the 16-byte-copy one (profiles/r2_flow_phases.md)
   const bool tma = (a.ctas_per_sm & 16) != 0 || a.ctas_per_sm == 0;
+  if (a.bc) {  // insulated ends (heat): the TMA-staged kernel with the wall-tile path
+    if constexpr (Prob::H == 1 && Prob::C == 1 && Prob::SIGMA == 1) {
+      if (a.bc != BC_MIRROR || a.prof) return NO_KERNEL;
+      switch (a.n / 32) {
+        case 8: return flow_go<Prob, 8, true, false, true>(a);
+        case 16: return flow_go<Prob, 16, true, false, true>(a);
+        case 32: return flow_go<Prob, 32, true, false, true>(a);
+      }
+    }
+    return NO_KERNEL;
+  }
   if (a.prof) {  // instrumented kernels (swept_flow_profile): the 3-point FP64 problem, the headline's kernel family
     if constexpr (Prob::H == 1 && sizeof(typename Prob::R) == 8) {
       switch (a.n / 32) {

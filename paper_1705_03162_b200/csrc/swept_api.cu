@@ -204,6 +204,7 @@ int launch_flow(swept_state* s, swept::FlowLaunch& a) {
   a.ticket = (unsigned*)s->flow_scratch;
   a.flags = s->flow_scratch + 4;
   a.prof = s->flow_prof_on ? s->flow_prof : nullptr;
+  a.bc = s->kernel_bc();
   int rc;
   switch (s->problem) {
     case SWEPT_HEAT: rc = swept::launch_flow_heat(s->dtype, a); break;
@@ -268,8 +269,11 @@ struct TimedScope {
 
 bool tile_ok(const swept_state* s, int flavor, int n, int P) {
   if (n <= 0 || s->N % n != 0) return false;
-  // walls are applied by the TIER kernels; the CHAR flavour can run beside them on all other tiles (heat: hybrid)
-  if (s->bc && flavor != SWEPT_FLAVOR_TIER && !(flavor == SWEPT_FLAVOR_CHAR && s->problem == SWEPT_HEAT)) return false;
+  // walls are applied by the TIER kernels; for heat also by the CHAR flavour in hybrid mode (wall tiles by TIER launches
+  // beside it) and by the FLOW flavour (wall tiles tier by tier inside the persistent launch)
+  if (s->bc && flavor != SWEPT_FLAVOR_TIER &&
+      !((flavor == SWEPT_FLAVOR_CHAR || flavor == SWEPT_FLAVOR_FLOW) && s->problem == SWEPT_HEAT))
+    return false;
   if (s->bc && flavor == SWEPT_FLAVOR_CHAR && !swept::tile_config_ok_heat(s->dtype, SWEPT_FLAVOR_TIER, s->N, n, 1))
     return false;
   if (flavor == SWEPT_FLAVOR_CLUSTER && (s->bc || (s->problem != SWEPT_HEAT && s->problem != SWEPT_KS))) return false;
@@ -851,7 +855,8 @@ swept_state* swept_create(int problem, int64_t N, double dx, double dt, const sw
   // allocates or synchronises: FLOW (periodic heat / KS, N a multiple of its narrowest tile) needs a ticket word,
   // a leave counter, an error word and 2 N/256 flags; PS_RESIDENT one flag line and two exchange lines per CTA.
   cudaError_t e = cudaSuccess;
-  if ((problem == SWEPT_HEAT || problem == SWEPT_KS) && q.bc == SWEPT_BC_PERIODIC && N % FLOW_MIN_WIDTH == 0) {
+  if (((problem == SWEPT_HEAT || problem == SWEPT_KS) && q.bc == SWEPT_BC_PERIODIC || (problem == SWEPT_HEAT && q.bc)) &&
+      N % FLOW_MIN_WIDTH == 0) {
     s->flow_scratch_ints = 4 + 2 * (size_t)(N / FLOW_MIN_WIDTH);
     s->flow_scratch = (int*)dev_alloc(s, s->flow_scratch_ints * sizeof(int));
     if (s->flow_scratch) e = cudaMemsetAsync(s->flow_scratch, 0, s->flow_scratch_ints * sizeof(int), s->stream);

@@ -53,6 +53,7 @@ struct FlowArgs {
   // PROF kernels only: 8 counters, summed over all warps — SM cycles spent [0] taking a ticket, [1] waiting for the
   // parents' flags, [2] staging the tile, [3] sweeping, [4] storing and publishing; [5] tiles done
   unsigned long long* prof;
+  int bc;  // WALLS kernels: BC_MIRROR = insulated ends (heat, Eq. (B.5)); else 0
 };
 
 // polling load: relaxed at GPU scope (no L1 invalidation per poll); the acquire fence follows once the flag is seen
@@ -150,6 +151,68 @@ __device__ __forceinline__ void bulk_store_wrapped(bool p, R* __restrict__ dst, 
 // acquired and before a bulk load of what it guards; after bulk stores have completed and before the flag is raised
 __device__ __forceinline__ void fence_proxy_async_all() { asm volatile("fence.proxy.async;" ::: "memory"); }
 
+// A tile that touches a wall (non-periodic ends, row f1): "node 0 is split across the spatial boundary and must apply the
+// boundary conditions at its center".  The characteristic sweep cannot run through a wall (its lines
+// reflect there), so the warp that draws such a tile advances it tier by tier in its shared-memory slice, as the TIER
+// flavour does for a whole CTA: lane l owns the P = n/32 points l P .. l P + P - 1, a tier reads the other row, and the
+// insulated ends T_{-1} = T_1, T_N = T_{N-2} (Eq. (B.5)) are applied where the stencil would cross the wall:
+//   wl / wr : the tile's first / last point is the domain's (aligned rows: the first / last tile of the row);
+//   split   : the tile wraps, point N-1 sits at slot n/2 - 1 and point 0 at slot n/2 (shifted rows: the last tile).
+// One __syncwarp() per tier; the same tier ranges and the same Heat::point as every other flavour, so the same bits.
+// Points are dealt to the lanes in quads, round-robin (lane l owns points 4 l .. 4 l + 3, 128 + 4 l .., ...: consecutive
+// lanes touch consecutive 16-byte words — with a block of n/32 points per lane every access was a 32-way bank conflict and
+// a wall tile took 5.5 tile times); all loads of a tier are issued before its first store (a skip of the groups outside
+// the tier's range was tried: the branches serialise the loads and cost more than they save).
+// The wall tiles of successive rows depend on one another, so rows x (time of a wall tile) bounds the launch from
+// below.  A wall tile computes every point at every tier (1.8 x the arithmetic of a swept tile, whose skew wastes 11 %),
+// on a scheduler it shares with two sweeping warps: measured 1.75 (n = 256) to 2 (n = 512) tile times.  So the flavour
+// pays where a warp has more than twice as many tiles per row to do as there are rows per tile: N >= 2^21 (4.4e12
+// against 4.1e12 for the hybrid CHAR + TIER-walls path at N = 2^22; 2.9e12 against 3.0e12 at 2^20); the autotuner decides.
+template <class Prob, int B, int KIND>
+__device__ __forceinline__ void flow_wall_tile(typename Prob::R* rows, const int RS, const int pad, const int lane,
+                                               const bool wl, const bool wr, const bool split,
+                                               const Consts<typename Prob::R>& k) {
+  using R = typename Prob::R;
+  static_assert(Prob::H == 1 && Prob::C == 1 && Prob::SIGMA == 1, "walls in the FLOW flavour: the heat problem");
+  constexpr int n = 32 * B, m = n / 2;
+  const int ntiers = KIND == KIND_UP ? m - 1 : (KIND == KIND_DOWN ? m : 2 * m - 1);
+  for (int t = 1; t <= ntiers; ++t) {
+    // (source and destination are different rows: all loads of a tier are issued before its first store)
+    const R* __restrict__ src = rows + ((t - 1) & 1) * RS + pad;  // phases start on even tiers: odd tiers read row 0
+    R* __restrict__ dst = rows + (t & 1) * RS + pad;
+    int lo, hi;
+    tier_range<KIND>(t, n, 1, m, lo, hi);
+    // lane l owns the quads of consecutive points 4 (32 g + l) .. + 3, g < B/4: one 16-byte-vector load of the quad (two
+    // for FP64) and its two outer neighbours instead of three loads per point; every quad, in range or not (no branch,
+    // so that the loads of a tier overlap)
+    R o[B];
+#pragma unroll
+    for (int g = 0; g < B / 4; ++g) {
+      const int q0 = 4 * (g * 32 + lane);
+      alignas(16) R body[4];
+      constexpr int NV = (int)(4 * sizeof(R) / 16);
+#pragma unroll
+      for (int v = 0; v < NV; ++v)
+        reinterpret_cast<int4*>(body)[v] = reinterpret_cast<const int4*>(src + q0)[v];
+      R left = src[q0 - 1], right = src[q0 + 4];
+      if ((wl && q0 == 0) || (split && q0 == n / 2)) left = body[1];                   // T_{-1} = T_1
+      if ((wr && q0 + 4 == n) || (split && q0 + 4 == n / 2)) right = body[2];          // T_N = T_{N-2}
+      o[4 * g + 0] = Prob::point(left, body[0], body[1], k);
+      o[4 * g + 1] = Prob::point(body[0], body[1], body[2], k);
+      o[4 * g + 2] = Prob::point(body[1], body[2], body[3], k);
+      o[4 * g + 3] = Prob::point(body[2], body[3], right, k);
+    }
+#pragma unroll
+    for (int g = 0; g < B / 4; ++g)
+#pragma unroll
+      for (int e = 0; e < 4; ++e) {
+        const int j = 4 * (g * 32 + lane) + e;
+        if (j >= lo && j < hi) dst[j] = o[4 * g + e];
+      }
+    __syncwarp();
+  }
+}
+
 #ifndef FLOW_MAX_SLEEP
 #define FLOW_MAX_SLEEP 256
 #endif
@@ -161,7 +224,8 @@ __device__ __forceinline__ void fence_proxy_async_all() { asm volatile("fence.pr
 // which one surrounds it (profiles/r2_flow_phases.md); swept_autotune measures both.
 // PROF = true: the same kernel with clock64() stamps between the parts of a task (swept_flow_profile; the timings
 // in profiles/r2_flow_phases.md).
-template <class Prob, int B, bool TMA, bool PROF = false>
+// WALLS = true: non-periodic ends (a.bc): the one or two tiles of a row that touch a wall go to flow_wall_tile.
+template <class Prob, int B, bool TMA, bool PROF = false, bool WALLS = false>
 __global__ void __launch_bounds__(128) swept_flow_kernel(const FlowArgs<typename Prob::R> a) {
   using R = typename Prob::R;
   constexpr int H = Prob::H, C = Prob::C, PAD = Pad16<R>::value, L = 32;
@@ -261,7 +325,18 @@ __global__ void __launch_bounds__(128) swept_flow_kernel(const FlowArgs<typename
     __syncwarp();
     if constexpr (PROF) { t1 = clock64(); pc[2] += t1 - t0; t0 = t1; }
     // ---- sweep (identical arithmetic and order to the CHAR flavour)
-    if (r == 0) char_sweep_tile<Prob, B, L, KIND_UP, RS>(rows, RS, PAD + n / 2, lane, a.k);
+    bool walled = false;
+    if constexpr (WALLS) {
+      const bool wl = !(r & 1) && k == 0, wr = !(r & 1) && k == a.K - 1, split = (r & 1) && k == a.K - 1;
+      walled = wl || wr || split;
+      if (walled) {
+        if (r == 0) flow_wall_tile<Prob, B, KIND_UP>(rows, RS, PAD, lane, wl, wr, split, a.k);
+        else if (r == a.rows - 1) flow_wall_tile<Prob, B, KIND_DOWN>(rows, RS, PAD, lane, wl, wr, split, a.k);
+        else flow_wall_tile<Prob, B, KIND_WHOLE>(rows, RS, PAD, lane, wl, wr, split, a.k);
+      }
+    }
+    if (walled) {
+    } else if (r == 0) char_sweep_tile<Prob, B, L, KIND_UP, RS>(rows, RS, PAD + n / 2, lane, a.k);
     else if (r == a.rows - 1) char_sweep_tile<Prob, B, L, KIND_DOWN, RS>(rows, RS, PAD + n / 2, lane, a.k);
     else char_sweep_tile<Prob, B, L, KIND_WHOLE, RS>(rows, RS, PAD + n / 2, lane, a.k);
     if constexpr (PROF) { __syncwarp(); t1 = clock64(); pc[3] += t1 - t0; t0 = t1; }

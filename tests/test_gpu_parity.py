@@ -72,7 +72,9 @@ def admissible(w, n, flavor, group, dtype=np.float64):
                 return True
         return False
     if flavor == sw.FLAVOR_FLOW:  # persistent launch: periodic heat / KS, 32 lanes per tile, B = n/32 in {8, 16, 32}
-        return problem != si.EULER and not bc and n in (256, 512, 1024) and N % 256 == 0 and (group & 15) <= 12 and group < 32
+        if bc and problem != si.HEAT:   # walls inside the persistent launch: insulated heat ends only
+            return False
+        return problem != si.EULER and n in (256, 512, 1024) and N % 256 == 0 and (group & 15) <= 12 and group < 32
     raise ValueError(flavor)
 
 
@@ -256,9 +258,23 @@ def test_heat_insulated_ends_bc_paper():
                 ran += 1
                 assert np.array_equal(sx, ref2), ("hybrid", N, n, L)
         assert ran == sum(admissible(w2, n, sw.FLAVOR_CHAR, L) for n in (64, 256, 512, 1024) for L in (8, 16, 32)) >= 8
+        # FLOW with walls: the one or two wall tiles of a row advance tier by tier inside the persistent launch
+        ran = 0
+        for n in (256, 512, 1024):
+            for grp in (0, 2, 16 + 3):
+                sx = run_or_refusal(w2, steps, n, sw.FLAVOR_FLOW, grp)
+                if sx is None:
+                    continue
+                ran += 1
+                assert np.array_equal(sx, ref2), ("flow walls", N, n, grp)
+        assert ran == sum(admissible(w2, n, sw.FLAVOR_FLOW, g) for n in (256, 512, 1024) for g in (0, 2, 19)) >= 3
+    w3 = si.heat_insulated(1 << 14, 6, 34, 777)
+    assert np.array_equal(gpu_run(w3, 777, sw.SWEPT, 256, sw.FLAVOR_FLOW, dtype=np.float32)[0],
+                          oracle.run_workload(w3, dtype=np.float32))
+    e = si.euler_sod(2048, 10)
+    with pytest.raises(sw.SweptError):               # walls in the persistent flavour: heat only
+        gpu_run(e, 10, sw.SWEPT, 256, sw.FLAVOR_FLOW)
     s = sw.Swept.from_workload(w)
-    with pytest.raises(sw.SweptError):               # the persistent flavours are periodic only: clean error
-        s.run(10, 256, sw.SWEPT, sw.FLAVOR_FLOW)
     best = s.autotune(sw.SWEPT)
     s.run(300, 0, sw.SWEPT)
     assert np.array_equal(s.read(), oracle.run_workload(w)) and best >= 32
