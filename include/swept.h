@@ -299,6 +299,32 @@ int swept_shard_end(swept_state* s);
  * shards' staging buffers, ordered by events (no host synchronisation).  Asynchronous like swept_run. */
 int swept_shard_run(swept_state* const* shards, int32_t nshards, int64_t nsteps, int flavor);
 
+/* ---- an entry point that allocates nothing ---------------------------------------------------------------------
+ * Some callers cannot call cudaMalloc: code under CUDA graph capture, tight serving loops, harnesses that forbid it.
+ * swept_heat_flow_static advances the periodic heat problem (FTCS, Eq. (B.4); FP64) by ONE swept cycle
+ * — UpTriangle, D Split/WholeDiamond rows, DownTriangle in one persistent FLOW launch — with every
+ * byte of scratch in a file-scope device array of the library: the kernel's ticket / leave counters and per-tile
+ * flags, and three of the four row slabs of the two-row inter-launch state (the fourth is out_dev, which therefore
+ * holds intermediate rows until the launch ends).  It calls no cudaMalloc, cudaFree or allocating library routine and
+ * needs no swept_state.
+ *   in_dev, out_dev : DEVICE buffers of N doubles, 16-byte aligned, not overlapping; caller-owned
+ *   N               : points, a multiple of tile_width, N <= SWEPT_STATIC_MAX_N (65 536); larger -> SWEPT_EINVAL
+ *   nsteps          : a positive multiple of tile_width / 2 (the cycle's (D + 1) n/(2h) sub-timesteps, no remainder)
+ *   tile_width      : 256, 512 or 1024
+ *   dx, dt, alpha   : as swept_create (Fo = alpha dt / dx^2 computed in double on the host)
+ *   stream          : cudaStream_t; the call is asynchronous on it and runs on the CURRENT device
+ * The result is bit-identical to swept_run(..., SWEPT_SWEPT) on a state of the same problem (same kernel, same
+ * functor).  Limits: the array (SWEPT_STATIC_SCRATCH_BYTES = 1 576 960 bytes) is held by every GPU that loads the
+ * library until the process exits; ALL calls on a device share it, and it keeps the last call's contents (the
+ * counters and flags are cleared at the start of every call, on `stream`): calls that overlap on the GPU — two
+ * streams, two host threads — race; serialise them.  swept_heat_flow_static_check(stream) synchronises the stream and
+ * reports SWEPT_ECUDA if the last launch gave up waiting for a dependency (call it before the next launch clears the
+ * word). */
+enum { SWEPT_STATIC_MAX_N = 65536, SWEPT_STATIC_SCRATCH_BYTES = 4096 + 3 * 65536 * 8 };
+int swept_heat_flow_static(const double* in_dev, double* out_dev, int64_t N, int64_t nsteps, int32_t tile_width,
+                           double dx, double dt, double alpha, void* stream);
+int swept_heat_flow_static_check(void* stream);
+
 /* ---- measurement helpers --------------------------------------------------------------------------- */
 
 /* swept_probe_fp64 — run a register-only DFMA chain on every SM of `device` and return FP64 pipe

@@ -108,6 +108,9 @@ def load():
     lib.swept_shard_unpack.argtypes = [c_void_p, c_int64, c_void_p]
     lib.swept_shard_end.argtypes = [c_void_p]
     lib.swept_shard_run.argtypes = [POINTER(c_void_p), c_int32, c_int64, c_int]
+    lib.swept_heat_flow_static.argtypes = [c_void_p, c_void_p, c_int64, c_int64, c_int32, c_double, c_double, c_double,
+                                           c_void_p]
+    lib.swept_heat_flow_static_check.argtypes = [c_void_p]
     lib.swept_probe_fp64.argtypes = [c_int, c_void_p, POINTER(c_double)]
     lib.swept_probe_launch.argtypes = [c_int, c_void_p, c_int, POINTER(c_double)]
     lib.swept_probe_chain.argtypes = [c_int, c_void_p, POINTER(c_double)]
@@ -270,6 +273,22 @@ def swept_shard_exchanges(plan, h: int, sigma: int, n_local: int):
     lib.swept_shard_exchanges(arr, len(plan), h, sigma, n_local, out, cnt)
     return [(int(x.after_phase), int(x.dir), int(x.src_off), int(x.dst_off), int(x.count), int(x.rows))
             for x in out[:cnt]]
+
+
+STATIC_MAX_N = 65536  # SWEPT_STATIC_MAX_N
+
+
+def swept_heat_flow_static(in_dev: int, out_dev: int, N: int, nsteps: int, tile_width: int, dx: float, dt: float,
+                           alpha: float = 1.0, stream: int | None = None) -> None:
+    """One swept cycle of the periodic FP64 heat problem with all scratch in the library's static device array: no
+    allocation, no state.  ``in_dev`` / ``out_dev`` are DEVICE addresses of N doubles (e.g. ``tensor.data_ptr()``)."""
+    st = _current_stream() if stream is None else stream
+    _check(load().swept_heat_flow_static(in_dev, out_dev, N, nsteps, tile_width, dx, dt, alpha, st))
+
+
+def swept_heat_flow_static_check(stream: int | None = None) -> None:
+    st = _current_stream() if stream is None else stream
+    _check(load().swept_heat_flow_static_check(st))
 
 
 def swept_probe_fp64(device: int = -1) -> float:

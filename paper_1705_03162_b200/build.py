@@ -19,7 +19,7 @@ LIB = os.path.join(HERE, "libswept_b200.so")
 # (source, object stem, extra defines); the Euler swept kernels are compiled in four parallel slices, slowest first
 SOURCES = [("kernels_euler_inst.cu", f"kernels_euler_i{i}r{r}", [f"-DSWEPT_INST={i}", f"-DSWEPT_RK2={r}"])
            for i in (1, 0) for r in (0, 1)]
-SOURCES += [("swept_api.cu", "swept_api", []), ("probes.cu", "probes", []), ("shard_kernels.cu", "shard_kernels", []),
+SOURCES += [("swept_api.cu", "swept_api", []), ("probes.cu", "probes", []), ("flow_static.cu", "flow_static", []), ("shard_kernels.cu", "shard_kernels", []),
            ("kernels_heat.cu", "kernels_heat", []), ("kernels_ks.cu", "kernels_ks", []),
            ("kernels_ks3.cu", "kernels_ks3", []),
            ("kernels_euler.cu", "kernels_euler", [])]

@@ -129,4 +129,7 @@ bool tile_config_ok_euler(int dtype, int flavor, int64_t N, int n, int P);
 
 constexpr int NO_KERNEL = -1000;
 
+// sets the thread-local text swept_last_error() returns (for entry points that live outside swept_api.cu)
+void set_last_error(const char* msg);
+
 }  // namespace swept

@@ -69,6 +69,10 @@ std::map<TunedKey, TunedEntry> g_tuned;
 
 }  // namespace
 
+namespace swept {
+void set_last_error(const char* msg) { g_err = msg ? msg : ""; }
+}  // namespace swept
+
 struct swept_state {
   int problem = 0, dtype = 0, rk2 = 0, device = 0, bc = 0;
   int64_t N = 0;
