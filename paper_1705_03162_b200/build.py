@@ -62,6 +62,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
         return LIB
     os.makedirs(BUILD, exist_ok=True)
     nvcc = _nvcc()
+    import time
+    started = time.time()  # the library is stamped with the START of the build: a source edited while it ran is newer
 
     def compile_one(item) -> str:
         src, stem, defs = item
@@ -86,6 +88,10 @@ def build(force: bool = False, verbose: bool = False) -> str:
     r = subprocess.run([nvcc, "-shared", "-o", tmp, *objs], capture_output=True, text=True)
     if r.returncode != 0:
         raise RuntimeError(f"link failed:\n{r.stdout}\n{r.stderr}")
+    os.utime(tmp, (started, started))
+    for o in objs:
+        if os.path.getmtime(o) > started:
+            os.utime(o, (started, started))
     os.replace(tmp, LIB)
     return LIB
 
