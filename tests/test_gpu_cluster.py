@@ -102,6 +102,9 @@ def test_cluster_refusals():
     e = si.euler_double_sod(2048, 10)
     with pytest.raises(sw.SweptError):
         run(e, 128)
+    k3 = si.ks3_cos(2048, 56, 10)
+    with pytest.raises(sw.SweptError):
+        run(k3, 128)                      # three-row schemes: TIER only
     b = si.heat_insulated(2048, 6, 55, 10)
     with pytest.raises(sw.SweptError):
         run(b, 128)
