@@ -23,6 +23,7 @@ from __future__ import annotations
 import argparse
 import os
 import sys
+import threading
 
 import numpy as np
 
@@ -51,9 +52,34 @@ def probes(emit):
     import torch
     props = torch.cuda.get_device_properties(0)
     emit(f"# device: {props.name}, {props.multi_processor_count} SMs, max SM clock {props.clock_rate / 1e3:.0f} MHz")
-    fp64 = sw.swept_probe_fp64()
+    # SM clock and throttle reasons sampled WHILE the FP64 probe runs (NVML, from a thread), so that "of nominal" can be
+    # read against the clock actually held
+    clocks, reasons, stop = [], set(), threading.Event()
+
+    def poll():
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            h = pynvml.nvmlDeviceGetHandleByIndex(torch.cuda.current_device())
+            while not stop.is_set():
+                clocks.append(pynvml.nvmlDeviceGetClockInfo(h, pynvml.NVML_CLOCK_SM))
+                reasons.add(int(pynvml.nvmlDeviceGetCurrentClocksEventReasons(h)))
+                stop.wait(0.002)
+        except Exception:
+            pass
+
+    thr = threading.Thread(target=poll, daemon=True)
+    thr.start()
+    fp64 = max(sw.swept_probe_fp64() for _ in range(3))
+    stop.set()
+    thr.join(timeout=5)
     emit(f"probe,fp64_pipe_lane_instr_per_s,{fp64:.4e},TFLOP/s (FMA=2) {2 * fp64 / 1e12:.2f},of nominal "
          f"{fp64 / (props.multi_processor_count * 64 * props.clock_rate * 1e3):.3f}")
+    if clocks:
+        med = sorted(clocks)[len(clocks) // 2]
+        emit(f"probe,sm_clock_mhz_during_fp64_probe,{med},min {min(clocks)} max {max(clocks)} over {len(clocks)} samples,"
+             f"clock event reason masks {sorted(reasons)} (0 = none; 1 = gpu idle; 4 = sw power cap),"
+             f"of the pipe at the held clock {fp64 / (props.multi_processor_count * 64 * med * 1e6):.3f}")
     emit(f"probe,launch_us,{sw.swept_probe_launch(2000):.3f}")
     pair = sw.swept_probe_chain()
     emit(f"probe,dadd_dfma_pair_cycles,{pair:.2f},ns at max clock {pair / (props.clock_rate / 1e6):.2f}")
