@@ -256,7 +256,19 @@ __global__ void __launch_bounds__(128) swept_flow_kernel(const FlowArgs<typename
     t = __shfl_sync(0xffffffffu, t, 0);
     if (t >= ntasks) break;
     if constexpr (PROF) { t1 = clock64(); pc[0] += t1 - t0; t0 = t1; }
-    const int r = (int)(t / (unsigned)a.K), k = (int)(t % (unsigned)a.K);
+    const int r = (int)(t / (unsigned)a.K);
+    int k = (int)(t % (unsigned)a.K);
+    if constexpr (WALLS) {
+      // The wall tiles of successive rows depend on one another and each costs about two tile times: their chain is the
+      // critical path of the launch.  Hand them out FIRST in every row (aligned rows: tiles 0 and K-1; shifted rows: the
+      // split tile K-1), so that the chain runs beside the bulk of the row instead of after it.  Any order inside a row
+      // keeps the protocol (a tile waits only for tiles of the previous row, which hold smaller tickets).
+      if (a.K >= 2) {
+        const int j = k;
+        if (r & 1) k = j == 0 ? a.K - 1 : j - 1;
+        else k = j == 0 ? 0 : (j == 1 ? a.K - 1 : j - 1);
+      }
+    }
     const int64_t S = (int64_t)k * n + ((r & 1) ? n / 2 : 0);  // < N; copies wrap
     if (r > 0) {
       // parents: the tiles of row r-1 overlapping [S, S+n); row r-1 publishes (r-1) + 1
