@@ -305,6 +305,18 @@ def main():
         b.synchronize()
         if r >= 2:
             e2e_ms.append(a.elapsed_time(b))
+    # what the end-to-end figure is bound by: the two 8 MiB copies over PCIe, measured here with the same pinned buffers
+    copy_ms = {}
+    dev_tmp = torch.empty_like(u0_dev)
+    for name, dst, src in (("h2d", dev_tmp, host_in), ("d2h", host_out, dev_tmp)):
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        dst.copy_(src, non_blocking=True)
+        a.record()
+        for _ in range(10):
+            dst.copy_(src, non_blocking=True)
+        b.record()
+        b.synchronize()
+        copy_ms[name] = a.elapsed_time(b) / 10
     e2e_total = sum(e2e_ms)
     e2e_total = max_over_ranks(e2e_total, dist, "cuda")
     e2e_value = replica_value(updates_per_step, args.steps, world, e2e_total)
@@ -425,7 +437,13 @@ def main():
                                               "L2-resident within a step by nature of the workload",
                        "parallelism": "replicas only" if world > 1 else "single GPU"},
             "clocks": clocks, "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(w.u0.nbytes),
-                                      "d2h_bytes_per_step": int(w.u0.nbytes)},
+                                      "d2h_bytes_per_step": int(w.u0.nbytes),
+                                      "ms_per_step": e2e_total / args.steps,
+                                      "h2d_ms": copy_ms["h2d"], "d2h_ms": copy_ms["d2h"],
+                                      "h2d_gbs": w.u0.nbytes / copy_ms["h2d"] / 1e6,
+                                      "d2h_gbs": w.u0.nbytes / copy_ms["d2h"] / 1e6,
+                                      "note": "device time of the step + the two pinned-memory copies over PCIe "
+                                              "(measured beside it) + two host synchronisations"},
             "gpu_launches": int(launches_per_step * args.steps), "roofline": roofline,
             "cpu_baseline": cpu_base, "peaks_source": peak_src, "wall_s_timed_region": t_wall,
             "detail": detail}
