@@ -42,7 +42,7 @@ enum { SWEPT_HEAT = 0, SWEPT_KS = 1, SWEPT_EULER = 2,       /* problem (PAPER.md
        SWEPT_KS3 = 3 };  /* the KS discretisation (C.2) with THREE sub-timesteps per timestep (Shu-Osher SSP-RK3):
                             the case PAPER.md:131 says the two-row decomposition "must be adjusted" for — the
                             inter-launch state has three rows (tier modulo 3).  FP64, periodic; per-step and the
-                            swept TIER flavour */
+                            swept TIER and CLUSTER flavours */
 enum { SWEPT_PER_STEP = 0, SWEPT_SWEPT = 1 };               /* variant                           */
 enum { SWEPT_F64 = 0, SWEPT_F32 = 1 };                      /* dtype                             */
 enum { SWEPT_RK2_MIDPOINT = 0, SWEPT_RK2_HEUN = 1 };        /* KS/Euler integrator (
@@ -73,8 +73,9 @@ enum {
                              Up..Down cycle; a warp per tile, its points in registers, one shuffle exchange per
                              tier; the edges pass from row to row through distributed shared memory behind a
                              cluster barrier instead of global memory.
-                             Periodic heat (FP64, FP32) and KS; n = 64, 128, 256, 512; N / n <= 256 tiles (128 for
-                             n >= 256); group = warps per CTA (0 = as few as fit a cluster of 16 CTAs)     */
+                             Periodic heat (FP64, FP32), KS and KS3 (three register rows per lane, n <= 256);
+                             n = 64, 128, 256, 512; N / n <= 256 tiles (128 for n >= 256); group = warps per CTA
+                             (0 = as few as fit a cluster of 16 CTAs)                                      */
 };
 
 /* Optional device allocator hooks (so that PyTorch's caching allocator owns the memory).

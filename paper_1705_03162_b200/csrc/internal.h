@@ -123,6 +123,7 @@ int launch_flow_heat(int dtype, const FlowLaunch& a);
 int launch_flow_ks(int dtype, int rk2, const FlowLaunch& a);
 int launch_cluster_heat(int dtype, const ClusterLaunch& a);
 int launch_cluster_ks(int dtype, int rk2, const ClusterLaunch& a);
+int launch_cluster_ks3(int dtype, const ClusterLaunch& a);
 bool tile_config_ok_heat(int dtype, int flavor, int64_t N, int n, int P);
 bool tile_config_ok_ks(int dtype, int flavor, int64_t N, int n, int P);
 bool tile_config_ok_euler(int dtype, int flavor, int64_t N, int n, int P);

@@ -74,6 +74,7 @@ inline int cluster_warps_per_cta(int64_t K, int n, int want) {
 template <class Prob>
 inline bool cluster_ok(int64_t N, int n, int want_wpc) {
   if (n != 64 && n != 128 && n != 256 && n != 512) return false;
+  if (Prob::ROWS == 3 && n > 256) return false;  // three register rows per lane: at most 8 points each
   if (N % n || n / 32 < Prob::H || (n / (2 * Prob::H)) % 2) return false;
   return cluster_warps_per_cta<Prob>(N / n, n, want_wpc) != 0;
 }
@@ -92,7 +93,9 @@ inline int cluster_go(const ClusterLaunch& a) {
   while ((1 << c.chunk_log2) < c.chunk) ++c.chunk_log2;
   c.k = round_consts<R>(a.consts);
   const size_t smem = cluster_smem_bytes<Prob>(c.chunk);
-  auto kern = swept_cluster_kernel<Prob, P>;
+  void (*kern)(const ClusterArgs<R>) = nullptr;
+  if constexpr (Prob::ROWS == 3) kern = swept_cluster3_kernel<Prob, P>;
+  else kern = swept_cluster_kernel<Prob, P>;
   cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (e == cudaSuccess && cs > 8) e = cudaFuncSetAttribute(kern, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
   if (e != cudaSuccess) return (int)e;
@@ -124,7 +127,7 @@ int cluster_T(const ClusterLaunch& a) {
     case 2: return cluster_go<Prob, 2>(a);
     case 4: return cluster_go<Prob, 4>(a);
     case 8: return cluster_go<Prob, 8>(a);
-    case 16: return cluster_go<Prob, 16>(a);
+    case 16: if constexpr (Prob::ROWS == 2) return cluster_go<Prob, 16>(a); break;
   }
   return NO_KERNEL;
 }

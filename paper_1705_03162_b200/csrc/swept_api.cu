@@ -280,7 +280,7 @@ bool tile_ok(const swept_state* s, int flavor, int n, int P) {
     return false;
   if (s->bc && flavor == SWEPT_FLAVOR_CHAR && !swept::tile_config_ok_heat(s->dtype, SWEPT_FLAVOR_TIER, s->N, n, 1))
     return false;
-  if (flavor == SWEPT_FLAVOR_CLUSTER && (s->bc || (s->problem != SWEPT_HEAT && s->problem != SWEPT_KS))) return false;
+  if (flavor == SWEPT_FLAVOR_CLUSTER && (s->bc || s->problem == SWEPT_EULER)) return false;
   if (flavor == SWEPT_FLAVOR_FLOW && (s->problem == SWEPT_EULER || s->problem == SWEPT_KS3 || P < 0 || (P & 15) > 12 || P > 31 || !s->flow_scratch)) return false;
   switch (s->problem) {
     case SWEPT_HEAT: return swept::tile_config_ok_heat(s->dtype, flavor, s->N, n, P);
@@ -483,8 +483,10 @@ void default_tile(const swept_state* s, int* n_io, int* flavor_io, int* P_io) {
   }
   // ... and on a small one (N <= 8192: at most 64 warp-sized tiles), where every flavour is bound by the latency of
   // the dependent tiers, the CLUSTER flavour: one launch per cycle, rows chained through distributed shared memory
-  if (n == 0 && flavor == SWEPT_FLAVOR_AUTO && !s->bc && (s->problem == SWEPT_HEAT || s->problem == SWEPT_KS) && s->N <= 8192) {
-    for (int cand : {s->N <= 4096 ? 64 : 128, 128, 256})
+  const bool small_two_row = (s->problem == SWEPT_HEAT || s->problem == SWEPT_KS) && s->N <= 8192;
+  const bool small_three_row = s->problem == SWEPT_KS3 && s->N <= 16384;  // measured: 1.5-2.2 x the TIER flavour there
+  if (n == 0 && flavor == SWEPT_FLAVOR_AUTO && !s->bc && (small_two_row || small_three_row)) {
+    for (int cand : {s->N <= 4096 ? 64 : (s->N <= 8192 ? 128 : 256), 128, 256})
       if (tile_ok(s, SWEPT_FLAVOR_CLUSTER, cand, 0)) {
         *n_io = cand;
         *flavor_io = SWEPT_FLAVOR_CLUSTER;
@@ -644,7 +646,9 @@ int run_next_phase(swept_state* s) {
     int rc;
     {
       TimedScope ts(s, KIND_FLOW, 1);
-      rc = s->problem == SWEPT_HEAT ? swept::launch_cluster_heat(s->dtype, c) : swept::launch_cluster_ks(s->dtype, s->rk2, c);
+      rc = s->problem == SWEPT_HEAT ? swept::launch_cluster_heat(s->dtype, c)
+           : s->problem == SWEPT_KS ? swept::launch_cluster_ks(s->dtype, s->rk2, c)
+                                    : swept::launch_cluster_ks3(s->dtype, c);
     }
     if (rc == NO_KERNEL) return fail(SWEPT_EUNSUPPORTED, "no CLUSTER kernel for N=%lld n=%d", (long long)s->N, ph.n);
     if (rc != 0) return fail(SWEPT_ECUDA, "cluster launch: %s", cudaGetErrorString((cudaError_t)rc));

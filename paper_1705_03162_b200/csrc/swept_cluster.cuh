@@ -202,9 +202,141 @@ __global__ void __launch_bounds__(ClusterMaxThreads<P>::value) swept_cluster_ker
   cluster.sync();  // nobody leaves while a slower CTA may still be reading its shared memory
 }
 
+// ---------------------------------------------------------------------------------------------------------------
+// The same for a scheme with THREE sub-timesteps per timestep on a three-row state (Prob::ROWS == 3: KS3, SURVEY.md
+// §8(f) row f3).  Row p of a lane's registers holds the latest value with tier = p (mod 3); the tier with
+// global index g reads row (g - 1) % 3, writes row g % 3, is stage g % 3 of its timestep (1, 2, 0) and takes u^n from
+// row 0.  A cycle starts on a full time level, so row r >= 1 of tiles starts at global tier (r - 1) m (the Up row at 0),
+// whose residue differs from row to row (m is a power of two): the tier loop is instantiated for the three residues and
+// rotates the register rows statically.
+template <class Prob, int P, int G>
+__device__ __forceinline__ void cluster3_tier(typename Prob::R (&v)[3][Prob::C][P],
+                                              const typename Prob::R (&hl)[3][Prob::C][Prob::H],
+                                              const typename Prob::R (&hr)[3][Prob::C][Prob::H], const int t,
+                                              const int (&ta)[P], const unsigned (&span)[P], const int lane,
+                                              const Consts<typename Prob::R>& k) {
+  constexpr int SRC = (G + 2) % 3;
+  cluster_tier<Prob, P>(v[SRC], v[G], v[0], hl[SRC], hr[SRC], G, t, ta, span, lane, k);
+}
+
+template <class Prob, int P, int Q0>
+__device__ __forceinline__ void cluster3_tiers(typename Prob::R (&v)[3][Prob::C][P],
+                                               const typename Prob::R (&hl)[3][Prob::C][Prob::H],
+                                               const typename Prob::R (&hr)[3][Prob::C][Prob::H], const int ntiers,
+                                               const int (&ta)[P], const unsigned (&span)[P], const int lane,
+                                               const Consts<typename Prob::R>& k) {
+  int t = 1;  // relative tier t has global residue (Q0 + t) % 3
+  for (; t + 2 <= ntiers; t += 3) {
+    cluster3_tier<Prob, P, (Q0 + 1) % 3>(v, hl, hr, t, ta, span, lane, k);
+    cluster3_tier<Prob, P, (Q0 + 2) % 3>(v, hl, hr, t + 1, ta, span, lane, k);
+    cluster3_tier<Prob, P, Q0 % 3>(v, hl, hr, t + 2, ta, span, lane, k);
+  }
+  if (t <= ntiers) cluster3_tier<Prob, P, (Q0 + 1) % 3>(v, hl, hr, t, ta, span, lane, k);
+  if (t + 1 <= ntiers) cluster3_tier<Prob, P, (Q0 + 2) % 3>(v, hl, hr, t + 1, ta, span, lane, k);
+}
+
+template <class Prob, int P>
+__global__ void __launch_bounds__(ClusterMaxThreads<P>::value) swept_cluster3_kernel(const ClusterArgs<typename Prob::R> a) {
+  namespace cg = cooperative_groups;
+  using R = typename Prob::R;
+  constexpr int H = Prob::H, C = Prob::C;
+  static_assert(Prob::ROWS == 3 && Prob::SIGMA == 3, "three sub-timesteps per timestep on three rows");
+  static_assert(P >= H, "a lane's block must hold its neighbour's halo");
+  constexpr int n = 32 * P, m = n / (2 * H);
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  R* sm = reinterpret_cast<R*>(smem_raw);  // [buffer 2][row 3][component C][chunk]
+  cg::cluster_group cluster = cg::this_cluster();
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int wpc = blockDim.x >> 5;
+  const unsigned rank = cluster.block_rank();
+  const int64_t N = a.N;
+  const int64_t k_tile = (int64_t)rank * wpc + warp;
+  const int chunk = a.chunk;
+  auto dsm = [&](int buf, int row, int c, int64_t g) -> R* {
+    const int i = (int)(g & (n - 1));
+    const int off = (int)(g & (chunk - 1)) - i + (i % P) * 32 + i / P;  // lane-major inside the aligned block
+    R* local = sm + (size_t)((buf * 3 + row) * C + c) * chunk + off;
+    return cluster.map_shared_rank(local, (unsigned)(g >> a.chunk_log2));
+  };
+  auto wrap = [&](int64_t g) -> int64_t { return g < 0 ? g + N : (g >= N ? g - N : g); };
+
+  R v[3][C][P], hl[3][C][H], hr[3][C][H];
+  for (int r = 0; r < a.rows; ++r) {
+    const int kind = r == 0 ? KIND_UP : (r == a.rows - 1 ? KIND_DOWN : KIND_WHOLE);
+    const int64_t S = wrap(k_tile * n + ((r & 1) ? n / 2 : 0));
+    const int64_t g0 = wrap(S + lane * P);
+    const int inb = (r + 1) & 1, outb = r & 1;
+    if (kind == KIND_UP) {
+#pragma unroll
+      for (int c = 0; c < C; ++c) {
+#pragma unroll
+        for (int j = 0; j < P; ++j) {
+          v[0][c][j] = __ldg(a.init + (int64_t)c * N + g0 + j);
+          v[1][c][j] = v[2][c][j] = (R)0;  // tiers before the cycle's first do not exist
+        }
+#pragma unroll
+        for (int e = 0; e < H; ++e)
+#pragma unroll
+          for (int row = 0; row < 3; ++row) hl[row][c][e] = hr[row][c][e] = (R)0;  // never used by a triangle
+      }
+    } else {
+#pragma unroll
+      for (int row = 0; row < 3; ++row)
+#pragma unroll
+        for (int c = 0; c < C; ++c) {
+          const R* p = dsm(inb, row, c, g0);
+#pragma unroll
+          for (int j = 0; j < P; ++j) v[row][c][j] = p[j * 32];
+#pragma unroll
+          for (int e = 0; e < H; ++e) {
+            hl[row][c][e] = *dsm(inb, row, c, wrap(S - H + e));
+            hr[row][c][e] = *dsm(inb, row, c, wrap(S + n + e));
+          }
+        }
+    }
+    const int ntiers = kind == KIND_UP ? m - 1 : (kind == KIND_DOWN ? m : 2 * m - 1);
+    int ta[P];
+    unsigned span[P];
+#pragma unroll
+    for (int j = 0; j < P; ++j) {  // tier window of each point: as in swept_cluster_kernel
+      const int x = lane * P + j;
+      const int d = x < n / 2 ? n / 2 - x : x - n / 2 + 1;
+      const int first = (d + H - 1) / H;
+      const int edge = (x < n - 1 - x ? x : n - 1 - x) / H;
+      const int t0 = kind == KIND_UP ? 1 : first;
+      const int tb = kind == KIND_UP ? edge : (kind == KIND_DOWN ? m : 2 * m - first);
+      const bool never = tb < t0;
+      span[j] = never ? 0u : (unsigned)(tb - t0);
+      ta[j] = never ? (1 << 30) : t0;
+    }
+    // residue of the global tier this row of tiles starts at: the Up row at tier 0, diamond / Down row r at (r - 1) m
+    const int q0 = r == 0 ? 0 : (int)(((int64_t)(r - 1) * m) % 3);
+    if (q0 == 0) cluster3_tiers<Prob, P, 0>(v, hl, hr, ntiers, ta, span, lane, a.k);
+    else if (q0 == 1) cluster3_tiers<Prob, P, 1>(v, hl, hr, ntiers, ta, span, lane, a.k);
+    else cluster3_tiers<Prob, P, 2>(v, hl, hr, ntiers, ta, span, lane, a.k);
+    if (kind == KIND_DOWN) {  // the cycle ends on a full timestep: row 0 is the time level
+#pragma unroll
+      for (int c = 0; c < C; ++c)
+#pragma unroll
+        for (int j = 0; j < P; ++j) a.out[(int64_t)c * N + g0 + j] = v[0][c][j];
+    } else {
+#pragma unroll
+      for (int row = 0; row < 3; ++row)
+#pragma unroll
+        for (int c = 0; c < C; ++c) {
+          R* p = dsm(outb, row, c, g0);
+#pragma unroll
+          for (int j = 0; j < P; ++j) p[j * 32] = v[row][c][j];
+        }
+      cluster.sync();
+    }
+  }
+  cluster.sync();
+}
+
 template <class Prob>
 inline size_t cluster_smem_bytes(int chunk) {
-  return (size_t)2 * 2 * Prob::C * (size_t)chunk * sizeof(typename Prob::R);
+  return (size_t)2 * Prob::ROWS * Prob::C * (size_t)chunk * sizeof(typename Prob::R);
 }
 
 }  // namespace swept

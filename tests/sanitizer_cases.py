@@ -65,6 +65,7 @@ def cases():
     yield "ks3 per_step", ks3, sw.PER_STEP, 0, 0, 0
     yield "ks3 TIER n=128 P=1", ks3, sw.SWEPT, 128, T, 1
     yield "ks3 TIER n=256 P=2", ks3, sw.SWEPT, 256, T, 2
+    yield "ks3 CLUSTER n=128", ks3, sw.SWEPT, 128, sw.FLAVOR_CLUSTER, 0
     yield "euler per_step (Heun)", eul, sw.PER_STEP, 0, 0, 0
     yield "euler per_step resident", eul, sw.PER_STEP, 0, sw.PS_RESIDENT, 0
     yield "euler TIER n=128 P=1 (Heun)", eul, sw.SWEPT, 128, T, 1

@@ -104,7 +104,7 @@ def test_cluster_refusals():
         run(e, 128)
     k3 = si.ks3_cos(2048, 56, 10)
     with pytest.raises(sw.SweptError):
-        run(k3, 128)                      # three-row schemes: TIER only
+        run(k3, 512)                      # three register rows per lane: n <= 256 (tests/test_gpu_ks3.py covers the rest)
     b = si.heat_insulated(2048, 6, 55, 10)
     with pytest.raises(sw.SweptError):
         run(b, 128)

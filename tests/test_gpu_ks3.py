@@ -99,3 +99,34 @@ def test_ks3_autotune_picks_an_admissible_width():
         assert np.array_equal(s.read(), oracle.run_workload(w))
     finally:
         s.close()
+
+
+@pytest.mark.parametrize("N,nsteps", [(128, 16), (2048, 100), (4096, 257), (16384, 64)])
+def test_ks3_cluster_flavour_matches_oracle(N, nsteps):
+    # the three-row scheme in registers: one thread-block cluster, a warp per tile, rows of tiles chained through
+    # distributed shared memory; diamonds start on any of the three stages (swept_cluster.cuh: swept_cluster3_kernel)
+    w = si.ks3_cos(N, 26, nsteps)
+    ref = oracle.run_workload(w)
+    ran = 0
+    for n in (64, 128, 256, 512):
+        for wpc in (0, 4, 8, 16):
+            K, P = N // n if N % n == 0 else 0, n // 32
+            max_wpc = 8 if P >= 8 else 16
+            ok = False
+            if K and n <= 256:
+                for cand in (1, 2, 4, 8, 16, 32):
+                    if (cand != wpc) if wpc else (cand < 4 and K > cand):
+                        continue
+                    if cand > max_wpc or K % cand or K // cand > 16 or 2 * 3 * cand * n * 8 > 200 * 1024:
+                        continue
+                    ok = True
+                    break
+            try:
+                got, launches = run(w, nsteps, sw.SWEPT, n, sw.FLAVOR_CLUSTER, wpc)
+            except sw.SweptError as e:
+                assert not ok, f"library refused n={n} wpc={wpc}: {e}"
+                continue
+            assert ok, f"library ran the inadmissible n={n} wpc={wpc}"
+            assert np.array_equal(got, ref), (n, wpc)
+            ran += 1
+    assert ran >= 2
