@@ -52,9 +52,10 @@ enum { SWEPT_RK2_MIDPOINT = 0, SWEPT_RK2_HEUN = 1 };        /* KS/Euler integrat
  * tube: cells -2, -1 and N, N+1 hold the states that swept_write found in the first and last
  * cell.  SWEPT_BC_PAPER is built for per-step (both flavours), the swept TIER flavour, where the
  * tile split across the boundary applies the condition at its centre, and for heat the CHAR
- * flavour in hybrid mode (wall tiles by the TIER kernels on a second stream) and the FLOW flavour
- * (the one or two wall tiles of a row advance tier by tier inside the persistent launch); KS (periodic in the paper,
- * PAPER.md:356), the CLUSTER flavour and Euler with FLOW / CHAR: SWEPT_EUNSUPPORTED. */
+ * flavour in hybrid mode (wall tiles by the TIER kernels on a second stream), the FLOW flavour
+ * (the one or two wall tiles of a row advance tier by tier inside the persistent launch) and the CLUSTER flavour (the
+ * lanes next to a wall take the mirror image of their own neighbour point); KS (periodic in the paper)
+ * and Euler with FLOW / CHAR / CLUSTER: SWEPT_EUNSUPPORTED. */
 enum { SWEPT_BC_PERIODIC = 0, SWEPT_BC_PAPER = 1 };
 enum { SWEPT_NKINDS = 6 };                                   /* phase kinds reported by swept_phase_times */
 enum { SWEPT_OK = 0, SWEPT_EINVAL = -1, SWEPT_EUNSUPPORTED = -2, SWEPT_ECUDA = -3, SWEPT_ENOMEM = -4 };

@@ -66,6 +66,7 @@ struct ClusterLaunch {
   int64_t N;
   int n, rows;       // tile width; rows = D + 2
   int warps_per_cta; // 0 = as few as fit a cluster of 16 CTAs
+  int bc = 0;        // kernel boundary mode: 0 wrap, 1 mirror (insulated heat ends)
   const double* consts;
   cudaStream_t stream;
 };

@@ -92,6 +92,8 @@ inline int cluster_go(const ClusterLaunch& a) {
   c.chunk_log2 = 0;
   while ((1 << c.chunk_log2) < c.chunk) ++c.chunk_log2;
   c.k = round_consts<R>(a.consts);
+  c.bc = a.bc;
+  if (a.bc && !(Prob::H == 1 && Prob::ROWS == 2 && a.bc == BC_MIRROR)) return NO_KERNEL;  // walls: the heat problem
   const size_t smem = cluster_smem_bytes<Prob>(c.chunk);
   void (*kern)(const ClusterArgs<R>) = nullptr;
   if constexpr (Prob::ROWS == 3) kern = swept_cluster3_kernel<Prob, P>;

@@ -276,11 +276,12 @@ bool tile_ok(const swept_state* s, int flavor, int n, int P) {
   // walls are applied by the TIER kernels; for heat also by the CHAR flavour in hybrid mode (wall tiles by TIER launches
   // beside it) and by the FLOW flavour (wall tiles tier by tier inside the persistent launch)
   if (s->bc && flavor != SWEPT_FLAVOR_TIER &&
-      !((flavor == SWEPT_FLAVOR_CHAR || flavor == SWEPT_FLAVOR_FLOW) && s->problem == SWEPT_HEAT))
+      !((flavor == SWEPT_FLAVOR_CHAR || flavor == SWEPT_FLAVOR_FLOW || flavor == SWEPT_FLAVOR_CLUSTER) &&
+        s->problem == SWEPT_HEAT))
     return false;
   if (s->bc && flavor == SWEPT_FLAVOR_CHAR && !swept::tile_config_ok_heat(s->dtype, SWEPT_FLAVOR_TIER, s->N, n, 1))
     return false;
-  if (flavor == SWEPT_FLAVOR_CLUSTER && (s->bc || s->problem == SWEPT_EULER)) return false;
+  if (flavor == SWEPT_FLAVOR_CLUSTER && s->problem == SWEPT_EULER) return false;
   if (flavor == SWEPT_FLAVOR_FLOW && (s->problem == SWEPT_EULER || s->problem == SWEPT_KS3 || P < 0 || (P & 15) > 12 || P > 31 || !s->flow_scratch)) return false;
   switch (s->problem) {
     case SWEPT_HEAT: return swept::tile_config_ok_heat(s->dtype, flavor, s->N, n, P);
@@ -485,7 +486,7 @@ void default_tile(const swept_state* s, int* n_io, int* flavor_io, int* P_io) {
   // the dependent tiers, the CLUSTER flavour: one launch per cycle, rows chained through distributed shared memory
   const bool small_two_row = (s->problem == SWEPT_HEAT || s->problem == SWEPT_KS) && s->N <= 8192;
   const bool small_three_row = s->problem == SWEPT_KS3 && s->N <= 16384;  // measured: 1.5-2.2 x the TIER flavour there
-  if (n == 0 && flavor == SWEPT_FLAVOR_AUTO && !s->bc && (small_two_row || small_three_row)) {
+  if (n == 0 && flavor == SWEPT_FLAVOR_AUTO && (!s->bc || s->problem == SWEPT_HEAT) && (small_two_row || small_three_row)) {
     for (int cand : {s->N <= 4096 ? 64 : (s->N <= 8192 ? 128 : 256), 128, 256})
       if (tile_ok(s, SWEPT_FLAVOR_CLUSTER, cand, 0)) {
         *n_io = cand;
@@ -641,6 +642,7 @@ int run_next_phase(swept_state* s) {
     c.n = ph.n;
     c.rows = (int)(jp - ip + 1);
     c.warps_per_cta = pr.cfg[ph.n].second;
+    c.bc = s->kernel_bc();
     c.consts = s->consts;
     c.stream = s->stream;
     int rc;

@@ -41,6 +41,7 @@ struct ClusterArgs {
   int chunk;      // points per CTA = warps per CTA * n (a power of two)
   int chunk_log2;
   Consts<R> k;
+  int bc = 0;  // BC_MIRROR: insulated ends (heat, Eq. (B.5)), applied by the lanes next to a wall
 };
 
 __device__ __forceinline__ double shfl_idx_(double v, int src) { return __shfl_sync(0xffffffffu, v, src); }
@@ -56,7 +57,8 @@ __device__ __forceinline__ void cluster_tier(const typename Prob::R (&vs)[Prob::
                                              const typename Prob::R (&hl)[Prob::C][Prob::H],
                                              const typename Prob::R (&hr)[Prob::C][Prob::H], const int par, const int t,
                                              const int (&ta)[P], const unsigned (&span)[P], const int lane,
-                                             const Consts<typename Prob::R>& k) {
+                                             const Consts<typename Prob::R>& k, const bool wall_l = false,
+                                             const bool wall_r = false) {
   using R = typename Prob::R;
   constexpr int H = Prob::H, C = Prob::C;
   R win[C][P + 2 * H], bs[C][P], o[C][P];
@@ -74,6 +76,12 @@ __device__ __forceinline__ void cluster_tier(const typename Prob::R (&vs)[Prob::
     for (int j = 0; j < P; ++j) {
       win[c][H + j] = vs[c][j];
       bs[c][j] = (Prob::SIGMA >= 2 && par != 1) ? v0[c][j] : vs[c][j];  // u^n: row 0
+    }
+    if constexpr (H == 1 && P >= 2) {
+      // a lane whose first / last point is an END POINT of the domain: the stencil's outer value is the mirror image
+      // of its own second / second-to-last point, T_{-1} = T_1 and T_N = T_{N-2} (Eq. (B.5), reading X17)
+      win[c][0] = wall_l ? vs[c][1] : win[c][0];
+      win[c][P + 1] = wall_r ? vs[c][P - 2] : win[c][P + 1];
     }
   }
   Prob::template stage<P>(win, bs, o, par, k);
@@ -175,9 +183,17 @@ __global__ void __launch_bounds__(ClusterMaxThreads<P>::value) swept_cluster_ker
     }
     // (Two tiers behind one shuffle exchange — 2h redundant evaluations per lane instead of a second exchange — was
     // built and measured: no faster for the 3-point scheme, 3 % for the 5-point one; not kept.)
+    // walls ("node 0 is split across the spatial boundary and must apply the boundary conditions at its center",
+    // PAPER.md:79-81): aligned rows: point 0 is lane 0 of the first tile, point N-1 lane 31 of the last; shifted rows:
+    // the last tile wraps, point N-1 is the last point of its lane 15 and point 0 the first of its lane 16
+    const int64_t K = N / n;
+    const bool shifted = (r & 1) != 0;
+    const bool wall_l = a.bc != 0 && (shifted ? (k_tile == K - 1 && lane == 16) : (k_tile == 0 && lane == 0));
+    const bool wall_r = a.bc != 0 && (shifted ? (k_tile == K - 1 && lane == 15) : (k_tile == K - 1 && lane == 31));
     for (int t = 1; t <= ntiers; t += 2) {
-      cluster_tier<Prob, P>(v0, v1, v0, hl0, hr0, 1, t, ta, span, lane, a.k);  // odd tier: reads row 0, writes row 1
-      if (t + 1 <= ntiers) cluster_tier<Prob, P>(v1, v0, v0, hl1, hr1, 0, t + 1, ta, span, lane, a.k);  // even: row 1 -> row 0
+      cluster_tier<Prob, P>(v0, v1, v0, hl0, hr0, 1, t, ta, span, lane, a.k, wall_l, wall_r);  // odd tier: row 0 -> row 1
+      if (t + 1 <= ntiers)
+        cluster_tier<Prob, P>(v1, v0, v0, hl1, hr1, 0, t + 1, ta, span, lane, a.k, wall_l, wall_r);  // even: row 1 -> row 0
     }
     // ---- hand the rows on: Down leaves the full time level (row 0) in global memory
     if (kind == KIND_DOWN) {

@@ -52,6 +52,7 @@ def cases():
     yield "heat walls TIER n=256", wall, sw.SWEPT, 256, T, 1
     yield "heat walls hybrid CHAR n=256", wall, sw.SWEPT, 256, C, 32
     yield "heat walls FLOW n=256", si.heat_insulated(4096, 6, 37, 300), sw.SWEPT, 256, F, 0
+    yield "heat walls CLUSTER n=128", wall, sw.SWEPT, 128, sw.FLAVOR_CLUSTER, 0
     yield "heat walls per_step", wall, sw.PER_STEP, 0, 0, 0
     yield "heat walls per_step resident", wall, sw.PER_STEP, 0, sw.PS_RESIDENT, 0
     yield "ks per_step (fused stages)", ks, sw.PER_STEP, 0, 0, 0

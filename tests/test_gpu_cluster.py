@@ -78,6 +78,36 @@ def test_ks_cluster_matches_oracle(N, nsteps, rk2):
     assert ran >= 2
 
 
+@pytest.mark.parametrize("N,nsteps", [(64, 50), (256, 333), (2048, 700), (8192, 1029)])
+def test_heat_insulated_ends_cluster(N, nsteps):
+    # the paper's own heat boundary condition (B.5) in the register-resident flavour: the lanes next to a wall take the
+    # mirror image of their own neighbour point instead of the shuffled value; K = 1 (one tile holds both walls), the
+    # split tile of the shifted rows, multi-level remainders; FP64 and FP32; slabs poisoned with NaNs
+    import os
+    os.environ["SWEPT_POISON"] = "1"
+    try:
+        w = si.heat_insulated(N, 6, 57, nsteps)
+        ref = oracle.run_workload(w)
+        ran = 0
+        for n in (64, 128, 256, 512):
+            for wpc in (0, 8):
+                if not admissible(si.HEAT, N, n, wpc):
+                    continue
+                got, _ = run(w, n, wpc)
+                assert np.array_equal(got, ref), (n, wpc)
+                ran += 1
+        assert ran >= 1
+        s = sw.Swept.from_workload(w)            # library default at these sizes: this flavour
+        s.run(nsteps, 0, sw.SWEPT)
+        assert np.array_equal(s.read(), ref)
+        s.close()
+        ref32 = oracle.run_workload(w, dtype=np.float32)
+        got32, _ = run(w, 64, 0, dtype=np.float32)
+        assert np.array_equal(got32, ref32)
+    finally:
+        del os.environ["SWEPT_POISON"]
+
+
 def test_heat_fp32_cluster():
     w = si.heat_sines(4096, 16, 53, 700)
     ref = oracle.run_workload(w, dtype=np.float32)
@@ -105,6 +135,6 @@ def test_cluster_refusals():
     k3 = si.ks3_cos(2048, 56, 10)
     with pytest.raises(sw.SweptError):
         run(k3, 512)                      # three register rows per lane: n <= 256 (tests/test_gpu_ks3.py covers the rest)
-    b = si.heat_insulated(2048, 6, 55, 10)
+    tube = si.euler_sod(2048, 10)
     with pytest.raises(sw.SweptError):
-        run(b, 128)
+        run(tube, 128)                    # walls in this flavour: the heat problem only
