@@ -152,7 +152,8 @@ def main(argv=None):
     ap.add_argument("--steps", type=int, default=0, help="timesteps per run (0 = the config's own count)")
     ap.add_argument("--reps", type=int, default=2)
     ap.add_argument("--bc", default="periodic", choices=["periodic", "paper"],
-                    help="paper = insulated heat ends (B.5) / Dirichlet Euler tube (PAPER.md:377); TIER flavour only")
+                    help="paper = insulated heat ends (B.5) / Dirichlet Euler tube (PAPER.md:377): every flavour that applies "
+                         "walls (heat: TIER, hybrid CHAR, FLOW, CLUSTER; Euler: TIER)")
     ap.add_argument("--csv", default="")
     ap.add_argument("--probes", action="store_true", help="print the probe measurements instead of a sweep")
     ap.add_argument("--flow-profile", action="store_true", help="cycle shares of the FLOW kernel's task parts")
