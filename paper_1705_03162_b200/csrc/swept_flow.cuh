@@ -32,6 +32,7 @@
 #include "common.cuh"
 #include "functors.cuh"
 #include "swept_char.cuh"
+#include "swept_cluster.cuh"
 
 namespace swept {
 
@@ -164,10 +165,11 @@ __device__ __forceinline__ void fence_proxy_async_all() { asm volatile("fence.pr
 // a wall tile took 5.5 tile times); all loads of a tier are issued before its first store (a skip of the groups outside
 // the tier's range was tried: the branches serialise the loads and cost more than they save).
 // The wall tiles of successive rows depend on one another, so rows x (time of a wall tile) bounds the launch from
-// below.  A wall tile computes every point at every tier (1.8 x the arithmetic of a swept tile, whose skew wastes 11 %),
-// on a scheduler it shares with two sweeping warps: measured 1.75 (n = 256) to 2 (n = 512) tile times.  So the flavour
-// pays where a warp has more than twice as many tiles per row to do as there are rows per tile: N >= 2^21 (4.4e12
-// against 4.1e12 for the hybrid CHAR + TIER-walls path at N = 2^22; 2.9e12 against 3.0e12 at 2^20); the autotuner decides.
+// below.  Through shared memory a wall tile computes every point at every tier (1.8 x the arithmetic of a swept tile) on
+// a scheduler it shares with two sweeping warps: 1.6 (n = 256) to 2 (n = 512) tile times.  For n = 256 the tile is
+// therefore kept in the warp's REGISTERS (the B == 8 branch below: the CLUSTER flavour's tier): 0.9 tile times, and walls
+// cost nothing any more (insulated heat N = 2^20, n = 256: 3.54e12, the periodic run's figure; N = 2^17: 8.3e11 against
+// 4.5e11 through shared memory).
 template <class Prob, int B, int KIND>
 __device__ __forceinline__ void flow_wall_tile(typename Prob::R* rows, const int RS, const int pad, const int lane,
                                                const bool wl, const bool wr, const bool split,
@@ -176,6 +178,49 @@ __device__ __forceinline__ void flow_wall_tile(typename Prob::R* rows, const int
   static_assert(Prob::H == 1 && Prob::C == 1 && Prob::SIGMA == 1, "walls in the FLOW flavour: the heat problem");
   constexpr int n = 32 * B, m = n / 2;
   const int ntiers = KIND == KIND_UP ? m - 1 : (KIND == KIND_DOWN ? m : 2 * m - 1);
+  if constexpr (B == 8) {
+    // n = 256: the tile fits the warp's registers (8 points of both rows per lane): the tiers run as in the CLUSTER
+    // flavour (swept_cluster.cuh: one shuffle exchange per tier, no shared-memory round trip, no warp barrier), the
+    // walls are its lane selects.  The wall tiles of successive rows form the critical path at N <= 2^19, so their
+    // latency is what counts.
+    constexpr int P = B;
+    R v0[1][P], v1[1][P], hl0[1][1], hr0[1][1], hl1[1][1], hr1[1][1];
+    R* r0 = rows + pad;
+    R* r1 = rows + RS + pad;
+#pragma unroll
+    for (int j = 0; j < P; ++j) {
+      v0[0][j] = r0[lane * P + j];
+      v1[0][j] = r1[lane * P + j];
+    }
+    hl0[0][0] = r0[-1]; hr0[0][0] = r0[n];
+    hl1[0][0] = r1[-1]; hr1[0][0] = r1[n];
+    int ta[P];
+    unsigned span[P];
+#pragma unroll
+    for (int j = 0; j < P; ++j) {  // tier window of each point (as swept_cluster_kernel)
+      const int x = lane * P + j;
+      const int d = x < n / 2 ? n / 2 - x : x - n / 2 + 1;
+      const int edge = x < n - 1 - x ? x : n - 1 - x;
+      const int t0 = KIND == KIND_UP ? 1 : d;
+      const int tb = KIND == KIND_UP ? edge : (KIND == KIND_DOWN ? m : 2 * m - d);
+      const bool never = tb < t0;
+      span[j] = never ? 0u : (unsigned)(tb - t0);
+      ta[j] = never ? (1 << 30) : t0;
+    }
+    const bool wall_l = split ? lane == 16 : (wl && lane == 0);
+    const bool wall_r = split ? lane == 15 : (wr && lane == 31);
+    for (int t = 1; t <= ntiers; t += 2) {
+      cluster_tier<Prob, P>(v0, v1, v0, hl0, hr0, 1, t, ta, span, lane, k, wall_l, wall_r);
+      if (t + 1 <= ntiers) cluster_tier<Prob, P>(v1, v0, v0, hl1, hr1, 0, t + 1, ta, span, lane, k, wall_l, wall_r);
+    }
+#pragma unroll
+    for (int j = 0; j < P; ++j) {
+      r0[lane * P + j] = v0[0][j];
+      r1[lane * P + j] = v1[0][j];
+    }
+    __syncwarp();
+    return;
+  }
   for (int t = 1; t <= ntiers; ++t) {
     // (source and destination are different rows: all loads of a tier are issued before its first store)
     const R* __restrict__ src = rows + ((t - 1) & 1) * RS + pad;  // phases start on even tiers: odd tiers read row 0
