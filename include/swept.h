@@ -75,7 +75,8 @@ enum {
                              tier; the edges pass from row to row through distributed shared memory behind a
                              cluster barrier instead of global memory.
                              Periodic heat (FP64, FP32), KS and KS3 (three register rows per lane, n <= 256);
-                             n = 64, 128, 256, 512; N / n <= 256 tiles (128 for n >= 256); group = warps per CTA
+                             n = 64, 128, 256, 512 (heat also 32: one point per lane); N / n <= 256 tiles (128 for
+                             n >= 256); group = warps per CTA
                              (0 = as few as fit a cluster of 16 CTAs)                                      */
 };
 

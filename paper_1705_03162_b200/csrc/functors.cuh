@@ -22,6 +22,16 @@ namespace swept {
 
 __device__ __forceinline__ double fma_(double a, double b, double c) { return fma(a, b, c); }
 __device__ __forceinline__ float fma_(float a, float b, float c) { return fmaf(a, b, c); }
+// x = fma(a, b, c) where rel <= span (unsigned), x unchanged elsewhere: the same fma.rn, issued under a predicate, so that a
+// register-resident tier (swept_cluster.cuh) needs no select between its arithmetic and the next tier's shuffle
+__device__ __forceinline__ void fma_if_(double& x, double a, double b, double c, unsigned rel, unsigned span) {
+  asm("{\n\t.reg .pred p;\n\tsetp.le.u32 p, %4, %5;\n\t@p fma.rn.f64 %0, %1, %2, %3;\n\t}"
+      : "+d"(x) : "d"(a), "d"(b), "d"(c), "r"(rel), "r"(span));
+}
+__device__ __forceinline__ void fma_if_(float& x, float a, float b, float c, unsigned rel, unsigned span) {
+  asm("{\n\t.reg .pred p;\n\tsetp.le.u32 p, %4, %5;\n\t@p fma.rn.f32 %0, %1, %2, %3;\n\t}"
+      : "+f"(x) : "f"(a), "f"(b), "f"(c), "r"(rel), "r"(span));
+}
 __device__ __forceinline__ double sqrt_(double a) { return sqrt(a); }
 __device__ __forceinline__ float sqrt_(float a) { return sqrtf(a); }
 __device__ __forceinline__ double fabs_(double a) { return fabs(a); }
@@ -80,6 +90,20 @@ struct Heat {
                                                R (&out)[C][P], int /*odd*/, const Consts<R>& k) {
 #pragma unroll
     for (int j = 0; j < P; ++j) out[0][j] = point(win[0][j], win[0][j + 1], win[0][j + 2], k);
+  }
+  // the same stage written into dst where point j's relative tier lies in its window (rel[j] <= span[j]); the other
+  // points of dst keep their values.  Same expression tree as point(): the last operation alone carries the predicate.
+  static constexpr bool HAS_STAGE_IF = true;
+  template <int P>
+  __device__ __forceinline__ static void stage_if(const R (&win)[C][P + 2 * H], const R (&/*base*/)[C][P],
+                                                  R (&dst)[C][P], int /*odd*/, const Consts<R>& k,
+                                                  const unsigned (&rel)[P], const unsigned (&span)[P]) {
+#pragma unroll
+    for (int j = 0; j < P; ++j) {
+      const R s = win[0][j] + win[0][j + 2];
+      const R t = k.a1 * win[0][j + 1];
+      fma_if_(dst[0][j], k.a0, s, t, rel[j], span[j]);
+    }
   }
 };
 

@@ -65,7 +65,7 @@ inline int cluster_warps_per_cta(int64_t K, int n, int want) {
   for (int wpc : {1, 2, 4, 8, 16, 32}) {
     if (want ? wpc != want : (wpc < 4 && K > wpc)) continue;
     if (wpc > max_wpc || K % wpc || K / wpc > 16) continue;
-    if (cluster_smem_bytes<Prob>(wpc * n) > (size_t)200 * 1024) continue;
+    if (cluster_smem_bytes<Prob>(wpc * n) > (size_t)200 * 1024) continue;  // (the two-row kernel's buffers: + 2h per row)
     return wpc;
   }
   return 0;
@@ -73,7 +73,7 @@ inline int cluster_warps_per_cta(int64_t K, int n, int want) {
 
 template <class Prob>
 inline bool cluster_ok(int64_t N, int n, int want_wpc) {
-  if (n != 64 && n != 128 && n != 256 && n != 512) return false;
+  if (n != 64 && n != 128 && n != 256 && n != 512 && !(n == 32 && Prob::H == 1 && Prob::ROWS == 2)) return false;
   if (Prob::ROWS == 3 && n > 256) return false;  // three register rows per lane: at most 8 points each
   if (N % n || n / 32 < Prob::H || (n / (2 * Prob::H)) % 2) return false;
   return cluster_warps_per_cta<Prob>(N / n, n, want_wpc) != 0;
@@ -94,10 +94,11 @@ inline int cluster_go(const ClusterLaunch& a) {
   c.k = round_consts<R>(a.consts);
   c.bc = a.bc;
   if (a.bc && !(Prob::H == 1 && Prob::ROWS == 2 && a.bc == BC_MIRROR)) return NO_KERNEL;  // walls: the heat problem
-  const size_t smem = cluster_smem_bytes<Prob>(c.chunk);
+  const size_t smem = Prob::ROWS == 3 ? cluster_smem_bytes<Prob>(c.chunk) : cluster_push_smem_bytes<Prob>(wpc, a.n);
   void (*kern)(const ClusterArgs<R>) = nullptr;
   if constexpr (Prob::ROWS == 3) kern = swept_cluster3_kernel<Prob, P>;
-  else kern = swept_cluster_kernel<Prob, P>;
+  else if constexpr (Prob::H == 1) kern = a.bc ? swept_cluster_kernel<Prob, P, true> : swept_cluster_kernel<Prob, P, false>;
+  else kern = swept_cluster_kernel<Prob, P, false>;
   cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (e == cudaSuccess && cs > 8) e = cudaFuncSetAttribute(kern, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
   if (e != cudaSuccess) return (int)e;
@@ -126,6 +127,7 @@ template <class Prob>
 int cluster_T(const ClusterLaunch& a) {
   if (!cluster_ok<Prob>(a.N, a.n, a.warps_per_cta)) return NO_KERNEL;
   switch (a.n / 32) {
+    case 1: if constexpr (Prob::H == 1 && Prob::ROWS == 2) return cluster_go<Prob, 1>(a); break;
     case 2: return cluster_go<Prob, 2>(a);
     case 4: return cluster_go<Prob, 4>(a);
     case 8: return cluster_go<Prob, 8>(a);

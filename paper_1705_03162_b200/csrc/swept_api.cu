@@ -473,21 +473,26 @@ void default_tile(const swept_state* s, int* n_io, int* flavor_io, int* P_io) {
       return;
     }
   }
-  // ... on a medium one (2^14 <= N < 2^19, a multiple of 256) the same flavour at n = 256: with TMA staging the persistent
+  // ... on a medium one (2^15 <= N < 2^19, a multiple of 256) the same flavour at n = 256: with TMA staging the persistent
   // launch beats a launch per row of tiles from N = 2^14 up (profiles/r2_sweep_heat_f64.csv, r2_sweep_ks.csv)
   if (n == 0 && flavor == SWEPT_FLAVOR_AUTO && !s->bc && (s->problem == SWEPT_HEAT || s->problem == SWEPT_KS) &&
-      s->N >= (1 << 14) && s->N < (1 << 19) && tile_ok(s, SWEPT_FLAVOR_FLOW, 256, 0)) {
+      s->N >= (1 << 15) && s->N < (1 << 19) && tile_ok(s, SWEPT_FLAVOR_FLOW, 256, 0)) {
     *n_io = 256;
     *flavor_io = SWEPT_FLAVOR_FLOW;
     *P_io = 0;
     return;
   }
-  // ... and on a small one (N <= 8192: at most 64 warp-sized tiles), where every flavour is bound by the latency of
-  // the dependent tiers, the CLUSTER flavour: one launch per cycle, rows chained through distributed shared memory
-  const bool small_two_row = (s->problem == SWEPT_HEAT || s->problem == SWEPT_KS) && s->N <= 8192;
+  // ... and on a small one (N <= 2^14: at most 256 warp-sized tiles), where every flavour is bound by the latency of
+  // the dependent tiers, the CLUSTER flavour: one launch per cycle, a warp per tile in registers, the rows chained by
+  // stores into the next tile's shared memory.  Widths as measured (profiles/r2_sweep_*.csv): one warp per scheduler
+  // as long as the tiles fit a cluster that way.
+  const bool small_two_row = (s->problem == SWEPT_HEAT || s->problem == SWEPT_KS) && s->N <= (s->bc ? 8192 : 16384);
   const bool small_three_row = s->problem == SWEPT_KS3 && s->N <= 16384;  // measured: 1.5-2.2 x the TIER flavour there
   if (n == 0 && flavor == SWEPT_FLAVOR_AUTO && (!s->bc || s->problem == SWEPT_HEAT) && (small_two_row || small_three_row)) {
-    for (int cand : {s->N <= 4096 ? 64 : (s->N <= 8192 ? 128 : 256), 128, 256})
+    const int first = s->problem == SWEPT_HEAT  ? (s->N <= 8192 ? 64 : 256)
+                      : s->problem == SWEPT_KS ? (s->N <= 4096 ? 64 : 128)
+                                               : (s->N <= 4096 ? 64 : (s->N <= 8192 ? 128 : 256));
+    for (int cand : {first, 128, 256, 64})
       if (tile_ok(s, SWEPT_FLAVOR_CLUSTER, cand, 0)) {
         *n_io = cand;
         *flavor_io = SWEPT_FLAVOR_CLUSTER;
@@ -1334,7 +1339,7 @@ int swept_autotune(swept_state* s, int variant, int32_t* best_tile_width) {
       for (int fl : {SWEPT_FLAVOR_TIER, SWEPT_FLAVOR_CHAR})
         for (int P : {1, 2, 4, 8, 16, 32})
           if (tile_ok(s, fl, n, P)) cands.push_back({n, fl, P});
-    for (int n : {64, 128, 256, 512})
+    for (int n : {32, 64, 128, 256, 512})
       for (int wpc : {0, 4, 8, 16, 32})  // warps per CTA of the CLUSTER flavour (0 = the fewest that fit)
         if (tile_ok(s, SWEPT_FLAVOR_CLUSTER, n, wpc)) cands.push_back({n, SWEPT_FLAVOR_CLUSTER, wpc});
     for (int n : {256, 512, 1024})

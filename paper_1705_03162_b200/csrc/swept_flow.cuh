@@ -209,9 +209,10 @@ __device__ __forceinline__ void flow_wall_tile(typename Prob::R* rows, const int
     }
     const bool wall_l = split ? lane == 16 : (wl && lane == 0);
     const bool wall_r = split ? lane == 15 : (wr && lane == 31);
+    const TierLanes TL = tier_lanes(lane);
     for (int t = 1; t <= ntiers; t += 2) {
-      cluster_tier<Prob, P>(v0, v1, v0, hl0, hr0, 1, t, ta, span, lane, k, wall_l, wall_r);
-      if (t + 1 <= ntiers) cluster_tier<Prob, P>(v1, v0, v0, hl1, hr1, 0, t + 1, ta, span, lane, k, wall_l, wall_r);
+      cluster_tier<Prob, P, true>(v0, v1, v0, hl0, hr0, 1, t, ta, span, TL, k, wall_l, wall_r);
+      if (t + 1 <= ntiers) cluster_tier<Prob, P, true>(v1, v0, v0, hl1, hr1, 0, t + 1, ta, span, TL, k, wall_l, wall_r);
     }
 #pragma unroll
     for (int j = 0; j < P; ++j) {

@@ -39,8 +39,9 @@ KERNELS = [
     ("FLOW KS f64 n=1024", "swept_flow_kernelINS_2KSIdLi0EEELi32ELb0ELb0E"),
     ("CHAR heat f64 B=16 L=32 WholeDiamond", "swept_char_kernelINS_4HeatIdEELi16ELi32ELi2E"),
     ("CHAR KS f64 B=32 L=32 WholeDiamond", "swept_char_kernelINS_2KSIdLi0EEELi32ELi32ELi2E"),
-    ("CLUSTER heat f64 n=64 (P=2)", "swept_cluster_kernelINS_4HeatIdEELi2E"),
-    ("CLUSTER KS f64 n=128 (P=4)", "swept_cluster_kernelINS_2KSIdLi0EEELi4E"),
+    ("CLUSTER heat f64 n=64 (P=2), periodic", "swept_cluster_kernelINS_4HeatIdEELi2ELb0E"),
+    ("CLUSTER heat f64 n=64 (P=2), walls", "swept_cluster_kernelINS_4HeatIdEELi2ELb1E"),
+    ("CLUSTER KS f64 n=128 (P=4)", "swept_cluster_kernelINS_2KSIdLi0EEELi4ELb0E"),
     ("TIER heat f64 P=1 WholeDiamond", "swept_tier_kernelINS_4HeatIdEELi1ELi2E"),
     ("TIER Euler f64 Heun P=2 WholeDiamond", "swept_tier_kernelINS_5EulerIdLi1EEELi2ELi2E"),
     ("TIER KS3 f64 P=1 WholeDiamond", "swept_tier_kernelINS_3KS3IdEELi1ELi2E"),

@@ -16,7 +16,9 @@ CL = sw.FLAVOR_CLUSTER
 def admissible(problem, N, n, wpc, size=8):
     """The rules of include/swept.h / DESIGN.md §5.10, restated: which (N, n, warps per CTA) must run."""
     h, _, C = si.PROBLEM_SHAPE[problem]
-    if n not in (64, 128, 256, 512) or N % n or problem not in (si.HEAT, si.KS):
+    if n not in (32, 64, 128, 256, 512) or N % n or problem not in (si.HEAT, si.KS):
+        return False
+    if n == 32 and problem != si.HEAT:          # one point per lane: the three-point scheme only (a lane's block must hold h points)
         return False
     K, P = N // n, n // 32
     max_wpc = 8 if P >= 8 else 16
@@ -43,7 +45,7 @@ def test_heat_cluster_matches_oracle(N, nsteps):
     w = si.heat_sines(N, 8, 51, nsteps)
     ref = oracle.run_workload(w)
     ran = 0
-    for n in (64, 128, 256, 512):
+    for n in (32, 64, 128, 256, 512):
         for wpc in (0, 1, 4, 8, 16, 32):
             want = admissible(si.HEAT, N, n, wpc)
             try:
@@ -64,7 +66,7 @@ def test_ks_cluster_matches_oracle(N, nsteps, rk2):
     w.rk2 = rk2
     ref = oracle.run_workload(w)
     ran = 0
-    for n in (64, 128, 256, 512):
+    for n in (32, 64, 128, 256, 512):
         for wpc in (0, 8):
             want = admissible(si.KS, N, n, wpc)
             try:
@@ -89,7 +91,7 @@ def test_heat_insulated_ends_cluster(N, nsteps):
         w = si.heat_insulated(N, 6, 57, nsteps)
         ref = oracle.run_workload(w)
         ran = 0
-        for n in (64, 128, 256, 512):
+        for n in (32, 64, 128, 256, 512):
             for wpc in (0, 8):
                 if not admissible(si.HEAT, N, n, wpc):
                     continue
