@@ -72,8 +72,9 @@ enum {
                              (DESIGN.md §5.5).  heat and KS, n = 256, 512, 1024   */
   SWEPT_FLAVOR_CLUSTER = 4 /* small problems: the whole domain in ONE thread-block cluster, one launch per
                              Up..Down cycle; a warp per tile, its points in registers, one shuffle exchange per
-                             tier; the edges pass from row to row through distributed shared memory behind a
-                             cluster barrier instead of global memory.
+                             tier; a tile stores its edges straight into the shared memory of the warps that
+                             continue them (distributed shared memory, st.async + mbarrier) instead of global
+                             memory and a launch.
                              Periodic heat (FP64, FP32), KS and KS3 (three register rows per lane, n <= 256);
                              n = 64, 128, 256, 512 (heat also 32: one point per lane); N / n <= 256 tiles (128 for
                              n >= 256); group = warps per CTA
@@ -350,6 +351,12 @@ int swept_flow_profile(swept_state* s, int on, uint64_t* counters);
  * update puts on the critical path of every tier, i.e. the denominator of the latency bound that governs small N
  * (a tile of n points cannot advance faster than one tier per chain link). */
 int swept_probe_chain(int device, void* stream, double* cycles_per_dadd_dfma);
+
+/* swept_probe_tier — cycles per link of the dependent chain of a register-resident tier (the CLUSTER flavour, one warp,
+ * one point per lane), written to the caller's HOST array of 4 doubles: [0] shuffle -> shuffle; [1] both neighbours by
+ * 64-bit shuffles -> DADD -> DFMA; [2] the same -> select on the tier window, i.e. one whole heat tier; [3] DFMA ->
+ * select.  [2] is the floor of that flavour's time per tier. */
+int swept_probe_tier(int device, void* stream, double* cycles4);
 
 /* swept_probe_smem — shared-memory read bandwidth of the whole device (conflict-free 16-byte loads from 32 KiB per
  * CTA, 2 CTAs of 1024 threads per SM), in bytes per second and, if the pointer is given, bytes per clock and SM at

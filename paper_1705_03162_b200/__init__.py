@@ -114,6 +114,7 @@ def load():
     lib.swept_probe_fp64.argtypes = [c_int, c_void_p, POINTER(c_double)]
     lib.swept_probe_launch.argtypes = [c_int, c_void_p, c_int, POINTER(c_double)]
     lib.swept_probe_chain.argtypes = [c_int, c_void_p, POINTER(c_double)]
+    lib.swept_probe_tier.argtypes = [c_int, c_void_p, POINTER(c_double)]
     lib.swept_probe_smem.argtypes = [c_int, c_void_p, POINTER(c_double), POINTER(c_double)]
     lib.swept_probe_sweep.argtypes = [c_int, c_void_p, c_int, c_int, c_int, POINTER(c_double), POINTER(c_double)]
     lib.swept_flow_profile.argtypes = [c_void_p, c_int, POINTER(c_uint64)]
@@ -302,6 +303,14 @@ def swept_probe_chain(device: int = -1) -> float:
     out = c_double(0)
     _check(load().swept_probe_chain(device, _current_stream(), byref(out)))
     return float(out.value)
+
+
+def swept_probe_tier(device: int = -1):
+    """Cycles per link of a register-resident tier's dependent chain: (shuffle -> shuffle, two 64-bit shuffles -> DADD
+    -> DFMA, the same -> select = one heat tier, DFMA -> select)."""
+    out = (c_double * 4)()
+    _check(load().swept_probe_tier(device, _current_stream(), out))
+    return tuple(float(x) for x in out)
 
 
 def swept_probe_smem(device: int = -1):

@@ -94,7 +94,7 @@ inline int cluster_go(const ClusterLaunch& a) {
   c.k = round_consts<R>(a.consts);
   c.bc = a.bc;
   if (a.bc && !(Prob::H == 1 && Prob::ROWS == 2 && a.bc == BC_MIRROR)) return NO_KERNEL;  // walls: the heat problem
-  const size_t smem = Prob::ROWS == 3 ? cluster_smem_bytes<Prob>(c.chunk) : cluster_push_smem_bytes<Prob>(wpc, a.n);
+  const size_t smem = cluster_push_smem_bytes<Prob>(wpc, a.n);
   void (*kern)(const ClusterArgs<R>) = nullptr;
   if constexpr (Prob::ROWS == 3) kern = swept_cluster3_kernel<Prob, P>;
   else if constexpr (Prob::H == 1) kern = a.bc ? swept_cluster_kernel<Prob, P, true> : swept_cluster_kernel<Prob, P, false>;

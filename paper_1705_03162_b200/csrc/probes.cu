@@ -44,6 +44,34 @@ __global__ void __launch_bounds__(32) dep_chain_kernel(double* sink, int iters, 
   if (x == 123.456) sink[0] = x;
 }
 
+// ---- the dependent chain of a REGISTER-RESIDENT tier (swept_cluster.cuh), one warp, one point per lane:
+// MODE 0: shuffle -> shuffle; 1: both neighbours by 64-bit shuffles -> DADD -> DFMA; 2: the same -> select on the tier
+// window (a whole heat tier); 3: DFMA -> select
+template <int MODE>
+__global__ void __launch_bounds__(32) tier_chain_kernel(double* sink, int iters, double a0, double a1, int span,
+                                                        long long* cycles) {
+  const int lane = threadIdx.x & 31;
+  double u = (double)lane * 1e-3;
+  int w = lane;
+  const int sl = (lane + 31) & 31, sr = (lane + 1) & 31;
+  const long long t0 = clock64();
+  for (int i = 0; i < iters; ++i) {
+    if (MODE == 0) w = __shfl_sync(0xffffffffu, w, sr);
+    if (MODE == 1) u = fma(a0, __shfl_sync(0xffffffffu, u, sl) + __shfl_sync(0xffffffffu, u, sr), a1 * u);
+    if (MODE == 2) {
+      const double o = fma(a0, __shfl_sync(0xffffffffu, u, sl) + __shfl_sync(0xffffffffu, u, sr), a1 * u);
+      u = (unsigned)(i - lane) <= (unsigned)span ? o : u;
+    }
+    if (MODE == 3) {
+      const double o = fma(a0, u, a1);
+      u = (unsigned)(i - lane) <= (unsigned)span ? o : u;
+    }
+  }
+  const long long t1 = clock64();
+  if (threadIdx.x == 0) cycles[0] = t1 - t0;
+  if (u + w == 123.456) sink[0] = u;
+}
+
 // ---- shared-memory bandwidth: every thread streams conflict-free 16-byte loads from its CTA's shared memory
 // (integer XORs keep the loaded values alive without touching the FP64 pipe)
 __global__ void __launch_bounds__(1024) smem_read_int_kernel(unsigned* sink, int iters) {
@@ -182,6 +210,30 @@ int swept_probe_chain(int device, void* stream_, double* cycles_per_dadd_dfma) {
   cudaFree(dc);
   if (e != cudaSuccess || e2 != cudaSuccess) return SWEPT_ECUDA;
   *cycles_per_dadd_dfma = (double)c / ((double)iters * 8);
+  return SWEPT_OK;
+}
+
+int swept_probe_tier(int device, void* stream_, double* cycles4) {
+  if (!cycles4) return SWEPT_EINVAL;
+  cudaStream_t stream = (cudaStream_t)stream_;
+  if (device >= 0 && cudaSetDevice(device) != cudaSuccess) return SWEPT_ECUDA;
+  double* sink = nullptr;
+  long long* dc = nullptr;
+  if (cudaMalloc(&sink, 8) != cudaSuccess || cudaMalloc(&dc, 4 * 8) != cudaSuccess) { cudaFree(sink); return SWEPT_ENOMEM; }
+  const int iters = 20000, span = 1 << 30;
+  long long c[4] = {0, 0, 0, 0};
+  for (int rep = 0; rep < 2; ++rep) {
+    tier_chain_kernel<0><<<1, 32, 0, stream>>>(sink, iters, 0.25, 0.5, span, dc + 0);
+    tier_chain_kernel<1><<<1, 32, 0, stream>>>(sink, iters, 0.25, 0.5, span, dc + 1);
+    tier_chain_kernel<2><<<1, 32, 0, stream>>>(sink, iters, 0.25, 0.5, span, dc + 2);
+    tier_chain_kernel<3><<<1, 32, 0, stream>>>(sink, iters, 0.25, 0.5, span, dc + 3);
+  }
+  const cudaError_t e = cudaMemcpyAsync(c, dc, 4 * 8, cudaMemcpyDeviceToHost, stream);
+  const cudaError_t e2 = cudaStreamSynchronize(stream);
+  cudaFree(sink);
+  cudaFree(dc);
+  if (e != cudaSuccess || e2 != cudaSuccess) return SWEPT_ECUDA;
+  for (int i = 0; i < 4; ++i) cycles4[i] = (double)c[i] / (double)iters;
   return SWEPT_OK;
 }
 

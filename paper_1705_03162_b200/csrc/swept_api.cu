@@ -486,7 +486,7 @@ void default_tile(const swept_state* s, int* n_io, int* flavor_io, int* P_io) {
   // the dependent tiers, the CLUSTER flavour: one launch per cycle, a warp per tile in registers, the rows chained by
   // stores into the next tile's shared memory.  Widths as measured (profiles/r2_sweep_*.csv): one warp per scheduler
   // as long as the tiles fit a cluster that way.
-  const bool small_two_row = (s->problem == SWEPT_HEAT || s->problem == SWEPT_KS) && s->N <= (s->bc ? 8192 : 16384);
+  const bool small_two_row = (s->problem == SWEPT_HEAT || s->problem == SWEPT_KS) && s->N <= 16384;
   const bool small_three_row = s->problem == SWEPT_KS3 && s->N <= 16384;  // measured: 1.5-2.2 x the TIER flavour there
   if (n == 0 && flavor == SWEPT_FLAVOR_AUTO && (!s->bc || s->problem == SWEPT_HEAT) && (small_two_row || small_three_row)) {
     const int first = s->problem == SWEPT_HEAT  ? (s->N <= 8192 ? 64 : 256)

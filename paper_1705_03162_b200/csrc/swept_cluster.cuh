@@ -14,7 +14,7 @@
 //     (the edges a node passes on) — st.async through the cluster's distributed shared memory, possibly
 //     into a neighbouring SM, each store counting its bytes on the receiver's mbarrier.  The receiver waits on its own
 //     barrier for its two producers only and reads its own shared memory: no cluster-wide barrier, no fence, no remote
-//     load between rows (the first version had all three: 1.3 k cycles per row; swept_cluster3_kernel still has).
+//     load between rows (the first version had all three: 1.3 k cycles per row).
 //     Global memory is touched twice: the Up row reads the time level, the Down row writes it.
 //   * receive buffers ping-pong with the row's parity; a buffer is rewritten only by tiles that consumed this warp's
 //     output of the row that read it (see the hand-off comment below).
@@ -400,30 +400,60 @@ __global__ void __launch_bounds__(ClusterMaxThreads<P>::value) swept_cluster3_ke
   static_assert(Prob::ROWS == 3 && Prob::SIGMA == 3, "three sub-timesteps per timestep on three rows");
   static_assert(P >= H, "a lane's block must hold its neighbour's halo");
   constexpr int n = 32 * P, m = n / (2 * H);
+  constexpr int W = n + 2 * H;                          // slots per (row, component)
+  constexpr int BUF = 3 * C * W;                        // values per receive buffer: three rows
+  constexpr uint32_t TX = (uint32_t)(BUF * sizeof(R));  // bytes a tile receives per row of tiles
   extern __shared__ __align__(128) unsigned char smem_raw[];
-  R* sm = reinterpret_cast<R*>(smem_raw);  // [buffer 2][row 3][component C][chunk]
   cg::cluster_group cluster = cg::this_cluster();
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const int wpc = blockDim.x >> 5;
   const unsigned rank = cluster.block_rank();
   const int64_t N = a.N;
-  const int64_t k_tile = (int64_t)rank * wpc + warp;
-  const int chunk = a.chunk;
-  auto dsm = [&](int buf, int row, int c, int64_t g) -> R* {
-    const int i = (int)(g & (n - 1));
-    const int off = (int)(g & (chunk - 1)) - i + (i % P) * 32 + i / P;  // lane-major inside the aligned block
-    R* local = sm + (size_t)((buf * 3 + row) * C + c) * chunk + off;
-    return cluster.map_shared_rank(local, (unsigned)(g >> a.chunk_log2));
+  const int K = (int)(N / n);
+  const int k_tile = (int)rank * wpc + warp;
+  // the pushed hand-off of swept_cluster_kernel (see there), with three rows per buffer
+  uint64_t* bars = reinterpret_cast<uint64_t*>(smem_raw);              // [warp][buffer]
+  R* recv = reinterpret_cast<R*>(smem_raw + cluster_bar_bytes(wpc));  // [warp][buffer][row 3][C][W]
+  const uint32_t smem_base = smem_u32(smem_raw);
+  auto bar_off = [&](int w, int b) -> uint32_t { return (uint32_t)((w * 2 + b) * 8); };
+  auto buf_off = [&](int w, int b) -> uint32_t {
+    return (uint32_t)cluster_bar_bytes(wpc) + (uint32_t)((w * 2 + b) * BUF * (int)sizeof(R));
   };
+  if (lane == 0) {
+    mbar_init(&bars[warp * 2 + 0], 1);
+    mbar_init(&bars[warp * 2 + 1], 1);
+  }
+  fence_mbar_init();
+  cluster.sync();
+  const int rows = a.rows;
+  if (lane == 0) {
+    if (rows > 1) mbar_arrive_expect_tx(&bars[warp * 2 + 0], TX);
+    if (rows > 2) mbar_arrive_expect_tx(&bars[warp * 2 + 1], TX);
+  }
   auto wrap = [&](int64_t g) -> int64_t { return g < 0 ? g + N : (g >= N ? g - N : g); };
+  uint32_t main_dst[2], main_bar[2], halo_dst[2], halo_bar[2];
+  const int wshift = 31 - __clz(wpc);
+#pragma unroll
+  for (int p = 0; p < 2; ++p) {
+    const int kL = p ? k_tile : (k_tile == 0 ? K - 1 : k_tile - 1);
+    const int kR = p ? (k_tile == K - 1 ? 0 : k_tile + 1) : k_tile;
+    const int mine = lane < 16 ? kL : kR, other = lane < 16 ? kR : kL;
+    main_bar[p] = mapa_u32(smem_base + bar_off(mine & (wpc - 1), p), (uint32_t)(mine >> wshift));
+    main_dst[p] = mapa_u32(smem_base + buf_off(mine & (wpc - 1), p), (uint32_t)(mine >> wshift)) +
+                  (uint32_t)((lane ^ 16) * sizeof(R));
+    halo_bar[p] = mapa_u32(smem_base + bar_off(other & (wpc - 1), p), (uint32_t)(other >> wshift));
+    halo_dst[p] = mapa_u32(smem_base + buf_off(other & (wpc - 1), p), (uint32_t)(other >> wshift)) +
+                  (uint32_t)((n + (lane == 16 ? H : 0)) * sizeof(R));
+  }
+  const R* recv_mine = recv + (size_t)(warp * 2) * BUF;
+  uint64_t* bars_mine = bars + warp * 2;
 
   R v[3][C][P], hl[3][C][H], hr[3][C][H];
-  for (int r = 0; r < a.rows; ++r) {
-    const int kind = r == 0 ? KIND_UP : (r == a.rows - 1 ? KIND_DOWN : KIND_WHOLE);
-    const int64_t S = wrap(k_tile * n + ((r & 1) ? n / 2 : 0));
-    const int64_t g0 = wrap(S + lane * P);
+  for (int r = 0; r < rows; ++r) {
+    const int kind = r == 0 ? KIND_UP : (r == rows - 1 ? KIND_DOWN : KIND_WHOLE);
     const int inb = (r + 1) & 1, outb = r & 1;
     if (kind == KIND_UP) {
+      const int64_t g0 = (int64_t)k_tile * n + lane * P;  // row 0 is an aligned row
 #pragma unroll
       for (int c = 0; c < C; ++c) {
 #pragma unroll
@@ -437,17 +467,20 @@ __global__ void __launch_bounds__(ClusterMaxThreads<P>::value) swept_cluster3_ke
           for (int row = 0; row < 3; ++row) hl[row][c][e] = hr[row][c][e] = (R)0;  // never used by a triangle
       }
     } else {
+      mbar_wait_warp_bounded(bars_mine + inb, (uint32_t)(((r - 1) >> 1) & 1));
+      if (lane == 0 && r + 2 < rows) mbar_arrive_expect_tx(bars_mine + inb, TX);  // the buffer's next use
+      const R* b0 = recv_mine + (size_t)inb * BUF;
 #pragma unroll
       for (int row = 0; row < 3; ++row)
 #pragma unroll
         for (int c = 0; c < C; ++c) {
-          const R* p = dsm(inb, row, c, g0);
+          const R* q = b0 + (size_t)(row * C + c) * W;
 #pragma unroll
-          for (int j = 0; j < P; ++j) v[row][c][j] = p[j * 32];
+          for (int j = 0; j < P; ++j) v[row][c][j] = q[j * 32 + lane];
 #pragma unroll
           for (int e = 0; e < H; ++e) {
-            hl[row][c][e] = *dsm(inb, row, c, wrap(S - H + e));
-            hr[row][c][e] = *dsm(inb, row, c, wrap(S + n + e));
+            hl[row][c][e] = q[n + e];
+            hr[row][c][e] = q[n + H + e];
           }
         }
     }
@@ -472,32 +505,50 @@ __global__ void __launch_bounds__(ClusterMaxThreads<P>::value) swept_cluster3_ke
     else if (q0 == 1) cluster3_tiers<Prob, P, 1>(v, hl, hr, ntiers, ta, span, lane, a.k);
     else cluster3_tiers<Prob, P, 2>(v, hl, hr, ntiers, ta, span, lane, a.k);
     if (kind == KIND_DOWN) {  // the cycle ends on a full timestep: row 0 is the time level
+      const int64_t S = wrap((int64_t)k_tile * n + ((r & 1) ? n / 2 : 0));
+      const int64_t g0 = wrap(S + lane * P);
 #pragma unroll
       for (int c = 0; c < C; ++c)
 #pragma unroll
         for (int j = 0; j < P; ++j) a.out[(int64_t)c * N + g0 + j] = v[0][c][j];
     } else {
+      {
+        const uint32_t bar = outb ? main_bar[1] : main_bar[0];
+        const uint32_t dst = outb ? main_dst[1] : main_dst[0];
 #pragma unroll
-      for (int row = 0; row < 3; ++row)
+        for (int row = 0; row < 3; ++row)
 #pragma unroll
-        for (int c = 0; c < C; ++c) {
-          R* p = dsm(outb, row, c, g0);
+          for (int c = 0; c < C; ++c)
 #pragma unroll
-          for (int j = 0; j < P; ++j) p[j * 32] = v[row][c][j];
-        }
-      cluster.sync();
+            for (int j = 0; j < P; ++j)
+              st_async_(dst + (uint32_t)(((row * C + c) * W + j * 32) * sizeof(R)), v[row][c][j], bar);
+      }
+      if (lane == 15 || lane == 16) {  // the h points next to the tile's centre are a neighbour consumer's halo
+        const uint32_t bar = outb ? halo_bar[1] : halo_bar[0];
+        const uint32_t dst = outb ? halo_dst[1] : halo_dst[0];
+#pragma unroll
+        for (int row = 0; row < 3; ++row)
+#pragma unroll
+          for (int c = 0; c < C; ++c)
+#pragma unroll
+            for (int e = 0; e < H; ++e) {
+              const R x = lane == 15 ? v[row][c][P - H + e] : v[row][c][e];
+              st_async_(dst + (uint32_t)(((row * C + c) * W + e) * sizeof(R)), x, bar);
+            }
+      }
     }
   }
-  cluster.sync();
+  cluster.sync();  // nobody leaves while a store into its shared memory may still be in flight
 }
 
-// the two-row kernel: per warp two barriers and two receive buffers of [2 rows][C][n + 2h]
+// per warp two barriers and two receive buffers of [ROWS][C][n + 2h] values
 template <class Prob>
 inline size_t cluster_push_smem_bytes(int wpc, int n) {
-  return (size_t)cluster_bar_bytes(wpc) + (size_t)wpc * 2 * 2 * Prob::C * (size_t)(n + 2 * Prob::H) * sizeof(typename Prob::R);
+  return (size_t)cluster_bar_bytes(wpc) +
+         (size_t)wpc * 2 * Prob::ROWS * Prob::C * (size_t)(n + 2 * Prob::H) * sizeof(typename Prob::R);
 }
 
-// the three-row kernel (barrier hand-off through point-indexed distributed shared memory)
+// (admission test of cluster_warps_per_cta: the buffers without their halo slots)
 template <class Prob>
 inline size_t cluster_smem_bytes(int chunk) {
   return (size_t)2 * Prob::ROWS * Prob::C * (size_t)chunk * sizeof(typename Prob::R);

@@ -83,6 +83,9 @@ def probes(emit):
     emit(f"probe,launch_us,{sw.swept_probe_launch(2000):.3f}")
     pair = sw.swept_probe_chain()
     emit(f"probe,dadd_dfma_pair_cycles,{pair:.2f},ns at max clock {pair / (props.clock_rate / 1e6):.2f}")
+    t = sw.swept_probe_tier()
+    emit(f"probe,register_tier_chain_cycles,{t[2]:.1f},shuffle->shuffle {t[0]:.1f},two 64-bit shuffles->DADD->DFMA {t[1]:.1f},"
+         f"DFMA->select {t[3]:.1f},[2] = one heat tier of the CLUSTER flavour (one point per lane) with nothing else in the way")
     bps, bpc = sw.swept_probe_smem()
     emit(f"probe,smem_read_bytes_per_s,{bps:.4e},bytes/clk/SM {bpc:.1f},of nominal 128 {bpc / 128:.3f}")
     emit("sweep_probe,problem,lines_per_lane,warps_per_scheduler,cycles_per_superstep,fp64_pipe_busy")

@@ -1,6 +1,6 @@
 """GPU parity for the CLUSTER flavour (include/swept.h SWEPT_FLAVOR_CLUSTER): the whole domain in one
-thread-block cluster, a warp per tile in registers, rows of tiles chained through distributed shared memory behind a
-cluster barrier (the device-side synchronisation PAPER.md:297-303 names as future work; the survey's row f2).  Same
+thread-block cluster, a warp per tile in registers, rows of tiles chained by stores into the next tiles' shared memory
+(st.async + mbarrier: the device-side synchronisation PAPER.md:297-303 names as future work; the survey's row f2).  Same
 functors as every other flavour, so the result must equal the oracle bit for bit."""
 import numpy as np
 import pytest
@@ -140,3 +140,11 @@ def test_cluster_refusals():
     tube = si.euler_sod(2048, 10)
     with pytest.raises(sw.SweptError):
         run(tube, 128)                    # walls in this flavour: the heat problem only
+
+
+def test_probe_tier_chain():
+    # the floor of this flavour's time per tier, measured by the library itself (include/swept.h swept_probe_tier):
+    # a shuffle round trip, the neighbour sum and the update, the window select — each link adds latency
+    t = sw.swept_probe_tier()
+    assert len(t) == 4 and all(x > 0 for x in t)
+    assert 10 < t[0] < 80 and t[0] < t[1] < t[2] < 300 and 8 < t[3] < 80
