@@ -490,7 +490,7 @@ void default_tile(const swept_state* s, int* n_io, int* flavor_io, int* P_io) {
   const bool small_three_row = s->problem == SWEPT_KS3 && s->N <= 16384;  // measured: 1.5-2.2 x the TIER flavour there
   if (n == 0 && flavor == SWEPT_FLAVOR_AUTO && (!s->bc || s->problem == SWEPT_HEAT) && (small_two_row || small_three_row)) {
     const int first = s->problem == SWEPT_HEAT  ? (s->N <= 8192 ? 64 : 256)
-                      : s->problem == SWEPT_KS ? (s->N <= 4096 ? 64 : 128)
+                      : s->problem == SWEPT_KS ? (s->N <= 8192 ? 64 : 256)
                                                : (s->N <= 4096 ? 64 : (s->N <= 8192 ? 128 : 256));
     for (int cand : {first, 128, 256, 64})
       if (tile_ok(s, SWEPT_FLAVOR_CLUSTER, cand, 0)) {

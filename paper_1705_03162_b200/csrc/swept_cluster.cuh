@@ -228,6 +228,9 @@ __global__ void __launch_bounds__(ClusterMaxThreads<P>::value) swept_cluster_ker
 
   R v0[C][P], v1[C][P];  // row 0 (even tiers) and row 1 (odd tiers) of this lane's P points
   R hl0[C][H], hr0[C][H], hl1[C][H], hr1[C][H];
+  int ta[P];           // tier window of each point of the lane (below), kept across the rows of one kind
+  unsigned span[P];
+  int window_kind = -1;
   for (int r = 0; r < rows; ++r) {
     const int kind = r == 0 ? KIND_UP : (r == rows - 1 ? KIND_DOWN : KIND_WHOLE);
     const int inb = (r + 1) & 1, outb = r & 1;
@@ -272,8 +275,8 @@ __global__ void __launch_bounds__(ClusterMaxThreads<P>::value) swept_cluster_ker
     // diamond (tier t covers the centre +- ht, then +- h(2m-t)): ceil(d/h) .. 2m - ceil(d/h) with d the
     // distance from the centre; Down: ceil(d/h) .. m.
     const int ntiers = kind == KIND_UP ? m - 1 : (kind == KIND_DOWN ? m : 2 * m - 1);
-    int ta[P];
-    unsigned span[P];
+    if (kind != window_kind) {  // the windows change with the kind of row only: three times per cycle
+      window_kind = kind;
 #pragma unroll
     for (int j = 0; j < P; ++j) {
       const int x = lane * P + j;
@@ -285,6 +288,7 @@ __global__ void __launch_bounds__(ClusterMaxThreads<P>::value) swept_cluster_ker
       const bool never = tb < t0;  // the end points of an UpTriangle's base row
       span[j] = never ? 0u : (unsigned)(tb - t0);
       ta[j] = never ? (1 << 30) : t0;
+    }
     }
     // (Two tiers behind one shuffle exchange — 2h redundant evaluations per lane instead of a second exchange — was
     // built and measured: no faster for the 3-point scheme, 3 % for the 5-point one; not kept.)
@@ -449,6 +453,9 @@ __global__ void __launch_bounds__(ClusterMaxThreads<P>::value) swept_cluster3_ke
   uint64_t* bars_mine = bars + warp * 2;
 
   R v[3][C][P], hl[3][C][H], hr[3][C][H];
+  int ta[P];
+  unsigned span[P];
+  int window_kind = -1;
   for (int r = 0; r < rows; ++r) {
     const int kind = r == 0 ? KIND_UP : (r == rows - 1 ? KIND_DOWN : KIND_WHOLE);
     const int inb = (r + 1) & 1, outb = r & 1;
@@ -485,8 +492,8 @@ __global__ void __launch_bounds__(ClusterMaxThreads<P>::value) swept_cluster3_ke
         }
     }
     const int ntiers = kind == KIND_UP ? m - 1 : (kind == KIND_DOWN ? m : 2 * m - 1);
-    int ta[P];
-    unsigned span[P];
+    if (kind != window_kind) {
+      window_kind = kind;
 #pragma unroll
     for (int j = 0; j < P; ++j) {  // tier window of each point: as in swept_cluster_kernel
       const int x = lane * P + j;
@@ -498,6 +505,7 @@ __global__ void __launch_bounds__(ClusterMaxThreads<P>::value) swept_cluster3_ke
       const bool never = tb < t0;
       span[j] = never ? 0u : (unsigned)(tb - t0);
       ta[j] = never ? (1 << 30) : t0;
+    }
     }
     // residue of the global tier this row of tiles starts at: the Up row at tier 0, diamond / Down row r at (r - 1) m
     const int q0 = r == 0 ? 0 : (int)(((int64_t)(r - 1) * m) % 3);
