@@ -464,8 +464,11 @@ void default_tile(const swept_state* s, int* n_io, int* flavor_io, int* P_io) {
   // CHAR flavour on wide tiles, Euler (about 250 live registers per point) with the TIER flavour
   // fully default call (no width, no flavour, nothing tuned) on a large periodic heat / KS problem: the persistent
   // FLOW launch at the width measured best on B200 (N >= 2^19)
-  if (n == 0 && flavor == SWEPT_FLAVOR_AUTO && !s->bc && (s->problem == SWEPT_HEAT || s->problem == SWEPT_KS) && s->N >= (1 << 19)) {
-    const int cand = s->problem == SWEPT_HEAT ? 512 : 1024;
+  // (the heat problem also with the paper's insulated ends: the wall tiles run inside the persistent launch, §5.8; n = 256
+  // keeps them in registers and wins up to N = 2^20, profiles/r2_sweep_bc_heat.csv)
+  const bool flow_default = (s->problem == SWEPT_HEAT || s->problem == SWEPT_KS) && (!s->bc || s->problem == SWEPT_HEAT);
+  if (n == 0 && flavor == SWEPT_FLAVOR_AUTO && flow_default && s->N >= (1 << 19)) {
+    const int cand = s->problem == SWEPT_HEAT ? ((s->bc && s->N < (1 << 21)) ? 256 : 512) : 1024;
     if (tile_ok(s, SWEPT_FLAVOR_FLOW, cand, 0)) {
       *n_io = cand;
       *flavor_io = SWEPT_FLAVOR_FLOW;
@@ -475,7 +478,7 @@ void default_tile(const swept_state* s, int* n_io, int* flavor_io, int* P_io) {
   }
   // ... on a medium one (2^15 <= N < 2^19, a multiple of 256) the same flavour at n = 256: with TMA staging the persistent
   // launch beats a launch per row of tiles from N = 2^14 up (profiles/r2_sweep_heat_f64.csv, r2_sweep_ks.csv)
-  if (n == 0 && flavor == SWEPT_FLAVOR_AUTO && !s->bc && (s->problem == SWEPT_HEAT || s->problem == SWEPT_KS) &&
+  if (n == 0 && flavor == SWEPT_FLAVOR_AUTO && flow_default &&
       s->N >= (1 << 15) && s->N < (1 << 19) && tile_ok(s, SWEPT_FLAVOR_FLOW, 256, 0)) {
     *n_io = 256;
     *flavor_io = SWEPT_FLAVOR_FLOW;

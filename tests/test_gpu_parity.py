@@ -433,6 +433,17 @@ def test_phase_timing_and_fully_default_run():
         assert np.array_equal(got, ps)
 
 
+def test_default_run_with_insulated_ends_medium_and_large():
+    # swept_run(state, nsteps, 0, SWEPT) with nothing tuned on the heat problem with the paper's own ends (B.5): the
+    # persistent FLOW launch from N = 2^15 up (wall tiles inside the launch), i.e. a handful of launches, not one per row
+    for N, steps in ((1 << 15, 700), (1 << 19, 300), (1 << 21, 520)):
+        w = si.heat_insulated(N, 6, 71, steps)
+        got, launches = gpu_run(w, steps, sw.SWEPT)
+        ref = oracle.run_workload(w) if N <= (1 << 19) else gpu_run(w, steps, sw.PER_STEP)[0]
+        assert np.array_equal(got, ref), N
+        assert launches <= 24, (N, launches)
+
+
 def test_error_codes():
     w = si.heat_sines(4096, 8, 2, 0)
     s = sw.Swept.from_workload(w)
