@@ -455,8 +455,8 @@ def main():
 
 
 def problem_table(torch, sw, flush, hbm):
-    """Swept vs per-step for the three PDEs at N = 2^20 (configs 2-4 shapes, shortened runs) and the HBM-bound
-    per-step regime at N = 2^26 (config 5's largest size)."""
+    """Swept vs per-step for the three PDEs at N = 2^20 (configs 2-4 shapes, shortened runs), config 1 (N = 2048) and
+    the HBM-bound per-step regime at N = 2^26 (config 5's largest size)."""
     rows = []
     cases = [("heat", si.config(2, N=1 << 20, nsteps=10000)), ("ks", si.config(3, N=1 << 20, nsteps=4000)),
              ("euler_heun", si.config(4, N=1 << 20, nsteps=1000))]
@@ -471,6 +471,16 @@ def problem_table(torch, sw, flush, hbm):
                      "swept_updates_per_s": w.N * w.nsteps / (sx * 1e-3),
                      "per_step_updates_per_s": w.N * w.nsteps / (ps * 1e-3), "speedup": ps / sx})
         st.close()
+    # BASELINE.json configs[0] (heat N = 2048, 20 000 steps): the latency-bound end, library defaults (CLUSTER flavour)
+    w = si.config(1)
+    st = sw.Swept.from_workload(w)
+    sx = min(time_runs(torch, sw, st, w, w.nsteps, 0, sw.SWEPT, sw.FLAVOR_AUTO, 0, reps=2, flush=flush))
+    ps = min(time_runs(torch, sw, st, w, w.nsteps, 0, sw.PER_STEP, 0, 0, reps=2, flush=flush))
+    rows.append({"problem": "heat_config1", "N": w.N, "nsteps": w.nsteps, "tile_width": 0, "flavor": sw.FLAVOR_AUTO,
+                 "note": "untuned library default: one thread-block cluster, a warp per tile in registers (DESIGN.md 5.10)",
+                 "swept_updates_per_s": w.N * w.nsteps / (sx * 1e-3), "swept_ns_per_timestep": sx * 1e6 / w.nsteps,
+                 "per_step_updates_per_s": w.N * w.nsteps / (ps * 1e-3), "speedup": ps / sx})
+    st.close()
     # HBM-bound per-step: N = 2^26 heat FP64 (512 MiB per array > L2)
     w = si.heat_sines(1 << 26, 16, si.BASE_SEED + 5, 200)
     st = sw.Swept.from_workload(w)
