@@ -88,9 +88,6 @@ inline int cluster_go(const ClusterLaunch& a) {
   const int cs = (int)(K / wpc);
   ClusterArgs<R> c;
   c.init = (const R*)a.init; c.out = (R*)a.out; c.N = a.N; c.n = a.n; c.rows = a.rows;
-  c.chunk = wpc * a.n;
-  c.chunk_log2 = 0;
-  while ((1 << c.chunk_log2) < c.chunk) ++c.chunk_log2;
   c.k = round_consts<R>(a.consts);
   c.bc = a.bc;
   if (a.bc && !(Prob::H == 1 && Prob::ROWS == 2 && a.bc == BC_MIRROR)) return NO_KERNEL;  // walls: the heat problem

@@ -40,8 +40,6 @@ struct ClusterArgs {
   int64_t N;
   int n;          // tile width = 32 P
   int rows;       // D + 2
-  int chunk;      // points per CTA = warps per CTA * n (a power of two)
-  int chunk_log2;
   Consts<R> k;
   int bc = 0;  // BC_MIRROR: insulated ends (heat, Eq. (B.5)), applied by the lanes next to a wall
 };
