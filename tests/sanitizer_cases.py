@@ -49,10 +49,14 @@ def cases():
     yield "heat FLOW n=512 TMA", heat_flow, sw.SWEPT, 512, F, 16
     yield "heat CLUSTER n=64", heat, sw.SWEPT, 64, sw.FLAVOR_CLUSTER, 0
     yield "heat CLUSTER n=256 (one CTA)", heat, sw.SWEPT, 256, sw.FLAVOR_CLUSTER, 8
+    yield "heat CLUSTER n=32 (16 CTAs)", heat, sw.SWEPT, 32, sw.FLAVOR_CLUSTER, 4
+    yield "heat CLUSTER n=64 one tile", si.heat_sines(64, 4, 38, 150), sw.SWEPT, 64, sw.FLAVOR_CLUSTER, 0
     yield "heat walls TIER n=256", wall, sw.SWEPT, 256, T, 1
     yield "heat walls hybrid CHAR n=256", wall, sw.SWEPT, 256, C, 32
     yield "heat walls FLOW n=256", si.heat_insulated(4096, 6, 37, 300), sw.SWEPT, 256, F, 0
     yield "heat walls CLUSTER n=128", wall, sw.SWEPT, 128, sw.FLAVOR_CLUSTER, 0
+    yield "heat walls CLUSTER n=64 (source lanes)", wall, sw.SWEPT, 64, sw.FLAVOR_CLUSTER, 0
+    yield "heat walls CLUSTER n=32 (source lanes)", wall, sw.SWEPT, 32, sw.FLAVOR_CLUSTER, 0
     yield "heat walls per_step", wall, sw.PER_STEP, 0, 0, 0
     yield "heat walls per_step resident", wall, sw.PER_STEP, 0, sw.PS_RESIDENT, 0
     yield "ks per_step (fused stages)", ks, sw.PER_STEP, 0, 0, 0
@@ -63,6 +67,7 @@ def cases():
     yield "ks FLOW n=256", ks_flow, sw.SWEPT, 256, F, 0
     yield "ks FLOW n=512 TMA", ks_flow, sw.SWEPT, 512, F, 16
     yield "ks CLUSTER n=128", ks, sw.SWEPT, 128, sw.FLAVOR_CLUSTER, 0
+    yield "ks CLUSTER n=64 two warps per scheduler", ks, sw.SWEPT, 64, sw.FLAVOR_CLUSTER, 8
     yield "ks3 per_step", ks3, sw.PER_STEP, 0, 0, 0
     yield "ks3 TIER n=128 P=1", ks3, sw.SWEPT, 128, T, 1
     yield "ks3 TIER n=256 P=2", ks3, sw.SWEPT, 256, T, 2
