@@ -145,6 +145,7 @@ def test_cluster_refusals():
 def test_probe_tier_chain():
     # the floor of this flavour's time per tier, measured by the library itself (include/swept.h swept_probe_tier):
     # a shuffle round trip, the neighbour sum and the update, the window select — each link adds latency
-    t = sw.swept_probe_tier()
+    runs = [sw.swept_probe_tier() for _ in range(3)]
+    t = tuple(min(r[i] for r in runs) for i in range(4))   # a pre-empted run reads high: the minimum is the latency
     assert len(t) == 4 and all(x > 0 for x in t)
     assert 10 < t[0] < 80 and t[0] < t[1] < t[2] < 300 and 8 < t[3] < 80
