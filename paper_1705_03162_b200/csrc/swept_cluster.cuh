@@ -276,17 +276,17 @@ __global__ void __launch_bounds__(ClusterMaxThreads<P>::value) swept_cluster_ker
     if (kind != window_kind) {  // the windows change with the kind of row only: three times per cycle
       window_kind = kind;
 #pragma unroll
-    for (int j = 0; j < P; ++j) {
-      const int x = lane * P + j;
-      const int d = x < n / 2 ? n / 2 - x : x - n / 2 + 1;
-      const int first = (d + H - 1) / H;
-      const int edge = (x < n - 1 - x ? x : n - 1 - x) / H;
-      const int t0 = kind == KIND_UP ? 1 : first;
-      const int tb = kind == KIND_UP ? edge : (kind == KIND_DOWN ? m : 2 * m - first);
-      const bool never = tb < t0;  // the end points of an UpTriangle's base row
-      span[j] = never ? 0u : (unsigned)(tb - t0);
-      ta[j] = never ? (1 << 30) : t0;
-    }
+      for (int j = 0; j < P; ++j) {
+        const int x = lane * P + j;
+        const int d = x < n / 2 ? n / 2 - x : x - n / 2 + 1;
+        const int first = (d + H - 1) / H;
+        const int edge = (x < n - 1 - x ? x : n - 1 - x) / H;
+        const int t0 = kind == KIND_UP ? 1 : first;
+        const int tb = kind == KIND_UP ? edge : (kind == KIND_DOWN ? m : 2 * m - first);
+        const bool never = tb < t0;  // the end points of an UpTriangle's base row
+        span[j] = never ? 0u : (unsigned)(tb - t0);
+        ta[j] = never ? (1 << 30) : t0;
+      }
     }
     // (Two tiers behind one shuffle exchange — 2h redundant evaluations per lane instead of a second exchange — was
     // built and measured: no faster for the 3-point scheme, 3 % for the 5-point one; not kept.)
@@ -493,17 +493,17 @@ __global__ void __launch_bounds__(ClusterMaxThreads<P>::value) swept_cluster3_ke
     if (kind != window_kind) {
       window_kind = kind;
 #pragma unroll
-    for (int j = 0; j < P; ++j) {  // tier window of each point: as in swept_cluster_kernel
-      const int x = lane * P + j;
-      const int d = x < n / 2 ? n / 2 - x : x - n / 2 + 1;
-      const int first = (d + H - 1) / H;
-      const int edge = (x < n - 1 - x ? x : n - 1 - x) / H;
-      const int t0 = kind == KIND_UP ? 1 : first;
-      const int tb = kind == KIND_UP ? edge : (kind == KIND_DOWN ? m : 2 * m - first);
-      const bool never = tb < t0;
-      span[j] = never ? 0u : (unsigned)(tb - t0);
-      ta[j] = never ? (1 << 30) : t0;
-    }
+      for (int j = 0; j < P; ++j) {  // tier window of each point: as in swept_cluster_kernel
+        const int x = lane * P + j;
+        const int d = x < n / 2 ? n / 2 - x : x - n / 2 + 1;
+        const int first = (d + H - 1) / H;
+        const int edge = (x < n - 1 - x ? x : n - 1 - x) / H;
+        const int t0 = kind == KIND_UP ? 1 : first;
+        const int tb = kind == KIND_UP ? edge : (kind == KIND_DOWN ? m : 2 * m - first);
+        const bool never = tb < t0;
+        span[j] = never ? 0u : (unsigned)(tb - t0);
+        ta[j] = never ? (1 << 30) : t0;
+      }
     }
     // residue of the global tier this row of tiles starts at: the Up row at tier 0, diamond / Down row r at (r - 1) m
     const int q0 = r == 0 ? 0 : (int)(((int64_t)(r - 1) * m) % 3);
